@@ -1,0 +1,441 @@
+/*
+ * rumd_oracle.c -- fp64 CPU oracle for the RUMD short-range pair-interaction hot path.
+ *
+ * THIS FILE IS TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only tests/, __graft_entry__.smoke()
+ * and bench.py's cpu_baseline / --impl reference legs may build, load or call it.  It shares
+ * no source, header, constant or helper with the CUDA path (paper_1506_05094_b200/csrc) and
+ * neither imports the other.
+ *
+ * What it is: a plain, slow, obviously-correct double-precision restatement of what the path
+ * computes, written from /root/reference/PAPER.md ("P:n" = PAPER.md line n) and, where the
+ * paper prints no equation, from the readings listed in SURVEY.md 8(c) (O1..O10, S1..S28),
+ * which DESIGN.md repeats.  No blocking, no fusion, no reordering: one function per definition.
+ *
+ * Pins (tests/test_oracle_pins.py, -m "not gpu"):
+ *   orc_lj_raw / orc_lj_sf / orc_coulomb_sf : closed forms (u(2^(1/6) s) = -e, 0.4^6 = 0.004096
+ *       constants), force = -du/dr by central differences, continuity at rc.
+ *   orc_forces_allpairs / orc_forces_list   : Newton's third law, translation / relabelling
+ *       invariance, static fcc / rock-salt lattice sums (tests/golden/lattice_sums.txt),
+ *       brute force == list based, independence of the skin.
+ *   orc_nblist_n2 / orc_nblist_cell         : agree with each other, symmetric, lattice shell counts.
+ *   orc_integrate (NVE)                     : time reversibility, momentum conservation,
+ *       energy fluctuation ~ dt^2, small drift.
+ *   orc_integrate (NVT)                     : tau -> inf reproduces NVE bit for bit, conserved
+ *       quantity H fluctuation ~ dt^2, <T_kin> -> T0.  The discretisation itself is a reading
+ *       (S9): "parity unpinned" against the paper for NVT trajectories (the paper prints no
+ *       Nose-Hoover equations).
+ *
+ * Conventions: positions r[3*i+k], velocities v[3*i+k], forces F[3*i+k]; box[3] = (Lx,Ly,Lz),
+ * orthorhombic, origin-centred, coordinates in [-L/2, L/2] (S7).  Potentials are one record of
+ * ORC_POT_STRIDE doubles per ORDERED type pair (a*ntypes+b):
+ *     pot[0]=epsilon pot[1]=sigma pot[2]=rc_LJ (<=0: no LJ term) pot[3]=k*qa*qb pot[4]=rc_Coulomb (<=0: none)
+ * rc values are ABSOLUTE distances (S2).
+ */
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define ORC_POT_STRIDE 5
+
+int orc_num_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+void orc_set_num_threads(int n)
+{
+#ifdef _OPENMP
+    if (n > 0) omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}
+
+/* ---------------------------------------------------------------- pair functions ------- */
+
+/* O3, unshifted 12-6 Lennard-Jones ("Pot_LJ_12_6"):
+ *   u(r) = 4 e [ (s/r)^12 - (s/r)^6 ],  f(r) = -du/dr = (24 e / r) [ 2 (s/r)^12 - (s/r)^6 ]. */
+void orc_lj_raw(double r, double eps, double sig, double *u, double *f)
+{
+    double sr = sig / r;
+    double sr6 = sr * sr * sr * sr * sr * sr;
+    double sr12 = sr6 * sr6;
+    *u = 4.0 * eps * (sr12 - sr6);
+    *f = 24.0 * eps * (2.0 * sr12 - sr6) / r;
+}
+
+/* O3, shifted-force cutoff ("truncation plus shift of the pair force [46] to ensure its
+ * continuity (this corresponds to adding a linear term in the potential)"):
+ *   r < rc : f_SF(r) = f(r) - f(rc),  u_SF(r) = u(r) - u(rc) + (r - rc) f(rc);  else both 0 (S3). */
+void orc_lj_sf(double r, double eps, double sig, double rc, double *u, double *f)
+{
+    if (r < rc) {
+        double ur, fr, uc, fc;
+        orc_lj_raw(r, eps, sig, &ur, &fr);
+        orc_lj_raw(rc, eps, sig, &uc, &fc);
+        *u = ur - uc + (r - rc) * fc;
+        *f = fr - fc;
+    } else {
+        *u = 0.0;
+        *f = 0.0;
+    }
+}
+
+/* O4, Coulomb with shifted-force cutoff ("Wolf ... alpha set to zero ... equivalent
+ * to the shifted force method"); no self term (S6):
+ *   u(r) = qq / r, f(r) = qq / r^2;  u_SF = qq [ 1/r - 1/rc + (r - rc)/rc^2 ],  f_SF = qq [ 1/r^2 - 1/rc^2 ]. */
+void orc_coulomb_sf(double r, double qq, double rc, double *u, double *f)
+{
+    if (r < rc) {
+        double ur = qq / r, fr = qq / (r * r);
+        double uc = qq / rc, fc = qq / (rc * rc);
+        *u = ur - uc + (r - rc) * fc;
+        *f = fr - fc;
+    } else {
+        *u = 0.0;
+        *f = 0.0;
+    }
+}
+
+/* S5: terms of different kinds on one type pair add; each applies its own rc. */
+void orc_pair_sf(const double *p, double r, double *u, double *f)
+{
+    double ut = 0.0, ft = 0.0, uu, ff;
+    if (p[2] > 0.0) {
+        orc_lj_sf(r, p[0], p[1], p[2], &uu, &ff);
+        ut += uu;
+        ft += ff;
+    }
+    if (p[4] > 0.0) {
+        orc_coulomb_sf(r, p[3], p[4], &uu, &ff);
+        ut += uu;
+        ft += ff;
+    }
+    *u = ut;
+    *f = ft;
+}
+
+/* S4/S5: interaction range of a type pair = max over its terms; list cutoff adds the skin. */
+double orc_pair_rc(const double *p)
+{
+    double rc = 0.0;
+    if (p[2] > rc) rc = p[2];
+    if (p[4] > rc) rc = p[4];
+    return rc;
+}
+
+/* ---------------------------------------------------------------- box ------------------ */
+
+/* O1: d_k -= L_k * nint(d_k / L_k). */
+void orc_min_image(double *d, const double *box)
+{
+    for (int k = 0; k < 3; ++k) d[k] -= box[k] * rint(d[k] / box[k]);
+}
+
+static double dist2_min_image(const double *ri, const double *rj, const double *box, double *d)
+{
+    d[0] = ri[0] - rj[0];
+    d[1] = ri[1] - rj[1];
+    d[2] = ri[2] - rj[2];
+    orc_min_image(d, box);
+    return d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
+}
+
+/* ---------------------------------------------------------------- forces --------------- */
+
+/* O5: F_i = sum_j f_SF(r_ij) d_ij / r_ij,  u_i = 1/2 sum_j u_SF(r_ij) (P:160 halving),
+ *     w_i = 1/2 sum_j r_ij f_SF(r_ij).  Adds one pair (i <- j) to the accumulators of i. */
+static void add_pair(const double *p, const double *d, double r2, double *Fi, double *ui, double *wi)
+{
+    double r = sqrt(r2), u, f;
+    orc_pair_sf(p, r, &u, &f);
+    Fi[0] += f * d[0] / r;
+    Fi[1] += f * d[1] / r;
+    Fi[2] += f * d[2] / r;
+    *ui += 0.5 * u;
+    *wi += 0.5 * r * f;
+}
+
+/* Brute force over ALL pairs j != i: no list, no cells (pin P4). */
+void orc_forces_allpairs(int N, const double *r, const int *type, const double *box, int nt,
+                         const double *pot, double *F, double *u, double *w)
+{
+#pragma omp parallel for schedule(static)
+    for (int i = 0; i < N; ++i) {
+        double Fi[3] = {0, 0, 0}, ui = 0, wi = 0, d[3];
+        for (int j = 0; j < N; ++j) {
+            if (j == i) continue;
+            const double *p = pot + ORC_POT_STRIDE * (type[i] * nt + type[j]);
+            double r2 = dist2_min_image(r + 3 * i, r + 3 * j, box, d);
+            double rc = orc_pair_rc(p);
+            if (r2 < rc * rc) add_pair(p, d, r2, Fi, &ui, &wi);
+        }
+        F[3 * i] = Fi[0];
+        F[3 * i + 1] = Fi[1];
+        F[3 * i + 2] = Fi[2];
+        u[i] = ui;
+        w[i] = wi;
+    }
+}
+
+/* Same sums restricted to a full Verlet list (both directions stored, no
+ * Newton's third law).  list is row-major here: k-th neighbour of i at list[i*cap + k]. */
+void orc_forces_list(int N, const double *r, const int *type, const double *box, int nt,
+                     const double *pot, int cap, const int *count, const int *list, double *F,
+                     double *u, double *w)
+{
+#pragma omp parallel for schedule(static)
+    for (int i = 0; i < N; ++i) {
+        double Fi[3] = {0, 0, 0}, ui = 0, wi = 0, d[3];
+        for (int k = 0; k < count[i]; ++k) {
+            int j = list[(size_t)i * cap + k];
+            const double *p = pot + ORC_POT_STRIDE * (type[i] * nt + type[j]);
+            double r2 = dist2_min_image(r + 3 * i, r + 3 * j, box, d);
+            double rc = orc_pair_rc(p);
+            if (r2 < rc * rc) add_pair(p, d, r2, Fi, &ui, &wi);
+        }
+        F[3 * i] = Fi[0];
+        F[3 * i + 1] = Fi[1];
+        F[3 * i + 2] = Fi[2];
+        u[i] = ui;
+        w[i] = wi;
+    }
+}
+
+/* ---------------------------------------------------------------- neighbour lists ------ */
+
+/* O2 (Fig. 4): NB(i) = { j != i : |d_ij|^2 < (rc_{ti tj} + s)^2 }, strict <, per type
+ * pair, full list.  O(N^2) double loop.  Returns the largest count found; entries beyond cap are
+ * dropped (count[i] still holds the true count, so max > cap signals overflow). */
+int orc_nblist_n2(int N, const double *r, const int *type, const double *box, int nt,
+                  const double *pot, double skin, int cap, int *count, int *list)
+{
+    int maxc = 0;
+#pragma omp parallel for schedule(static) reduction(max : maxc)
+    for (int i = 0; i < N; ++i) {
+        int c = 0;
+        double d[3];
+        for (int j = 0; j < N; ++j) {
+            if (j == i) continue;
+            double rcl = orc_pair_rc(pot + ORC_POT_STRIDE * (type[i] * nt + type[j])) + skin;
+            double r2 = dist2_min_image(r + 3 * i, r + 3 * j, box, d);
+            if (r2 < rcl * rcl) {
+                if (c < cap) list[(size_t)i * cap + c] = j;
+                ++c;
+            }
+        }
+        count[i] = c;
+        if (c > maxc) maxc = c;
+    }
+    return maxc;
+}
+
+/* Independent O(N) search ("cell-index method [1,2]"): textbook linked cells of edge
+ * >= max list cutoff, 27-cell stencil (NOT the paper's half-size cells / 125 stencil, which the CUDA
+ * path uses -- the two searches share nothing).  Needs >= 3 cells per axis; returns -1 otherwise. */
+int orc_nblist_cell(int N, const double *r, const int *type, const double *box, int nt,
+                    const double *pot, double skin, int cap, int *count, int *list)
+{
+    double rmax = 0.0;
+    for (int a = 0; a < nt * nt; ++a) {
+        double rc = orc_pair_rc(pot + ORC_POT_STRIDE * a);
+        if (rc > rmax) rmax = rc;
+    }
+    rmax += skin;
+    int nc[3];
+    for (int k = 0; k < 3; ++k) {
+        nc[k] = (int)floor(box[k] / rmax);
+        if (nc[k] < 3) return -1;
+    }
+    int ncell = nc[0] * nc[1] * nc[2];
+    int *head = (int *)malloc(sizeof(int) * (size_t)ncell);
+    int *next = (int *)malloc(sizeof(int) * (size_t)N);
+    int *cell = (int *)malloc(sizeof(int) * 3 * (size_t)N);
+    for (int c = 0; c < ncell; ++c) head[c] = -1;
+    for (int i = 0; i < N; ++i) {
+        int cc[3];
+        for (int k = 0; k < 3; ++k) {
+            /* wrapped coordinate in [0, L) */
+            double x = r[3 * i + k] - box[k] * floor(r[3 * i + k] / box[k] + 0.5) + 0.5 * box[k];
+            int c = (int)floor(x / box[k] * nc[k]);
+            if (c < 0) c = 0;
+            if (c >= nc[k]) c = nc[k] - 1;
+            cc[k] = c;
+            cell[3 * i + k] = c;
+        }
+        int ci = (cc[2] * nc[1] + cc[1]) * nc[0] + cc[0];
+        next[i] = head[ci];
+        head[ci] = i;
+    }
+    int maxc = 0;
+#pragma omp parallel for schedule(static) reduction(max : maxc)
+    for (int i = 0; i < N; ++i) {
+        int c = 0;
+        double d[3];
+        for (int dz = -1; dz <= 1; ++dz)
+            for (int dy = -1; dy <= 1; ++dy)
+                for (int dx = -1; dx <= 1; ++dx) {
+                    int cx = (cell[3 * i] + dx + nc[0]) % nc[0];
+                    int cy = (cell[3 * i + 1] + dy + nc[1]) % nc[1];
+                    int cz = (cell[3 * i + 2] + dz + nc[2]) % nc[2];
+                    for (int j = head[(cz * nc[1] + cy) * nc[0] + cx]; j >= 0; j = next[j]) {
+                        if (j == i) continue;
+                        double rcl =
+                            orc_pair_rc(pot + ORC_POT_STRIDE * (type[i] * nt + type[j])) + skin;
+                        double r2 = dist2_min_image(r + 3 * i, r + 3 * j, box, d);
+                        if (r2 < rcl * rcl) {
+                            if (c < cap) list[(size_t)i * cap + c] = j;
+                            ++c;
+                        }
+                    }
+                }
+        count[i] = c;
+        if (c > maxc) maxc = c;
+    }
+    free(head);
+    free(next);
+    free(cell);
+    return maxc;
+}
+
+/* O9 / S14 ("no particles have moved more than half the skin distance"; P:217 positions stored
+ * at build): 1 iff some |minimg(r_i - r_i^build)| > skin/2, strict. */
+int orc_needs_rebuild(int N, const double *r, const double *r_build, const double *box, double skin)
+{
+    double lim2 = 0.25 * skin * skin;
+    for (int i = 0; i < N; ++i) {
+        double d[3];
+        double r2 = dist2_min_image(r + 3 * i, r_build + 3 * i, box, d);
+        if (r2 > lim2) return 1;
+    }
+    return 0;
+}
+
+/* ---------------------------------------------------------------- integrators ---------- */
+
+#define ORC_NVE 0
+#define ORC_NVT 1
+
+/* One leap-frog step given F(t) (O6, O7, S7-S11; P:78 names the integrators, prints no equations).
+ *   NVE: v(t+dt/2) = v(t-dt/2) + dt F/m ;                         r(t+dt) = r(t) + dt v(t+dt/2)
+ *   NVT: v(t+dt/2) = [ (1 - xi dt/2) v(t-dt/2) + dt F/m ] / (1 + xi dt/2) ; same r update;
+ *        T_kin = sum m |v(t+dt/2)|^2 / g ; xi(t+dt) = xi + dt w2 (T_kin/T0 - 1), w2 = (2 pi / tau)^2
+ *        (tau <= 0 or inf: w2 = 0) ; eta(t+dt) = eta + dt/2 [xi(t) + xi(t+dt)].
+ *   wrap: n = nint(r/L); r -= L n; image += n  (S7).
+ * thermostat[0] = xi, thermostat[1] = eta (updated in place, NVT only).
+ * out[0] = K(t) = 1/2 sum m | (v_old + v_new)/2 |^2   (O10)
+ * out[1] = sum m |v(t+dt/2)|^2. */
+void orc_integrate(int N, double *r, double *v, const double *m, int *image, const double *F,
+                   const double *box, double dt, int mode, double T0, double tau, double g,
+                   double *thermostat, double *out)
+{
+    double xi = thermostat[0];
+    double Kt = 0.0, mv2 = 0.0;
+    for (int i = 0; i < N; ++i) {
+        for (int k = 0; k < 3; ++k) {
+            double vo = v[3 * i + k], vn;
+            if (mode == ORC_NVT)
+                vn = ((1.0 - 0.5 * xi * dt) * vo + dt * F[3 * i + k] / m[i]) / (1.0 + 0.5 * xi * dt);
+            else
+                vn = vo + dt * F[3 * i + k] / m[i];
+            double vh = 0.5 * (vo + vn);
+            Kt += 0.5 * m[i] * vh * vh;
+            mv2 += m[i] * vn * vn;
+            v[3 * i + k] = vn;
+            double x = r[3 * i + k] + dt * vn;
+            double n = rint(x / box[k]);
+            r[3 * i + k] = x - box[k] * n;
+            image[3 * i + k] += (int)n;
+        }
+    }
+    if (mode == ORC_NVT) {
+        double w2 = 0.0;
+        if (tau > 0.0 && isfinite(tau)) w2 = (2.0 * M_PI / tau) * (2.0 * M_PI / tau);
+        double xin = xi + dt * w2 * (mv2 / g / T0 - 1.0);
+        thermostat[1] += 0.5 * dt * (xi + xin);
+        thermostat[0] = xin;
+    }
+    out[0] = Kt;
+    out[1] = mv2;
+}
+
+/* O8 step order: (rebuild list if flag) -> F(r(t)) -> integrate -> displacement check sets the flag
+ * for the next step.  Runs nsteps from (r, v, image, thermostat), flag initially set.
+ * log (may be NULL): 6 doubles per step = U(t), K(t), W(t), xi(t), eta(t), H(t) where
+ *   H = K + U                                   (NVE)
+ *   H = K + U + g T0 xi^2 / (2 w2) + g T0 eta   (NVT, O10; the xi^2 term is dropped when w2 = 0).
+ * use_cell != 0 selects orc_nblist_cell (falls back to the N^2 search when the box is too small).
+ * Returns the number of list builds, or -1 on allocation failure. */
+long orc_run(int N, double *r, double *v, const double *m, int *image, const int *type,
+             const double *box, int nt, const double *pot, double skin, double dt, int mode,
+             double T0, double tau, double *thermostat, long nsteps, int use_cell, double *log)
+{
+    int cap = 64;
+    int *count = (int *)malloc(sizeof(int) * (size_t)N);
+    int *list = (int *)malloc(sizeof(int) * (size_t)N * cap);
+    double *rb = (double *)malloc(sizeof(double) * 3 * (size_t)N);
+    double *F = (double *)malloc(sizeof(double) * 3 * (size_t)N);
+    double *u = (double *)malloc(sizeof(double) * (size_t)N);
+    double *w = (double *)malloc(sizeof(double) * (size_t)N);
+    if (!count || !list || !rb || !F || !u || !w) return -1;
+    double g = 3.0 * N - 3.0; /* S10 */
+    double w2 = 0.0;
+    if (mode == ORC_NVT && tau > 0.0 && isfinite(tau)) w2 = (2.0 * M_PI / tau) * (2.0 * M_PI / tau);
+    int flag = 1;
+    long nbuild = 0;
+    for (long s = 0; s < nsteps; ++s) {
+        if (flag) {
+            for (;;) {
+                int mc = -1;
+                if (use_cell) mc = orc_nblist_cell(N, r, type, box, nt, pot, skin, cap, count, list);
+                if (mc < 0) mc = orc_nblist_n2(N, r, type, box, nt, pot, skin, cap, count, list);
+                if (mc <= cap) break;
+                /* "automatically re-allocated with doubled capacity" */
+                while (cap < mc) cap *= 2;
+                free(list);
+                list = (int *)malloc(sizeof(int) * (size_t)N * cap);
+                if (!list) return -1;
+            }
+            memcpy(rb, r, sizeof(double) * 3 * (size_t)N);
+            flag = 0;
+            ++nbuild;
+        }
+        orc_forces_list(N, r, type, box, nt, pot, cap, count, list, F, u, w);
+        double xi = thermostat[0], eta = thermostat[1], out[2];
+        orc_integrate(N, r, v, m, image, F, box, dt, mode, T0, tau, g, thermostat, out);
+        if (log) {
+            double U = 0.0, W = 0.0;
+            for (int i = 0; i < N; ++i) {
+                U += u[i];
+                W += w[i];
+            }
+            double H = out[0] + U;
+            if (mode == ORC_NVT) {
+                H += g * T0 * eta;
+                if (w2 > 0.0) H += 0.5 * g * T0 * xi * xi / w2;
+            }
+            double *l = log + 6 * s;
+            l[0] = U;
+            l[1] = out[0];
+            l[2] = W;
+            l[3] = xi;
+            l[4] = eta;
+            l[5] = H;
+        }
+        flag = orc_needs_rebuild(N, r, rb, box, skin);
+    }
+    free(count);
+    free(list);
+    free(rb);
+    free(F);
+    free(u);
+    free(w);
+    return nbuild;
+}
