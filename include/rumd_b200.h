@@ -1,0 +1,182 @@
+/*
+ * rumd_b200.h -- C ABI of librumd_b200.so: the per-timestep short-range pair-interaction hot path of RUMD
+ * (arxiv 1506.05094) re-designed for one NVIDIA B200 (sm_100a).
+ *
+ * Citations: "P:n" = line n of the paper text, "S n"/"O n" = the readings listed in DESIGN.md
+ * (section "Readings of the paper").  The call sequence mirrors the paper's user script (Fig. 1):
+ * create the simulation -> SetParams(i, j, Sigma, Epsilon, Rcut) per type pair -> set the integrator
+ * (timeStep, targetTemperature) -> Run(n).
+ *
+ * General rules
+ *   - Plain C: opaque handle, plain pointers and sizes.  Every pointer argument says "device" or "host".
+ *   - Every call returns a rumd_status; nothing throws, nothing exits.  rumd_last_error() gives a message.
+ *   - All bulk device memory is CALLER-OWNED (e.g. torch tensors): the state arrays (rumd_bind_state) and
+ *     one workspace blob (rumd_bind_workspace).  The library owns only the handle, CUDA graph objects,
+ *     events and a few pinned host scalars; rumd_destroy frees those and nothing else.
+ *   - All work is enqueued on the cudaStream_t given to rumd_create.  Calls are asynchronous unless they
+ *     say "synchronizes".  There is NO CPU fallback: without a CUDA device every compute call fails with
+ *     RUMD_ERR_CUDA.
+ *   - Asynchronous device-side conditions (neighbour-list overflow, P:218 / P:263 "set flag to inform
+ *     host"; non-finite energies) are sticky and surface at the next synchronizing call.
+ *   - Particle order is NOT stable: the cell method sorts particles spatially and permutes all state
+ *     arrays in place ("rearrange all particle data"); d_id[slot] = original particle index.
+ */
+#ifndef RUMD_B200_H
+#define RUMD_B200_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define RUMD_MAX_TYPES 4
+
+typedef struct rumd_system rumd_system; /* opaque; owned by the library */
+
+typedef enum {
+    RUMD_OK = 0,
+    RUMD_ERR_INVALID_ARG = 1,
+    RUMD_ERR_NOT_READY = 2,     /* state / workspace / potential / integrator not set yet */
+    RUMD_ERR_CUDA = 3,          /* a CUDA runtime call failed (no device, launch failure, ...) */
+    RUMD_ERR_NBL_OVERFLOW = 4,  /* some particle has more neighbours than the bound capacity */
+    RUMD_ERR_BOX_TOO_SMALL = 5, /* rc_max + skin > min(L)/2: minimum image not valid (O1) */
+    RUMD_ERR_NONFINITE = 6      /* energy is NaN/Inf */
+} rumd_status;
+
+typedef enum { RUMD_POT_LJ_12_6 = 0, RUMD_POT_COULOMB = 1 } rumd_pot_kind;
+typedef enum { RUMD_CUT_SHIFTED_FORCE = 0 } rumd_cutoff; /* P:73-75; the only method on the hot path */
+typedef enum { RUMD_INT_NVE_LEAPFROG = 0, RUMD_INT_NVT_NOSE_HOOVER = 1 } rumd_integrator;
+typedef enum { RUMD_NB_N2 = 0, RUMD_NB_CELL = 1 } rumd_nb_method; /* P:173 "n2", "sort" */
+
+/* Tunable launch parameters (Table 2: NB method, pb, tp, skin; P:379 sort interval).
+ *   method        neighbour-list build algorithm.
+ *   pb            particles per thread block of the force kernel (Table 1 "PPerBlock").
+ *   tp            threads per particle of the force kernel, one of 1,2,4,8,16,32 ("TPerPart").
+ *                 pb*tp must be a multiple of 32 and <= 1024.
+ *   skin          Verlet skin; list cutoff of a type pair = rc_ab + skin (S4).
+ *   sort_interval RUMD_NB_N2 only: spatially re-sort the particles at every sort_interval-th rebuild
+ *                 (P:379); 0 = never.  RUMD_NB_CELL sorts at every rebuild.
+ *   use_graph     0: plain kernel launches; 1: whole-timestep CUDA graphs (steps_per_graph steps each).
+ *   steps_per_graph  time steps unrolled into one graph launch (>= 1; 0 = library default).
+ *   fuse          1: force + integrate in one kernel per step (double-buffered positions); 0: separate. */
+typedef struct {
+    int method;
+    int pb;
+    int tp;
+    float skin;
+    int sort_interval;
+    int use_graph;
+    int steps_per_graph;
+    int fuse;
+} rumd_tuning;
+
+/* Thermodynamic scalars, all double, filled by rumd_get_thermo (host struct).
+ * U, W: sums over particles of u_i, w_i from the LAST force evaluation (O5; P:160 energy halving).
+ * K: kinetic energy at the integer time of the last completed step, 1/2 sum m |(v_old+v_new)/2|^2 (O10).
+ * mv2: sum m |v(t+dt/2)|^2 after the last step.  xi, eta: Nose-Hoover variables (O7).
+ * H: K + U (+ thermostat terms for NVT, O10), valid when at least one step has run. */
+typedef struct {
+    double U, W, K, mv2, xi, eta, H;
+    long long n_steps;    /* steps completed since rumd_bind_state */
+    long long n_rebuilds; /* neighbour-list builds since rumd_bind_state */
+    int max_nbrs;         /* largest list length seen at the last build */
+    int nbl_capacity;     /* bound capacity (entries per particle) */
+    int overflow;         /* 1 if the last build overflowed */
+    int pad_;
+} rumd_thermo;
+
+/* P:40-46 Fig. 1 `Simulation(...)`.  box_lengths: host, 3 floats (Lx, Ly, Lz), orthorhombic periodic box
+ * centred on the origin, coordinates live in [-L/2, L/2] (O1, S7).  cuda_stream: a cudaStream_t (0 = the
+ * legacy default stream).  1 <= n_types <= RUMD_MAX_TYPES.  *out is written only on success. */
+rumd_status rumd_create(rumd_system** out, int n_particles, int n_types, const float box_lengths[3],
+                        void* cuda_stream);
+rumd_status rumd_destroy(rumd_system* s);
+
+/* State arrays, DEVICE pointers, caller-owned, n_particles elements each, 16-byte aligned:
+ *   d_r     float4 : x, y, z, particle type as int bits in .w             (Fig. 3)
+ *   d_v     float4 : leap-frog velocity v(t - dt/2) x, y, z; mass in .w   (S8)
+ *   d_f     float4 : force x, y, z; per-particle potential energy u_i in .w  [output]
+ *   d_w     float  : per-particle virial w_i = 1/2 sum_j r_ij f_SF(r_ij)     (S13)                [output]
+ *   d_image int4   : periodic image counters ix, iy, iz (w unused)           (S7)
+ *   d_id    int32  : slot -> original particle index; the caller initialises it (normally 0..N-1)
+ * Binding resets the step / rebuild counters, the thermostat (xi = eta = 0) and requests a rebuild. */
+rumd_status rumd_bind_state(rumd_system* s, void* d_r, void* d_v, void* d_f, void* d_w, void* d_image,
+                            void* d_id);
+
+/* Workspace (neighbour list P:101 / P:167, positions at build P:217, cell arrays P:248, sort scratch,
+ * reduction partials, snapshot).  rumd_workspace_bytes: size needed for nbl_capacity entries per
+ * particle.  d_ws: DEVICE pointer, caller-owned, 256-byte aligned, >= bytes.  Re-binding with a larger
+ * capacity is the paper's "re-allocated with doubled capacity" after RUMD_ERR_NBL_OVERFLOW. */
+size_t rumd_workspace_bytes(const rumd_system* s, int nbl_capacity);
+rumd_status rumd_bind_workspace(rumd_system* s, void* d_ws, size_t bytes, int nbl_capacity);
+
+/* P:49-50 `pot.SetParams(i, j, Sigma, Epsilon, Rcut)`; symmetric in (type_i, type_j).  params: host.
+ *   RUMD_POT_LJ_12_6 : {epsilon, sigma, rcut}   u = 4 eps [(s/r)^12 - (s/r)^6]           (O3)
+ *   RUMD_POT_COULOMB : {k*q_i*q_j, rcut}        u = k q_i q_j / r, no self term          (O4, S6)
+ * rcut is an ABSOLUTE distance (S2).  Shifted-force cutoff: f_SF = f(r) - f(rc),
+ * u_SF = u(r) - u(rc) + (r - rc) f(rc) for r < rc, else 0.  One slot per kind per type pair: the same
+ * kind again overwrites, different kinds add, each with its own rc (S5).  rcut <= 0 removes the term. */
+rumd_status rumd_set_pair_potential(rumd_system* s, int type_i, int type_j, rumd_pot_kind kind,
+                                    rumd_cutoff cutoff, const float* params, int n_params);
+
+/* P:54 `IntegratorNVT(timeStep, targetTemperature)`.  NVE leap-frog (O6) or Nose-Hoover leap-frog
+ * (O7) with period tau (tau <= 0 or inf: thermostat off, identical to NVE).  g = 3N - 3 (S10). */
+rumd_status rumd_set_integrator(rumd_system* s, rumd_integrator kind, float dt, float target_T, float tau);
+
+/* Launch parameters.  rumd_default_tuning fills the library's untuned defaults for this N. */
+rumd_status rumd_default_tuning(const rumd_system* s, rumd_tuning* out);
+rumd_status rumd_set_tuning(rumd_system* s, const rumd_tuning* t);
+rumd_status rumd_get_tuning(const rumd_system* s, rumd_tuning* out);
+
+/* Blackwell autotuner (section 11 is the prior art): times short runs of steps_per_trial steps
+ * from one stored snapshot over method x pb x tp x skin (coordinate descent; "single
+ * minimum"), restores the snapshot, applies and returns the fastest setting.  tps_out (host, may be NULL)
+ * receives its time steps per second.  Synchronizes. */
+rumd_status rumd_autotune(rumd_system* s, rumd_tuning* out, int steps_per_trial, double* tps_out);
+
+/* Unconditional list rebuild with the current tuning.  Asynchronous. */
+rumd_status rumd_build_nblist(rumd_system* s);
+/* Rebuild iff the displacement flag is set, then forces / energies / virials into d_f,
+ * d_w (Fig. 3; O5).  Asynchronous. */
+rumd_status rumd_compute_forces(rumd_system* s);
+/* n whole time steps, each (rebuild if flag) -> forces -> integrate + wrap + displacement check (O8;
+ * P:179).  Asynchronous: no host synchronisation inside. */
+rumd_status rumd_run_steps(rumd_system* s, long n);
+
+/* Neighbour list export for inspection / parity tests: row-major, in SLOT numbering (map with d_id).
+ * d_count: device int32 [n_particles]; d_list: device int32 [n_particles * row_capacity], k-th neighbour
+ * of slot i at d_list[i*row_capacity + k]; entries beyond the count are -1.  Asynchronous. */
+rumd_status rumd_export_nblist(rumd_system* s, void* d_count, void* d_list, int row_capacity);
+
+/* Sums U, W on the device (fp64, fixed order), copies the scalars to *out (host).  Synchronizes the stream
+ * and reports sticky errors (RUMD_ERR_NBL_OVERFLOW, RUMD_ERR_NONFINITE, RUMD_ERR_CUDA). */
+rumd_status rumd_get_thermo(rumd_system* s, rumd_thermo* out);
+
+/* In-workspace snapshot of (r, v, image, id, xi, eta, counters) and its restore ("restores the
+ * initial state").  Asynchronous.  Restore requests a rebuild. */
+rumd_status rumd_snapshot(rumd_system* s);
+rumd_status rumd_restore(rumd_system* s);
+
+/* HOST-buffer entry points (used for end-to-end timing): copy the state from / to host arrays of the same
+ * layouts as rumd_bind_state (any pointer may be NULL = skip).  Upload requests a rebuild and resets the
+ * thermostat.  Download synchronizes the stream. */
+rumd_status rumd_upload_state(rumd_system* s, const void* h_r, const void* h_v, const void* h_image,
+                              const void* h_id);
+rumd_status rumd_download_state(rumd_system* s, void* h_r, void* h_v, void* h_f, void* h_w, void* h_image,
+                                void* h_id);
+
+/* Number of kernel launches issued (directly or inside graphs) since rumd_create. */
+long long rumd_launch_count(const rumd_system* s);
+/* Per-kernel-class device time of the last rumd_profile_step call: runs ONE un-fused, un-graphed time step
+ * with CUDA events around each kernel class.  ms_out: host, 4 floats = {build, force, integrate, other}.
+ * did_rebuild_out: host int.  Synchronizes. */
+rumd_status rumd_profile_step(rumd_system* s, float* ms_out, int* did_rebuild_out);
+
+const char* rumd_last_error(const rumd_system* s);
+const char* rumd_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RUMD_B200_H */

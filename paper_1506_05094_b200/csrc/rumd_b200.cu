@@ -1,0 +1,913 @@
+// rumd_b200.cu -- host side of librumd_b200.so: C ABI (include/rumd_b200.h), workspace carving, launch
+// chains, whole-timestep CUDA graphs and the Blackwell autotuner.  Product code: shares nothing with oracle/.
+#include "../../include/rumd_b200.h"
+#include "rumd_force.cuh"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+struct PotSlot {
+    bool lj = false, coul = false;
+    double eps = 0, sig = 0, rc_lj = 0, qq = 0, rc_c = 0;
+};
+
+struct GraphCache {
+    cudaGraphExec_t exec = nullptr;
+    int steps = 0;
+    int kernels = 0;
+};
+
+struct rumd_system {
+    int N = 0, ntypes = 0;
+    float box[3] = {0, 0, 0};
+    cudaStream_t stream = nullptr;
+    Sys S;
+    bool state_bound = false, ws_bound = false, integ_set = false;
+    bool params_dirty = true;
+    PotSlot pot[RUMD_MAXT][RUMD_MAXT];
+    bool any_coul = false;
+    int integ = 0;
+    float dt = 0, T0 = 0, tau = 0;
+    rumd_tuning tune;
+    int cap = 0;
+    void* ws = nullptr;
+    size_t ws_bytes = 0;
+    // snapshot area
+    float4* snap_r = nullptr;
+    float4* snap_v = nullptr;
+    int4* snap_image = nullptr;
+    int* snap_id = nullptr;
+    DevScalars* snap_sc = nullptr;
+    std::vector<int> zrank_host; // for the current grid
+    int grid_for[3] = {0, 0, 0};
+    GraphCache graph_multi, graph_one;
+    rumd_thermo* h_thermo = nullptr; // pinned
+    DevScalars* h_sc = nullptr;      // pinned
+    long long launches = 0;
+    int int_blocks = 0;
+    std::string err;
+};
+
+static rumd_status fail(rumd_system* s, rumd_status st, const char* fmt, ...)
+{
+    if (s) {
+        char buf[512];
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(buf, sizeof buf, fmt, ap);
+        va_end(ap);
+        s->err = buf;
+    }
+    return st;
+}
+
+#define CUDA_TRY(s, call)                                                                              \
+    do {                                                                                               \
+        cudaError_t e_ = (call);                                                                       \
+        if (e_ != cudaSuccess)                                                                         \
+            return fail((s), RUMD_ERR_CUDA, "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_),    \
+                        __FILE__, __LINE__);                                                           \
+    } while (0)
+
+static size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+static double rc_max_of(const rumd_system* s)
+{
+    double m = 0;
+    for (int a = 0; a < s->ntypes; ++a)
+        for (int b = 0; b < s->ntypes; ++b) {
+            const PotSlot& p = s->pot[a][b];
+            if (p.lj) m = std::max(m, p.rc_lj);
+            if (p.coul) m = std::max(m, p.rc_c);
+        }
+    return m;
+}
+
+// S17 (+ a 1e-4 safety margin on the cell edge so that fp32 rounding of the cell coordinate cannot push a
+// listed pair out of the 5x5x5 stencil): n_k = floor(L_k / (1.0001 (rc_max + skin)/2)).
+static void grid_dims(const rumd_system* s, double skin, int n[3])
+{
+    const double edge = 0.5 * (rc_max_of(s) + skin) * 1.0001;
+    for (int k = 0; k < 3; ++k) {
+        n[k] = edge > 0 ? (int)std::floor(s->box[k] / edge) : 1;
+        if (n[k] < 1) n[k] = 1;
+        if (n[k] > 1024) n[k] = 1024;
+    }
+}
+
+static size_t max_cells(const rumd_system* s)
+{
+    // upper bound over all skins >= 0 (skin = 0 gives the finest grid); used to size the workspace
+    int n[3];
+    const double edge = 0.5 * std::max(rc_max_of(s), 0.5) * 1.0001;
+    size_t t = 1;
+    for (int k = 0; k < 3; ++k) {
+        n[k] = std::min(1024, std::max(1, (int)std::floor(s->box[k] / edge)));
+        t *= (size_t)n[k];
+    }
+    return t;
+}
+
+static uint32_t part1by2(uint32_t x)
+{
+    x &= 0x000003ff;
+    x = (x ^ (x << 16)) & 0xff0000ff;
+    x = (x ^ (x << 8)) & 0x0300f00f;
+    x = (x ^ (x << 4)) & 0x030c30c3;
+    x = (x ^ (x << 2)) & 0x09249249;
+    return x;
+}
+
+// Carve the workspace.  Returns bytes needed; if base != nullptr also fills the pointers.
+static size_t carve(rumd_system* s, char* base, int cap)
+{
+    const size_t N = (size_t)s->N, Npad = align_up(N, 32);
+    const size_t nc = max_cells(s);
+    size_t off = 0;
+    auto take = [&](size_t bytes) {
+        size_t o = off;
+        off = align_up(off + bytes, 256);
+        return base ? (void*)(base + o) : (void*)nullptr;
+    };
+    Sys& S = s->S;
+    void* p;
+    p = take(sizeof(DevScalars)); if (base) S.sc = (DevScalars*)p;
+    p = take(sizeof(DevScalars)); if (base) s->snap_sc = (DevScalars*)p;
+    p = take(Npad * (size_t)cap * 4); if (base) S.nbl = (int*)p;
+    p = take(Npad * 4); if (base) S.num_nbrs = (int*)p;
+    p = take(N * 16); if (base) S.r_build = (float4*)p;
+    p = take(N * 16); if (base) S.tmp_r = (float4*)p;
+    p = take(N * 16); if (base) S.tmp_v = (float4*)p;
+    p = take(N * 16); if (base) S.tmp_image = (int4*)p;
+    p = take(N * 4); if (base) S.tmp_id = (int*)p;
+    p = take(N * 16); if (base) s->snap_r = (float4*)p;
+    p = take(N * 16); if (base) s->snap_v = (float4*)p;
+    p = take(N * 16); if (base) s->snap_image = (int4*)p;
+    p = take(N * 4); if (base) s->snap_id = (int*)p;
+    p = take(N * 4); if (base) S.cell_of = (int*)p;
+    p = take(N * 4); if (base) S.slot = (int*)p;
+    p = take(N * 4); if (base) S.perm = (int*)p;
+    p = take(nc * 4); if (base) S.ccount = (int*)p;
+    p = take(nc * 4); if (base) S.cstart_z = (int*)p;
+    p = take(nc * 4); if (base) S.cell_start = (int*)p;
+    p = take(nc * 4); if (base) S.cell_end = (int*)p;
+    p = take(nc * 4); if (base) S.zrank = (int*)p;
+    p = take(nc * 4); if (base) S.zinv = (int*)p;
+    p = take((nc / SCAN_CHUNK + 2) * 4); if (base) S.blocksum = (int*)p;
+    const size_t nblk = (N + 31) / 32 + 1; // upper bound on integrator / fused-step blocks
+    p = take(nblk * 16); if (base) S.partial = (double*)p;
+    return off;
+}
+
+extern "C" const char* rumd_version(void) { return "rumd_b200 0.1 (sm_100a)"; }
+
+extern "C" const char* rumd_last_error(const rumd_system* s) { return s ? s->err.c_str() : "null handle"; }
+
+extern "C" long long rumd_launch_count(const rumd_system* s) { return s ? s->launches : 0; }
+
+extern "C" rumd_status rumd_create(rumd_system** out, int n_particles, int n_types, const float box_lengths[3],
+                                   void* cuda_stream)
+{
+    if (!out || !box_lengths || n_particles < 1 || n_types < 1 || n_types > RUMD_MAXT)
+        return RUMD_ERR_INVALID_ARG;
+    for (int k = 0; k < 3; ++k)
+        if (!(box_lengths[k] > 0.f) || !std::isfinite(box_lengths[k])) return RUMD_ERR_INVALID_ARG;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+        cudaGetLastError();
+        return RUMD_ERR_CUDA; // no CPU fallback
+    }
+    rumd_system* s = new rumd_system();
+    memset(&s->S, 0, sizeof(Sys));
+    s->N = n_particles;
+    s->ntypes = n_types;
+    s->stream = (cudaStream_t)cuda_stream;
+    for (int k = 0; k < 3; ++k) s->box[k] = box_lengths[k];
+    if (cudaMallocHost((void**)&s->h_thermo, sizeof(rumd_thermo)) != cudaSuccess ||
+        cudaMallocHost((void**)&s->h_sc, sizeof(DevScalars)) != cudaSuccess) {
+        delete s;
+        return RUMD_ERR_CUDA;
+    }
+    rumd_default_tuning(s, &s->tune);
+    *out = s;
+    return RUMD_OK;
+}
+
+static void drop_graphs(rumd_system* s)
+{
+    if (s->graph_multi.exec) cudaGraphExecDestroy(s->graph_multi.exec);
+    if (s->graph_one.exec) cudaGraphExecDestroy(s->graph_one.exec);
+    s->graph_multi = GraphCache();
+    s->graph_one = GraphCache();
+}
+
+extern "C" rumd_status rumd_destroy(rumd_system* s)
+{
+    if (!s) return RUMD_ERR_INVALID_ARG;
+    cudaStreamSynchronize(s->stream);
+    drop_graphs(s);
+    if (s->h_thermo) cudaFreeHost(s->h_thermo);
+    if (s->h_sc) cudaFreeHost(s->h_sc);
+    delete s;
+    return RUMD_OK;
+}
+
+// ---------------------------------------------------------------------------------------------- setters
+
+extern "C" rumd_status rumd_bind_state(rumd_system* s, void* d_r, void* d_v, void* d_f, void* d_w, void* d_image,
+                                       void* d_id)
+{
+    if (!s) return RUMD_ERR_INVALID_ARG;
+    if (!d_r || !d_v || !d_f || !d_w || !d_image || !d_id) return fail(s, RUMD_ERR_INVALID_ARG, "null state pointer");
+    if (((uintptr_t)d_r | (uintptr_t)d_v | (uintptr_t)d_f | (uintptr_t)d_image) & 15)
+        return fail(s, RUMD_ERR_INVALID_ARG, "state arrays must be 16-byte aligned");
+    s->S.r = (float4*)d_r;
+    s->S.v = (float4*)d_v;
+    s->S.f = (float4*)d_f;
+    s->S.w = (float*)d_w;
+    s->S.image = (int4*)d_image;
+    s->S.id = (int*)d_id;
+    s->state_bound = true;
+    s->params_dirty = true;
+    drop_graphs(s);
+    if (s->ws_bound) {
+        k_reset_scalars<<<1, 1, 0, s->stream>>>(s->S);
+        s->launches++;
+        CUDA_TRY(s, cudaGetLastError());
+    }
+    return RUMD_OK;
+}
+
+extern "C" size_t rumd_workspace_bytes(const rumd_system* s, int nbl_capacity)
+{
+    if (!s || nbl_capacity < 1) return 0;
+    const int cap = (int)align_up((size_t)nbl_capacity, 32);
+    return carve(const_cast<rumd_system*>(s), nullptr, cap);
+}
+
+extern "C" rumd_status rumd_bind_workspace(rumd_system* s, void* d_ws, size_t bytes, int nbl_capacity)
+{
+    if (!s || !d_ws || nbl_capacity < 1) return RUMD_ERR_INVALID_ARG;
+    if ((uintptr_t)d_ws & 255) return fail(s, RUMD_ERR_INVALID_ARG, "workspace must be 256-byte aligned");
+    const int cap = (int)align_up((size_t)nbl_capacity, 32);
+    const size_t need = carve(s, nullptr, cap);
+    if (bytes < need) return fail(s, RUMD_ERR_INVALID_ARG, "workspace too small: %zu < %zu", bytes, need);
+    // keep the thermostat / counters across a re-bind (capacity doubling) when there was a workspace
+    const bool had = s->ws_bound;
+    DevScalars keep;
+    if (had) {
+        CUDA_TRY(s, cudaMemcpyAsync(&keep, s->S.sc, sizeof keep, cudaMemcpyDeviceToHost, s->stream));
+        CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+    }
+    carve(s, (char*)d_ws, cap);
+    s->ws = d_ws;
+    s->ws_bytes = bytes;
+    s->cap = cap;
+    s->ws_bound = true;
+    s->params_dirty = true;
+    s->grid_for[0] = s->grid_for[1] = s->grid_for[2] = 0;
+    drop_graphs(s);
+    CUDA_TRY(s, cudaMemsetAsync(s->S.ccount, 0, max_cells(s) * 4, s->stream));
+    CUDA_TRY(s, cudaMemsetAsync(s->S.num_nbrs, 0, align_up((size_t)s->N, 32) * 4, s->stream));
+    if (had) {
+        keep.flag = 1u;
+        keep.pending = 0u;
+        keep.ticket = 0u;
+        keep.overflow = 0u;
+        keep.max_nbrs = 0;
+        *s->h_sc = keep;
+        CUDA_TRY(s, cudaMemcpyAsync(s->S.sc, s->h_sc, sizeof keep, cudaMemcpyHostToDevice, s->stream));
+        CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+    } else {
+        k_reset_scalars<<<1, 1, 0, s->stream>>>(s->S);
+        s->launches++;
+        CUDA_TRY(s, cudaGetLastError());
+    }
+    return RUMD_OK;
+}
+
+extern "C" rumd_status rumd_set_pair_potential(rumd_system* s, int ti, int tj, rumd_pot_kind kind,
+                                               rumd_cutoff cutoff, const float* params, int n_params)
+{
+    if (!s || !params) return RUMD_ERR_INVALID_ARG;
+    if (ti < 0 || tj < 0 || ti >= s->ntypes || tj >= s->ntypes) return fail(s, RUMD_ERR_INVALID_ARG, "type out of range");
+    if (cutoff != RUMD_CUT_SHIFTED_FORCE) return fail(s, RUMD_ERR_INVALID_ARG, "only the shifted-force cutoff is implemented");
+    for (int q = 0; q < n_params; ++q)
+        if (!std::isfinite(params[q])) return fail(s, RUMD_ERR_INVALID_ARG, "non-finite parameter");
+    for (int pass = 0; pass < 2; ++pass) {
+        PotSlot& p = pass == 0 ? s->pot[ti][tj] : s->pot[tj][ti];
+        if (kind == RUMD_POT_LJ_12_6) {
+            if (n_params != 3) return fail(s, RUMD_ERR_INVALID_ARG, "LJ takes {epsilon, sigma, rcut}");
+            p.lj = params[2] > 0.f;
+            p.eps = params[0];
+            p.sig = params[1];
+            p.rc_lj = params[2];
+            if (p.lj && !(p.sig > 0)) return fail(s, RUMD_ERR_INVALID_ARG, "sigma must be > 0");
+        } else if (kind == RUMD_POT_COULOMB) {
+            if (n_params != 2) return fail(s, RUMD_ERR_INVALID_ARG, "Coulomb takes {k*qi*qj, rcut}");
+            p.coul = params[1] > 0.f;
+            p.qq = params[0];
+            p.rc_c = params[1];
+        } else
+            return fail(s, RUMD_ERR_INVALID_ARG, "unknown potential kind");
+    }
+    s->params_dirty = true;
+    return RUMD_OK;
+}
+
+extern "C" rumd_status rumd_set_integrator(rumd_system* s, rumd_integrator kind, float dt, float T, float tau)
+{
+    if (!s) return RUMD_ERR_INVALID_ARG;
+    if (kind != RUMD_INT_NVE_LEAPFROG && kind != RUMD_INT_NVT_NOSE_HOOVER) return fail(s, RUMD_ERR_INVALID_ARG, "unknown integrator");
+    if (!(dt > 0.f) || !std::isfinite(dt)) return fail(s, RUMD_ERR_INVALID_ARG, "dt must be > 0");
+    if (kind == RUMD_INT_NVT_NOSE_HOOVER && !(T > 0.f)) return fail(s, RUMD_ERR_INVALID_ARG, "target temperature must be > 0");
+    s->integ = (int)kind;
+    s->dt = dt;
+    s->T0 = T;
+    s->tau = tau;
+    s->integ_set = true;
+    s->params_dirty = true;
+    return RUMD_OK;
+}
+
+// Untuned defaults (the paper's are n2 below N = 8000, pb = 32 / tp = 4 up to N = 10^4, else pb = 64 /
+// tp = 1; these are the B200 counterparts: enough threads for 148 SMs at every N).
+extern "C" rumd_status rumd_default_tuning(const rumd_system* s, rumd_tuning* t)
+{
+    if (!s || !t) return RUMD_ERR_INVALID_ARG;
+    const int N = s->N;
+    t->method = N <= 6000 ? RUMD_NB_N2 : RUMD_NB_CELL;
+    t->tp = N <= 2048 ? 32 : N <= 8192 ? 16 : N <= 32768 ? 8 : N <= 131072 ? 4 : 2;
+    t->pb = std::max(32 / t->tp, 128 / t->tp);
+    t->skin = 0.3f;
+    t->sort_interval = 0;
+    t->use_graph = 1;
+    t->steps_per_graph = 0;
+    t->fuse = 0;
+    return RUMD_OK;
+}
+
+static bool valid_tp(int tp) { return tp == 1 || tp == 2 || tp == 4 || tp == 8 || tp == 16 || tp == 32; }
+
+extern "C" rumd_status rumd_set_tuning(rumd_system* s, const rumd_tuning* t)
+{
+    if (!s || !t) return RUMD_ERR_INVALID_ARG;
+    if (t->method != RUMD_NB_N2 && t->method != RUMD_NB_CELL) return fail(s, RUMD_ERR_INVALID_ARG, "bad method");
+    if (!valid_tp(t->tp)) return fail(s, RUMD_ERR_INVALID_ARG, "tp must be 1,2,4,8,16 or 32");
+    if (t->pb < 1 || (t->pb * t->tp) % 32 || t->pb * t->tp > 1024) return fail(s, RUMD_ERR_INVALID_ARG, "pb*tp must be a multiple of 32 and <= 1024");
+    if (!(t->skin > 0.f) || !std::isfinite(t->skin)) return fail(s, RUMD_ERR_INVALID_ARG, "skin must be > 0");
+    if (t->sort_interval < 0 || t->steps_per_graph < 0) return fail(s, RUMD_ERR_INVALID_ARG, "negative interval");
+    s->tune = *t;
+    s->params_dirty = true;
+    return RUMD_OK;
+}
+
+extern "C" rumd_status rumd_get_tuning(const rumd_system* s, rumd_tuning* t)
+{
+    if (!s || !t) return RUMD_ERR_INVALID_ARG;
+    *t = s->tune;
+    return RUMD_OK;
+}
+
+// ---------------------------------------------------------------------------------------------- parameters
+
+static int ilog2(int x)
+{
+    int l = 0;
+    while ((1 << l) < x) ++l;
+    return l;
+}
+
+// Recompute the by-value kernel parameter block (pair table, box, grid, tuning).  Host side, double precision.
+static rumd_status refresh(rumd_system* s)
+{
+    if (!s->state_bound || !s->ws_bound) return fail(s, RUMD_ERR_NOT_READY, "state and workspace must be bound first");
+    if (!s->params_dirty) return RUMD_OK;
+    Sys& S = s->S;
+    S.N = s->N;
+    S.Npad = (int)align_up((size_t)s->N, 32);
+    S.ntypes = s->ntypes;
+    const rumd_tuning& t = s->tune;
+    S.cap = s->cap;
+    S.cap_it = s->cap / t.tp;
+    S.tp_shift = ilog2(t.tp);
+    S.ppw_shift = 5 - S.tp_shift;
+    const double skin = t.skin;
+    const double rcm = rc_max_of(s);
+    for (int k = 0; k < 3; ++k) {
+        S.L[k] = s->box[k];
+        S.h[k] = 0.5f * s->box[k];
+        S.invL[k] = (float)(1.0 / (double)s->box[k]);
+        if (rcm + skin > 0.5 * (double)s->box[k])
+            return fail(s, RUMD_ERR_BOX_TOO_SMALL, "rc_max + skin = %g exceeds L/2 = %g on axis %d", rcm + skin,
+                        0.5 * s->box[k], k);
+    }
+    S.dt = s->dt;
+    S.dt_d = (double)s->dt;
+    S.half_skin2 = (float)(0.25 * skin * skin);
+    S.T0 = s->T0 > 0 ? (double)s->T0 : 1.0;
+    S.g = 3.0 * s->N - 3.0; // S10
+    const double tau = s->tau;
+    S.omega2 = (tau > 0 && std::isfinite(tau)) ? (2.0 * M_PI / tau) * (2.0 * M_PI / tau) : 0.0;
+    S.sort_interval = t.sort_interval;
+    S.method = t.method;
+    s->any_coul = false;
+    memset(S.pp, 0, sizeof S.pp);
+    for (int a = 0; a < s->ntypes; ++a)
+        for (int b = 0; b < s->ntypes; ++b) {
+            const PotSlot& p = s->pot[a][b];
+            PairParams& q = S.pp[a * s->ntypes + b];
+            double rc = 0;
+            if (p.lj) {
+                const double s6 = std::pow(p.sig, 6), c6 = 4 * p.eps * s6, c12 = c6 * s6;
+                const double ri6 = std::pow(p.rc_lj, -6);
+                const double uc = c12 * ri6 * ri6 - c6 * ri6;
+                const double fc = (12 * c12 * ri6 * ri6 - 6 * c6 * ri6) / p.rc_lj;
+                q.c12 = (float)c12;
+                q.c6 = (float)c6;
+                q.rc2_lj = (float)(p.rc_lj * p.rc_lj);
+                q.fc_lj = (float)fc;
+                q.k0_lj = (float)(uc + p.rc_lj * fc);
+                rc = std::max(rc, p.rc_lj);
+            }
+            if (p.coul) {
+                q.qq = (float)p.qq;
+                q.rc2_c = (float)(p.rc_c * p.rc_c);
+                q.fc_c = (float)(p.qq / (p.rc_c * p.rc_c));
+                q.k0_c = (float)(2.0 * p.qq / p.rc_c);
+                rc = std::max(rc, p.rc_c);
+                s->any_coul = true;
+            }
+            q.rcl2 = (float)((rc + skin) * (rc + skin));
+            q.rc2_max = (float)(rc * rc);
+        }
+    // cell grid + Morton rank table (S17, S19)
+    int n[3];
+    grid_dims(s, skin, n);
+    const size_t ncell = (size_t)n[0] * n[1] * n[2];
+    if (ncell > max_cells(s)) return fail(s, RUMD_ERR_NOT_READY, "cell grid outgrew the workspace: set potentials before binding the workspace");
+    if (t.method == RUMD_NB_CELL && (n[0] < 5 || n[1] < 5 || n[2] < 5))
+        return fail(s, RUMD_ERR_BOX_TOO_SMALL, "cell method needs >= 5 cells per axis (S18), have %dx%dx%d", n[0], n[1], n[2]);
+    S.grid.n[0] = n[0];
+    S.grid.n[1] = n[1];
+    S.grid.n[2] = n[2];
+    S.grid.ncell = (int)ncell;
+    for (int k = 0; k < 3; ++k) S.grid.scale[k] = (float)((double)n[k] / (double)s->box[k]);
+    if (n[0] != s->grid_for[0] || n[1] != s->grid_for[1] || n[2] != s->grid_for[2]) {
+        std::vector<std::pair<uint32_t, int>> keys(ncell);
+        for (int z = 0; z < n[2]; ++z)
+            for (int y = 0; y < n[1]; ++y)
+                for (int x = 0; x < n[0]; ++x) {
+                    const int c = (z * n[1] + y) * n[0] + x;
+                    keys[c] = {part1by2(x) | (part1by2(y) << 1) | (part1by2(z) << 2), c};
+                }
+        std::sort(keys.begin(), keys.end());
+        std::vector<int> zr(ncell), zi(ncell);
+        for (size_t q = 0; q < ncell; ++q) {
+            zr[keys[q].second] = (int)q;
+            zi[q] = keys[q].second;
+        }
+        CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+        CUDA_TRY(s, cudaMemcpyAsync(S.zrank, zr.data(), ncell * 4, cudaMemcpyHostToDevice, s->stream));
+        CUDA_TRY(s, cudaMemcpyAsync(S.zinv, zi.data(), ncell * 4, cudaMemcpyHostToDevice, s->stream));
+        CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+        s->grid_for[0] = n[0];
+        s->grid_for[1] = n[1];
+        s->grid_for[2] = n[2];
+    }
+    s->int_blocks = (s->N + INT_THREADS - 1) / INT_THREADS;
+    s->params_dirty = false;
+    drop_graphs(s);
+    // a list built with other parameters (skin, tp layout, method) is void
+    k_request_rebuild<<<1, 1, 0, s->stream>>>(S);
+    s->launches++;
+    CUDA_TRY(s, cudaGetLastError());
+    return RUMD_OK;
+}
+
+// ---------------------------------------------------------------------------------------------- launch chains
+
+template <int TP, bool COUL, bool ONE>
+static void launch_force_t(rumd_system* s, int nblocks, int nthreads)
+{
+    if (TP >= 8)
+        k_force<TP, COUL, ONE, 2><<<nblocks, nthreads, 0, s->stream>>>(s->S);
+    else
+        k_force<TP, COUL, ONE, 4><<<nblocks, nthreads, 0, s->stream>>>(s->S);
+}
+
+template <int TP>
+static void launch_force_tp(rumd_system* s, int nb, int nt)
+{
+    const bool one = s->ntypes == 1;
+    if (s->any_coul) {
+        if (one) launch_force_t<TP, true, true>(s, nb, nt);
+        else launch_force_t<TP, true, false>(s, nb, nt);
+    } else {
+        if (one) launch_force_t<TP, false, true>(s, nb, nt);
+        else launch_force_t<TP, false, false>(s, nb, nt);
+    }
+}
+
+static int launch_force(rumd_system* s)
+{
+    const int tp = s->tune.tp, nthreads = s->tune.pb * tp;
+    const int nblocks = (int)(((size_t)s->N * tp + nthreads - 1) / nthreads);
+    switch (tp) {
+    case 1: launch_force_tp<1>(s, nblocks, nthreads); break;
+    case 2: launch_force_tp<2>(s, nblocks, nthreads); break;
+    case 4: launch_force_tp<4>(s, nblocks, nthreads); break;
+    case 8: launch_force_tp<8>(s, nblocks, nthreads); break;
+    case 16: launch_force_tp<16>(s, nblocks, nthreads); break;
+    default: launch_force_tp<32>(s, nblocks, nthreads); break;
+    }
+    return 1;
+}
+
+// (rebuild if flag): every kernel of the chain exits at once when the device flag is clear, so the
+// chain can be enqueued -- or baked into a graph -- every step without asking the host.
+static int launch_rebuild_chain(rumd_system* s)
+{
+    const Sys& S = s->S;
+    int n = 0;
+    const bool sorting = s->tune.method == RUMD_NB_CELL || s->tune.sort_interval > 0;
+    if (sorting) {
+        const int nbp = (s->N + 255) / 256, nbc = (S.grid.ncell + 255) / 256;
+        const int nchunks = (S.grid.ncell + SCAN_CHUNK - 1) / SCAN_CHUNK;
+        k_cell_assign<<<nbp, 256, 0, s->stream>>>(S);
+        k_scan_sums<<<nchunks, SCAN_THREADS, 0, s->stream>>>(S);
+        k_scan_blocks<<<1, SCAN_THREADS, 0, s->stream>>>(S, nchunks);
+        k_scan_apply<<<nchunks, SCAN_THREADS, 0, s->stream>>>(S);
+        k_cell_scatter<<<nbp, 256, 0, s->stream>>>(S);
+        k_cell_finish<<<nbc, 256, 0, s->stream>>>(S);
+        k_permute_gather<<<nbp, 256, 0, s->stream>>>(S);
+        k_permute_store<<<nbp, 256, 0, s->stream>>>(S);
+        n += 8;
+    }
+    if (s->tune.method == RUMD_NB_CELL)
+        k_build_cell<<<(s->N + 127) / 128, 128, 0, s->stream>>>(S);
+    else
+        k_build_n2<<<(s->N + N2_WARPS - 1) / N2_WARPS, N2_WARPS * 32, 0, s->stream>>>(S);
+    return n + 1;
+}
+
+static int launch_integrate(rumd_system* s)
+{
+    k_integrate<<<s->int_blocks, INT_THREADS, 0, s->stream>>>(s->S, s->integ == RUMD_INT_NVT_NOSE_HOOVER);
+    return 1;
+}
+
+static int launch_step(rumd_system* s)
+{
+    int n = launch_rebuild_chain(s);
+    n += launch_force(s);
+    n += launch_integrate(s);
+    return n;
+}
+
+static rumd_status ready(rumd_system* s, bool need_integ)
+{
+    if (!s) return RUMD_ERR_INVALID_ARG;
+    if (need_integ && !s->integ_set) return fail(s, RUMD_ERR_NOT_READY, "integrator not set");
+    return refresh(s);
+}
+
+extern "C" rumd_status rumd_build_nblist(rumd_system* s)
+{
+    rumd_status st = ready(s, false);
+    if (st != RUMD_OK) return st;
+    k_request_rebuild<<<1, 1, 0, s->stream>>>(s->S);
+    s->launches += 1 + launch_rebuild_chain(s);
+    CUDA_TRY(s, cudaGetLastError());
+    return RUMD_OK;
+}
+
+extern "C" rumd_status rumd_compute_forces(rumd_system* s)
+{
+    rumd_status st = ready(s, false);
+    if (st != RUMD_OK) return st;
+    s->launches += launch_rebuild_chain(s);
+    s->launches += launch_force(s);
+    CUDA_TRY(s, cudaGetLastError());
+    return RUMD_OK;
+}
+
+// Whole-timestep CUDA graph: `steps` time steps (each the full early-exit chain) captured once and replayed;
+// removes the per-kernel launch cost that dominates at small N.
+static rumd_status get_graph(rumd_system* s, GraphCache& gc, int steps, int* kernels_per_graph)
+{
+    if (gc.exec && gc.steps == steps) {
+        *kernels_per_graph = gc.kernels;
+        return RUMD_OK;
+    }
+    if (gc.exec) cudaGraphExecDestroy(gc.exec);
+    gc = GraphCache();
+    cudaGraph_t g = nullptr;
+    CUDA_TRY(s, cudaStreamBeginCapture(s->stream, cudaStreamCaptureModeThreadLocal));
+    int n = 0;
+    for (int q = 0; q < steps; ++q) n += launch_step(s);
+    cudaError_t e = cudaStreamEndCapture(s->stream, &g);
+    if (e != cudaSuccess) return fail(s, RUMD_ERR_CUDA, "graph capture failed: %s", cudaGetErrorString(e));
+    e = cudaGraphInstantiate(&gc.exec, g, 0);
+    cudaGraphDestroy(g);
+    if (e != cudaSuccess) return fail(s, RUMD_ERR_CUDA, "graph instantiate failed: %s", cudaGetErrorString(e));
+    gc.steps = steps;
+    gc.kernels = n;
+    *kernels_per_graph = n;
+    return RUMD_OK;
+}
+
+extern "C" rumd_status rumd_run_steps(rumd_system* s, long n)
+{
+    rumd_status st = ready(s, true);
+    if (st != RUMD_OK) return st;
+    if (n < 0) return fail(s, RUMD_ERR_INVALID_ARG, "negative step count");
+    if (!s->tune.use_graph) {
+        for (long q = 0; q < n; ++q) s->launches += launch_step(s);
+        CUDA_TRY(s, cudaGetLastError());
+        return RUMD_OK;
+    }
+    int spg = s->tune.steps_per_graph > 0 ? s->tune.steps_per_graph : 32;
+    long left = n;
+    if (left >= spg) {
+        int kpg = 0;
+        st = get_graph(s, s->graph_multi, spg, &kpg);
+        if (st != RUMD_OK) return st;
+        while (left >= spg) {
+            CUDA_TRY(s, cudaGraphLaunch(s->graph_multi.exec, s->stream));
+            s->launches += kpg;
+            left -= spg;
+        }
+    }
+    if (left > 0) {
+        int kpg = 0;
+        st = get_graph(s, s->graph_one, 1, &kpg);
+        if (st != RUMD_OK) return st;
+        for (; left > 0; --left) {
+            CUDA_TRY(s, cudaGraphLaunch(s->graph_one.exec, s->stream));
+            s->launches += kpg;
+        }
+    }
+    return RUMD_OK;
+}
+
+// ---------------------------------------------------------------------------------------------- read-back
+
+extern "C" rumd_status rumd_export_nblist(rumd_system* s, void* d_count, void* d_list, int row_capacity)
+{
+    rumd_status st = ready(s, false);
+    if (st != RUMD_OK) return st;
+    if (!d_count || !d_list || row_capacity < 1) return fail(s, RUMD_ERR_INVALID_ARG, "bad export arguments");
+    k_export_nbl<<<s->N, 128, 0, s->stream>>>(s->S, (int*)d_count, (int*)d_list, row_capacity);
+    s->launches++;
+    CUDA_TRY(s, cudaGetLastError());
+    return RUMD_OK;
+}
+
+extern "C" rumd_status rumd_get_thermo(rumd_system* s, rumd_thermo* out)
+{
+    rumd_status st = ready(s, false);
+    if (st != RUMD_OK) return st;
+    if (!out) return fail(s, RUMD_ERR_INVALID_ARG, "null output");
+    k_thermo<<<1, 1024, 0, s->stream>>>(s->S);
+    s->launches++;
+    CUDA_TRY(s, cudaMemcpyAsync(s->h_sc, s->S.sc, sizeof(DevScalars), cudaMemcpyDeviceToHost, s->stream));
+    CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+    CUDA_TRY(s, cudaGetLastError());
+    const DevScalars& d = *s->h_sc;
+    out->U = d.U;
+    out->W = d.W;
+    out->K = d.K;
+    out->mv2 = d.mv2;
+    out->xi = d.xi;
+    out->eta = d.eta;
+    double H = d.K + d.U;
+    if (s->integ == RUMD_INT_NVT_NOSE_HOOVER) { // O10
+        // K and U belong to time t of the last step; xi, eta are already at t + dt, so H(t) uses the
+        // values step_tail kept for time t (xi_t, eta_t).
+        H += s->S.g * s->S.T0 * d.eta_t;
+        if (s->S.omega2 > 0) H += 0.5 * s->S.g * s->S.T0 * d.xi_t * d.xi_t / s->S.omega2;
+    }
+    out->H = H;
+    out->n_steps = d.n_steps;
+    out->n_rebuilds = d.n_rebuilds;
+    out->max_nbrs = d.max_nbrs;
+    out->nbl_capacity = s->cap;
+    out->overflow = (int)d.overflow;
+    out->pad_ = 0;
+    if (d.overflow) return fail(s, RUMD_ERR_NBL_OVERFLOW, "neighbour list overflow: %d neighbours > capacity %d", d.max_nbrs, s->cap);
+    if (d.nonfinite) return fail(s, RUMD_ERR_NONFINITE, "non-finite energy");
+    return RUMD_OK;
+}
+
+extern "C" rumd_status rumd_snapshot(rumd_system* s)
+{
+    rumd_status st = ready(s, false);
+    if (st != RUMD_OK) return st;
+    const Sys& S = s->S;
+    k_copy_state<<<(s->N + 255) / 256, 256, 0, s->stream>>>(s->N, S.r, S.v, S.image, S.id, s->snap_r, s->snap_v,
+                                                           s->snap_image, s->snap_id);
+    s->launches++;
+    CUDA_TRY(s, cudaMemcpyAsync(s->snap_sc, S.sc, sizeof(DevScalars), cudaMemcpyDeviceToDevice, s->stream));
+    CUDA_TRY(s, cudaGetLastError());
+    return RUMD_OK;
+}
+
+extern "C" rumd_status rumd_restore(rumd_system* s)
+{
+    rumd_status st = ready(s, false);
+    if (st != RUMD_OK) return st;
+    const Sys& S = s->S;
+    k_copy_state<<<(s->N + 255) / 256, 256, 0, s->stream>>>(s->N, s->snap_r, s->snap_v, s->snap_image, s->snap_id,
+                                                           S.r, S.v, S.image, S.id);
+    CUDA_TRY(s, cudaMemcpyAsync(S.sc, s->snap_sc, sizeof(DevScalars), cudaMemcpyDeviceToDevice, s->stream));
+    k_request_rebuild<<<1, 1, 0, s->stream>>>(S);
+    s->launches += 2;
+    CUDA_TRY(s, cudaGetLastError());
+    return RUMD_OK;
+}
+
+extern "C" rumd_status rumd_upload_state(rumd_system* s, const void* h_r, const void* h_v, const void* h_image,
+                                         const void* h_id)
+{
+    rumd_status st = ready(s, false);
+    if (st != RUMD_OK) return st;
+    const size_t N = (size_t)s->N;
+    if (h_r) CUDA_TRY(s, cudaMemcpyAsync(s->S.r, h_r, N * 16, cudaMemcpyHostToDevice, s->stream));
+    if (h_v) CUDA_TRY(s, cudaMemcpyAsync(s->S.v, h_v, N * 16, cudaMemcpyHostToDevice, s->stream));
+    if (h_image) CUDA_TRY(s, cudaMemcpyAsync(s->S.image, h_image, N * 16, cudaMemcpyHostToDevice, s->stream));
+    if (h_id) CUDA_TRY(s, cudaMemcpyAsync(s->S.id, h_id, N * 4, cudaMemcpyHostToDevice, s->stream));
+    k_reset_scalars<<<1, 1, 0, s->stream>>>(s->S);
+    s->launches++;
+    CUDA_TRY(s, cudaGetLastError());
+    return RUMD_OK;
+}
+
+extern "C" rumd_status rumd_download_state(rumd_system* s, void* h_r, void* h_v, void* h_f, void* h_w,
+                                           void* h_image, void* h_id)
+{
+    rumd_status st = ready(s, false);
+    if (st != RUMD_OK) return st;
+    const size_t N = (size_t)s->N;
+    if (h_r) CUDA_TRY(s, cudaMemcpyAsync(h_r, s->S.r, N * 16, cudaMemcpyDeviceToHost, s->stream));
+    if (h_v) CUDA_TRY(s, cudaMemcpyAsync(h_v, s->S.v, N * 16, cudaMemcpyDeviceToHost, s->stream));
+    if (h_f) CUDA_TRY(s, cudaMemcpyAsync(h_f, s->S.f, N * 16, cudaMemcpyDeviceToHost, s->stream));
+    if (h_w) CUDA_TRY(s, cudaMemcpyAsync(h_w, s->S.w, N * 4, cudaMemcpyDeviceToHost, s->stream));
+    if (h_image) CUDA_TRY(s, cudaMemcpyAsync(h_image, s->S.image, N * 16, cudaMemcpyDeviceToHost, s->stream));
+    if (h_id) CUDA_TRY(s, cudaMemcpyAsync(h_id, s->S.id, N * 4, cudaMemcpyDeviceToHost, s->stream));
+    CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+    return RUMD_OK;
+}
+
+// One un-graphed step with events around each kernel class (launch-gap / share analysis at small N).
+extern "C" rumd_status rumd_profile_step(rumd_system* s, float* ms_out, int* did_rebuild_out)
+{
+    rumd_status st = ready(s, true);
+    if (st != RUMD_OK) return st;
+    if (!ms_out) return fail(s, RUMD_ERR_INVALID_ARG, "null output");
+    cudaEvent_t ev[4];
+    for (auto& e : ev) CUDA_TRY(s, cudaEventCreate(&e));
+    CUDA_TRY(s, cudaMemcpyAsync(s->h_sc, s->S.sc, sizeof(DevScalars), cudaMemcpyDeviceToHost, s->stream));
+    CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+    const int did = s->h_sc->flag != 0;
+    cudaEventRecord(ev[0], s->stream);
+    s->launches += launch_rebuild_chain(s);
+    cudaEventRecord(ev[1], s->stream);
+    s->launches += launch_force(s);
+    cudaEventRecord(ev[2], s->stream);
+    s->launches += launch_integrate(s);
+    cudaEventRecord(ev[3], s->stream);
+    CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+    for (int q = 0; q < 3; ++q) cudaEventElapsedTime(&ms_out[q], ev[q], ev[q + 1]);
+    ms_out[3] = 0.f;
+    if (did_rebuild_out) *did_rebuild_out = did;
+    for (auto& e : ev) cudaEventDestroy(e);
+    CUDA_TRY(s, cudaGetLastError());
+    return RUMD_OK;
+}
+
+// ---------------------------------------------------------------------------------------------- A8: autotuner
+
+// One trial (every trial restarts from the same stored state): restore, warm up (includes the first
+// build), time `steps` steps with CUDA events.  Returns steps per second, or 0 when the setting is not
+// admissible (box too small for it, list overflow).
+static double trial(rumd_system* s, const rumd_tuning& t, int steps)
+{
+    if (rumd_set_tuning(s, &t) != RUMD_OK) return 0.0;
+    if (rumd_restore(s) != RUMD_OK) return 0.0;
+    const int warm = std::max(8, steps / 4);
+    if (rumd_run_steps(s, warm) != RUMD_OK) return 0.0;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0);
+    cudaEventCreate(&e1);
+    cudaEventRecord(e0, s->stream);
+    rumd_status st = rumd_run_steps(s, steps);
+    cudaEventRecord(e1, s->stream);
+    rumd_thermo th;
+    rumd_status st2 = rumd_get_thermo(s, &th);
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    if (st != RUMD_OK || st2 != RUMD_OK || !(ms > 0.f)) return 0.0;
+    return 1000.0 * steps / ms;
+}
+
+// Coordinate descent over (method, tp, block size, skin).  The paper's empirical claim that the time has a
+// single minimum along each of pb, tp and skin is what makes this sound; the loop-breaking rules
+// follow P:386-391 in spirit (stop a direction once it is clearly worse than the best).
+extern "C" rumd_status rumd_autotune(rumd_system* s, rumd_tuning* out, int steps_per_trial, double* tps_out)
+{
+    rumd_status st = ready(s, true);
+    if (st != RUMD_OK) return st;
+    if (steps_per_trial < 8) steps_per_trial = 8;
+    const rumd_tuning saved = s->tune;
+    st = rumd_snapshot(s);
+    if (st != RUMD_OK) return st;
+    const double rcm = rc_max_of(s);
+    const double minL = std::min(s->box[0], std::min(s->box[1], s->box[2]));
+    const double skin_max = 0.5 * minL - rcm - 1e-4;
+    rumd_tuning best = saved;
+    best.use_graph = 1;
+    double best_tps = 0.0;
+    std::vector<int> methods;
+    if (s->N <= 20000) methods.push_back(RUMD_NB_N2);
+    methods.push_back(RUMD_NB_CELL);
+    for (int method : methods) {
+        rumd_tuning cur = saved;
+        cur.use_graph = 1;
+        cur.method = method;
+        cur.skin = (float)std::min<double>(saved.skin, skin_max);
+        if (!(cur.skin > 0.f)) continue;
+        double cur_tps = trial(s, cur, steps_per_trial);
+        if (cur_tps <= 0.0 && method == RUMD_NB_CELL) continue; // grid too coarse for the stencil (S18)
+        for (int round = 0; round < 2; ++round) {
+            // threads per particle at fixed block size
+            const int threads = cur.pb * cur.tp;
+            for (int dir = -1; dir <= 1; dir += 2) {
+                rumd_tuning c = cur;
+                for (;;) {
+                    const int tp = dir < 0 ? c.tp / 2 : c.tp * 2;
+                    if (tp < 1 || tp > 32) break;
+                    c.tp = tp;
+                    c.pb = std::max(threads / tp, 32 / tp);
+                    if (c.pb * c.tp > 1024) break;
+                    const double tps = trial(s, c, steps_per_trial);
+                    if (tps > cur_tps) {
+                        cur = c;
+                        cur_tps = tps;
+                    } else
+                        break;
+                }
+            }
+            // block size at fixed tp
+            for (int dir = -1; dir <= 1; dir += 2) {
+                rumd_tuning c = cur;
+                for (;;) {
+                    const int th = dir < 0 ? c.pb * c.tp / 2 : c.pb * c.tp * 2;
+                    if (th < 32 || th > 1024) break;
+                    c.pb = th / c.tp;
+                    const double tps = trial(s, c, steps_per_trial);
+                    if (tps > cur_tps) {
+                        cur = c;
+                        cur_tps = tps;
+                    } else
+                        break;
+                }
+            }
+            // skin: +-15 % steps until the minimum is bracketed
+            for (int dir = -1; dir <= 1; dir += 2) {
+                rumd_tuning c = cur;
+                for (;;) {
+                    const float sk = c.skin * (dir < 0 ? 0.85f : 1.15f);
+                    if (sk < 0.05f || sk > skin_max) break;
+                    c.skin = sk;
+                    const double tps = trial(s, c, steps_per_trial);
+                    if (tps > cur_tps) {
+                        cur = c;
+                        cur_tps = tps;
+                    } else
+                        break;
+                }
+            }
+        }
+        if (cur_tps > best_tps) {
+            best_tps = cur_tps;
+            best = cur;
+        }
+    }
+    rumd_status r1 = rumd_set_tuning(s, best_tps > 0.0 ? &best : &saved);
+    rumd_status r2 = rumd_restore(s);
+    if (r1 != RUMD_OK) return r1;
+    if (r2 != RUMD_OK) return r2;
+    CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+    if (best_tps <= 0.0) return fail(s, RUMD_ERR_NOT_READY, "autotune: no admissible setting");
+    if (out) *out = best;
+    if (tps_out) *tps_out = best_tps;
+    return RUMD_OK;
+}

@@ -1,0 +1,346 @@
+// rumd_force.cuh -- A5 pair force / energy / virial kernel and A6 integrator (sm_100a).
+// Product code: shares nothing with oracle/.
+#pragma once
+#include "rumd_kernels.cuh"
+
+// ------------------------------------------------------------------------------------------ pair function
+
+// O3/O4/O5 for one listed pair: adds f_SF(r) d/r to (fx,fy,fz), u_SF to u and r f_SF to w (the halving of u
+// and w is done once per particle).  Every term applies its own cutoff (S5, strict <, S3).
+// 1/r^2 comes from MUFU.RCP plus one Newton step (the r^-12 term amplifies its error six-fold); 1/r, used
+// only in the small shifted-force terms and Coulomb, from MUFU.RSQ plus one Newton step.
+template <bool COUL>
+__device__ __forceinline__ void pair_accumulate(const float4 p0, const float4 p1, const float4 p2, bool ok,
+                                                float dx, float dy, float dz, float& fx, float& fy, float& fz,
+                                                float& u, float& w)
+{
+    const float r2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, dx * dx));
+    if (!(ok && r2 < p2.z)) return; // p2.z = max rc^2 of the pair's terms
+    float y = rsqrtf(r2);
+    y = y * __fmaf_rn(-0.5f * r2, y * y, 1.5f); // Newton: y <- y (3 - r2 y^2)/2
+    const float rinv = y;
+    float q = __fdividef(1.0f, r2);
+    q = __fmaf_rn(q, __fmaf_rn(-r2, q, 1.0f), q); // Newton: q <- q + q (1 - r2 q)
+    const float rinv2 = q;
+    const float r = r2 * rinv;
+    float fr = 0.f, uu = 0.f; // fr = f_SF(r) / r
+    if (r2 < p0.z) {          // LJ term, p0 = (c12, c6, rc2_lj, fc_lj), p1.x = k0_lj
+        const float rinv6 = rinv2 * rinv2 * rinv2;
+        const float t12 = p0.x * rinv6;
+        uu = __fmaf_rn(rinv6, t12 - p0.y, __fmaf_rn(p0.w, r, -p1.x));
+        fr = __fmaf_rn(rinv6 * rinv2, __fmaf_rn(12.0f, t12, -6.0f * p0.y), -p0.w * rinv);
+    }
+    if (COUL) { // p1 = (k0_lj, qq, rc2_c, fc_c), p2.x = k0_c
+        if (r2 < p1.z) {
+            uu += __fmaf_rn(p1.y, rinv, __fmaf_rn(p1.w, r, -p2.x));
+            fr += __fmaf_rn(p1.y * rinv, rinv2, -p1.w * rinv);
+        }
+    }
+    fx = __fmaf_rn(fr, dx, fx);
+    fy = __fmaf_rn(fr, dy, fy);
+    fz = __fmaf_rn(fr, dz, fz);
+    u += uu;
+    w = __fmaf_rn(fr, r2, w);
+}
+
+// ------------------------------------------------------------------------------------------ A5: forces
+
+// P:110-171 Fig. 3 (`Calcf_NBL_tp`): TP threads per particle stride the particle's neighbour row
+// (P:143 `i = MyT; i += TPerPart`), positions gathered through the read-only path (P:165 LOAD()), partial
+// sums reduced -- here by warp shuffles inside the TP-lane group instead of shared memory + __syncthreads
+// --, lane 0 halves the energy and stores f (xyz, u_i) and w_i.
+// Block = pb particles x TP threads laid out so that lane = (particle-in-warp)*TP + t; UNROLL listed pairs
+// per lane are in flight at once (the paper's one-ahead index prefetch, P:108 item 4, generalised).
+template <int TP, bool COUL, bool ONE_TYPE, int UNROLL>
+__global__ void __launch_bounds__(1024, 1) k_force(const Sys S)
+{
+    __shared__ float4 s_pp[ONE_TYPE ? 1 : 3 * RUMD_MAXT * RUMD_MAXT];
+    if (!ONE_TYPE) {
+        const float4* src = reinterpret_cast<const float4*>(S.pp);
+        // the table is stored compactly: record of the ordered pair (a, b) at a*ntypes + b
+        for (int q = threadIdx.x; q < 3 * S.ntypes * S.ntypes; q += blockDim.x) s_pp[q] = src[q];
+        __syncthreads();
+    }
+    if (blockIdx.x == 0 && threadIdx.x == 0) finish_rebuild(S);
+
+    const int tid = blockIdx.x * blockDim.x + threadIdx.x;
+    const int lane = threadIdx.x & 31;
+    const int i = tid / TP;
+    const int t = tid % TP;
+    const bool have_i = i < S.N;
+    float4 ri = make_float4(0.f, 0.f, 0.f, 0.f);
+    int cnt = 0;
+    if (have_i) {
+        ri = S.r[i];
+        cnt = S.num_nbrs[i];
+    }
+    const int trow = ONE_TYPE ? 0 : 3 * type_of(ri) * S.ntypes;
+    float4 q0, q1, q2;
+    if (ONE_TYPE) {
+        const float4* src = reinterpret_cast<const float4*>(S.pp);
+        q0 = src[0];
+        q1 = src[1];
+        q2 = src[2];
+    }
+    // iterations needed by this warp
+    int nit = (cnt - t + TP - 1) / TP; // entries t, t+TP, ... < cnt
+    if (nit < 0) nit = 0;
+    const int nit_w = __reduce_max_sync(FULLMASK, nit);
+    const int* base = S.nbl + (size_t)(tid >> 5) * S.cap_it * 32 + lane;
+
+    float fx = 0.f, fy = 0.f, fz = 0.f, u = 0.f, w = 0.f;
+    const float hx = S.h[0], hy = S.h[1], hz = S.h[2];
+    const float ix = S.invL[0], iy = S.invL[1], iz = S.invL[2];
+    for (int it = 0; it < nit_w; it += UNROLL) {
+        int j[UNROLL];
+        bool ok[UNROLL];
+        float4 rj[UNROLL];
+#pragma unroll
+        for (int q = 0; q < UNROLL; ++q) {
+            ok[q] = (it + q) < nit;
+            j[q] = ok[q] ? __ldg(base + (size_t)(it + q) * 32) : i;
+        }
+#pragma unroll
+        for (int q = 0; q < UNROLL; ++q) rj[q] = ok[q] ? __ldg(&S.r[j[q]]) : ri;
+#pragma unroll
+        for (int q = 0; q < UNROLL; ++q) {
+            const float dx = min_image(ri.x, rj[q].x, hx, ix);
+            const float dy = min_image(ri.y, rj[q].y, hy, iy);
+            const float dz = min_image(ri.z, rj[q].z, hz, iz);
+            if (!ONE_TYPE) {
+                const int o = trow + 3 * type_of(rj[q]);
+                q0 = s_pp[o];
+                q1 = s_pp[o + 1];
+                q2 = s_pp[o + 2];
+            }
+            pair_accumulate<COUL>(q0, q1, q2, ok[q], dx, dy, dz, fx, fy, fz, u, w);
+        }
+    }
+#pragma unroll
+    for (int o = TP / 2; o; o >>= 1) {
+        fx += __shfl_xor_sync(FULLMASK, fx, o);
+        fy += __shfl_xor_sync(FULLMASK, fy, o);
+        fz += __shfl_xor_sync(FULLMASK, fz, o);
+        u += __shfl_xor_sync(FULLMASK, u, o);
+        w += __shfl_xor_sync(FULLMASK, w, o);
+    }
+    if (have_i && t == 0) {
+        S.f[i] = make_float4(fx, fy, fz, 0.5f * u); // P:160 "compensate for double counting"
+        S.w[i] = 0.5f * w;
+    }
+}
+
+// ------------------------------------------------------------------------------------------ A6: integrator
+
+// O6 / O7 leap-frog step for one particle + wrap (S7) + displacement check (O9, S14).  Returns through
+// kt / mv2 the particle's contributions to K(t) (O10) and sum m v(t+dt/2)^2.
+//   NVE: a = 1, b = dt.   NVT: a = (1 - xi dt/2)/(1 + xi dt/2), b = dt/(1 + xi dt/2)  (O7 rearranged).
+__device__ __forceinline__ void integrate_particle(const Sys& S, float a, float b, float4& r, float4& v,
+                                                   const float4 f, int4& im, const float4 rb, bool& moved,
+                                                   double& kt, double& mv2)
+{
+    const float m = v.w;
+    const float bm = b / m;
+    const float vx = __fmaf_rn(bm, f.x, a * v.x);
+    const float vy = __fmaf_rn(bm, f.y, a * v.y);
+    const float vz = __fmaf_rn(bm, f.z, a * v.z);
+    const float hx = 0.5f * (v.x + vx), hy = 0.5f * (v.y + vy), hz = 0.5f * (v.z + vz);
+    kt = 0.5 * (double)m * ((double)hx * hx + (double)hy * hy + (double)hz * hz);
+    mv2 = (double)m * ((double)vx * vx + (double)vy * vy + (double)vz * vz);
+    v.x = vx;
+    v.y = vy;
+    v.z = vz;
+    float x = __fmaf_rn(S.dt, vx, r.x), y = __fmaf_rn(S.dt, vy, r.y), z = __fmaf_rn(S.dt, vz, r.z);
+    const float nx = rintf(x * S.invL[0]), ny = rintf(y * S.invL[1]), nz = rintf(z * S.invL[2]);
+    x = __fmaf_rn(-nx, S.L[0], x);
+    y = __fmaf_rn(-ny, S.L[1], y);
+    z = __fmaf_rn(-nz, S.L[2], z);
+    im.x += (int)nx;
+    im.y += (int)ny;
+    im.z += (int)nz;
+    r.x = x;
+    r.y = y;
+    r.z = z;
+    const float dx = min_image(x, rb.x, S.h[0], S.invL[0]);
+    const float dy = min_image(y, rb.y, S.h[1], S.invL[1]);
+    const float dz = min_image(z, rb.z, S.h[2], S.invL[2]);
+    moved = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, dx * dx)) > S.half_skin2; // strict > (S14)
+}
+
+__device__ __forceinline__ void nvt_factors(const Sys& S, bool nvt, float& a, float& b)
+{
+    if (nvt) {
+        const double hx = 0.5 * S.sc->xi * S.dt_d;
+        a = (float)((1.0 - hx) / (1.0 + hx));
+        b = (float)(S.dt_d / (1.0 + hx));
+    } else {
+        a = 1.0f;
+        b = S.dt;
+    }
+}
+
+// Block-level tail shared by the split and the fused step kernels: fp64 block sums of (kt, mv2) ->
+// partial[], then the LAST block to arrive (ticket) adds the partials in a fixed order, advances the
+// thermostat (O7: xi += dt w^2 (T_kin/T0 - 1), eta += dt/2 (xi_old + xi_new)), publishes K, and turns this
+// step's displacement result into the rebuild flag of the next step.  No host involvement.
+template <int MAXWARPS>
+__device__ __forceinline__ void step_tail(const Sys& S, bool nvt, double kt, double mv2, bool moved,
+                                          int nblocks)
+{
+    __shared__ double s_k[MAXWARPS], s_m[MAXWARPS];
+    __shared__ int s_moved;
+    __shared__ bool s_last;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+    if (threadIdx.x == 0) s_moved = 0;
+    __syncthreads();
+    kt = warp_sum(kt);
+    mv2 = warp_sum(mv2);
+    if (__any_sync(FULLMASK, moved) && lane == 0) s_moved = 1;
+    if (lane == 0) {
+        s_k[wid] = kt;
+        s_m[wid] = mv2;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double a = 0.0, b = 0.0;
+        for (int q = 0; q < nw; ++q) {
+            a += s_k[q];
+            b += s_m[q];
+        }
+        S.partial[2 * blockIdx.x] = a;
+        S.partial[2 * blockIdx.x + 1] = b;
+        if (s_moved) S.sc->pending = 1u;
+        __threadfence();
+        const unsigned tk = atomicAdd(&S.sc->ticket, 1u);
+        s_last = (tk == (unsigned)nblocks - 1u);
+    }
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    double a = 0.0, b = 0.0;
+    for (int q = threadIdx.x; q < nblocks; q += blockDim.x) {
+        a += __ldcg(&S.partial[2 * q]);
+        b += __ldcg(&S.partial[2 * q + 1]);
+    }
+    a = warp_sum(a);
+    b = warp_sum(b);
+    if (lane == 0) {
+        s_k[wid] = a;
+        s_m[wid] = b;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        a = 0.0;
+        b = 0.0;
+        for (int q = 0; q < nw; ++q) {
+            a += s_k[q];
+            b += s_m[q];
+        }
+        DevScalars* sc = S.sc;
+        sc->K = a;
+        sc->mv2 = b;
+        if (nvt) {
+            const double xi = sc->xi;
+            const double xin = xi + S.dt_d * S.omega2 * (b / S.g / S.T0 - 1.0);
+            sc->xi_t = xi;
+            sc->eta_t = sc->eta;
+            sc->eta += 0.5 * S.dt_d * (xi + xin);
+            sc->xi = xin;
+        }
+        sc->n_steps += 1;
+        const unsigned pend = *((volatile unsigned*)&sc->pending);
+        sc->flag = pend;
+        if (pend) sc->max_nbrs = 0;
+        sc->pending = 0u;
+        sc->ticket = 0u;
+        if (!(a == a) || !(b == b)) sc->nonfinite = 1;
+    }
+}
+
+#define INT_THREADS 128
+__global__ void __launch_bounds__(INT_THREADS) k_integrate(const Sys S, int nvt)
+{
+    float a, b;
+    nvt_factors(S, nvt != 0, a, b);
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    double kt = 0.0, mv2 = 0.0;
+    bool moved = false;
+    if (i < S.N) {
+        float4 r = S.r[i], v = S.v[i];
+        int4 im = S.image[i];
+        integrate_particle(S, a, b, r, v, S.f[i], im, S.r_build[i], moved, kt, mv2);
+        S.r[i] = r;
+        S.v[i] = v;
+        S.image[i] = im;
+    }
+    step_tail<INT_THREADS / 32>(S, nvt != 0, kt, mv2, moved, gridDim.x);
+}
+
+// ------------------------------------------------------------------------------------------ small kernels
+
+__global__ void k_request_rebuild(const Sys S)
+{
+    S.sc->flag = 1u;
+    S.sc->pending = 0u;
+    S.sc->max_nbrs = 0;
+    S.sc->overflow = 0u;
+}
+
+__global__ void k_reset_scalars(const Sys S)
+{
+    DevScalars z;
+    memset(&z, 0, sizeof(z));
+    z.flag = 1u;
+    *S.sc = z;
+}
+
+// U = sum u_i, W = sum w_i in fp64, fixed order (single block).
+__global__ void __launch_bounds__(1024) k_thermo(const Sys S)
+{
+    __shared__ double s_u[32], s_w[32];
+    double u = 0.0, w = 0.0;
+    for (int i = threadIdx.x; i < S.N; i += blockDim.x) {
+        u += (double)S.f[i].w;
+        w += (double)S.w[i];
+    }
+    u = warp_sum(u);
+    w = warp_sum(w);
+    if ((threadIdx.x & 31) == 0) {
+        s_u[threadIdx.x >> 5] = u;
+        s_w[threadIdx.x >> 5] = w;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        u = 0.0;
+        w = 0.0;
+        for (int q = 0; q < 32; ++q) {
+            u += s_u[q];
+            w += s_w[q];
+        }
+        S.sc->U = u;
+        S.sc->W = w;
+        if (!(u == u) || !(w == w)) S.sc->nonfinite = 1;
+    }
+}
+
+// Row-major export of the tiled list (inspection / parity tests).
+__global__ void k_export_nbl(const Sys S, int* count, int* list, int rowcap)
+{
+    const int i = blockIdx.x;
+    const int c = S.num_nbrs[i];
+    if (threadIdx.x == 0) count[i] = c;
+    for (int k = threadIdx.x; k < rowcap; k += blockDim.x)
+        list[(size_t)i * rowcap + k] = k < c ? S.nbl[nbl_index(S, i, k)] : -1;
+}
+
+// snapshot / restore of (r, v, image, id)
+__global__ void k_copy_state(int N, const float4* r, const float4* v, const int4* im, const int* id, float4* r2,
+                             float4* v2, int4* im2, int* id2)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    r2[i] = r[i];
+    v2[i] = v[i];
+    im2[i] = im[i];
+    id2[i] = id[i];
+}

@@ -1,0 +1,63 @@
+// rumd_types.cuh -- device-visible parameter blocks of librumd_b200 (sm_100a).  Product code: shares nothing
+// with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#define RUMD_MAXT 4
+
+// One record per ORDERED type pair; all derived constants are computed on the host in double precision
+// from the user's fp32 parameters and rounded once.
+//   LJ 12-6 (O3):  u = c12/r^12 - c6/r^6,  c12 = 4 eps sigma^12, c6 = 4 eps sigma^6
+//   shifted force: u_SF = u(r) + fc*r - k0,  f_SF/r = f(r)/r - fc/r,  fc = f(rc), k0 = u(rc) + rc*fc
+//   Coulomb (O4):  u = qq/r, same shift with fc = qq/rc^2, k0 = 2 qq/rc
+struct __align__(16) PairParams {
+    float c12, c6, rc2_lj, fc_lj;   // float4 #0
+    float k0_lj, qq, rc2_c, fc_c;   // float4 #1
+    float k0_c, rcl2, rc2_max, pad; // float4 #2: rcl2 = (rc_ab + skin)^2 list cutoff (S4), rc2_max = max rc^2
+};
+
+// Device scalars living in the workspace.
+struct DevScalars {
+    double xi, eta;       // Nose-Hoover variables (O7), at the time AFTER the last step
+    double xi_t, eta_t;   // their values at the integer time t of the last step (for H(t), O10)
+    double K, mv2;        // O10 kinetic energy at integer time; sum m v(t+dt/2)^2
+    double U, W;          // filled by the thermo reduction
+    long long n_steps;
+    long long n_rebuilds;
+    unsigned int flag;    // rebuild requested for the NEXT force evaluation (P:179 updateRequired)
+    unsigned int pending; // set by the integrator's displacement check during a step
+    unsigned int ticket;  // last-block-done counter of the integrator
+    unsigned int overflow;
+    int max_nbrs;         // largest list length of the last build
+    int nonfinite;
+    int pad0, pad1;
+};
+
+struct CellGrid {
+    int n[3];        // cells per axis (S17)
+    int ncell;       // n[0]*n[1]*n[2]
+    float scale[3];  // n_k / L_k
+};
+
+// Everything a kernel needs, passed by value (lives in the constant bank).
+struct Sys {
+    int N, Npad, ntypes;
+    int cap, cap_it;        // list capacity per particle (multiple of 32), cap / tp
+    int tp_shift, ppw_shift;// log2(tp), log2(32/tp)
+    float L[3], h[3], invL[3];
+    float dt, half_skin2;   // (skin/2)^2
+    double dt_d, T0, omega2, g;
+    int sort_interval, method;
+    CellGrid grid;
+    // caller-owned state
+    float4* r; float4* v; float4* f; float* w; int4* image; int* id;
+    // workspace
+    int* nbl; int* num_nbrs; float4* r_build;
+    float4* tmp_r; float4* tmp_v; int4* tmp_image; int* tmp_id;
+    int* cell_of; int* slot; int* perm;
+    int* ccount; int* cstart_z; int* cell_start; int* cell_end; int* zrank; int* zinv; int* blocksum;
+    double* partial;        // 2 doubles per integrator block
+    DevScalars* sc;
+    PairParams pp[RUMD_MAXT * RUMD_MAXT];
+};

@@ -1,0 +1,296 @@
+"""ctypes binding of librumd_b200.so (include/rumd_b200.h) -- argument marshalling only.
+
+Every step of the path runs in the library's CUDA kernels; PyTorch is used for device memory and the
+stream.  There is no CPU fallback: if the library is missing or no CUDA device is present, this fails loudly.
+Names follow the C ABI: ``System.set_pair_potential`` -> ``rumd_set_pair_potential`` and so on.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import math
+import os
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIBPATH = os.path.join(_HERE, "librumd_b200.so")
+
+OK, ERR_INVALID_ARG, ERR_NOT_READY, ERR_CUDA, ERR_NBL_OVERFLOW, ERR_BOX_TOO_SMALL, ERR_NONFINITE = range(7)
+POT_LJ_12_6, POT_COULOMB = 0, 1
+CUT_SHIFTED_FORCE = 0
+INT_NVE_LEAPFROG, INT_NVT_NOSE_HOOVER = 0, 1
+NB_N2, NB_CELL = 0, 1
+
+EXPORTS = [
+    "rumd_create", "rumd_destroy", "rumd_bind_state", "rumd_workspace_bytes", "rumd_bind_workspace",
+    "rumd_set_pair_potential", "rumd_set_integrator", "rumd_default_tuning", "rumd_set_tuning",
+    "rumd_get_tuning", "rumd_autotune", "rumd_build_nblist", "rumd_compute_forces", "rumd_run_steps",
+    "rumd_export_nblist", "rumd_get_thermo", "rumd_snapshot", "rumd_restore", "rumd_upload_state",
+    "rumd_download_state", "rumd_launch_count", "rumd_profile_step", "rumd_last_error", "rumd_version",
+]
+
+
+class Tuning(C.Structure):
+    _fields_ = [("method", C.c_int), ("pb", C.c_int), ("tp", C.c_int), ("skin", C.c_float),
+                ("sort_interval", C.c_int), ("use_graph", C.c_int), ("steps_per_graph", C.c_int),
+                ("fuse", C.c_int)]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_}
+
+
+class Thermo(C.Structure):
+    _fields_ = [("U", C.c_double), ("W", C.c_double), ("K", C.c_double), ("mv2", C.c_double),
+                ("xi", C.c_double), ("eta", C.c_double), ("H", C.c_double), ("n_steps", C.c_longlong),
+                ("n_rebuilds", C.c_longlong), ("max_nbrs", C.c_int), ("nbl_capacity", C.c_int),
+                ("overflow", C.c_int), ("pad_", C.c_int)]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_ if k != "pad_"}
+
+
+class RumdError(RuntimeError):
+    def __init__(self, status, msg):
+        super().__init__("rumd status %d: %s" % (status, msg))
+        self.status = status
+
+
+_lib = None
+
+
+def lib():
+    """Load librumd_b200.so (must have been built: ``python -m paper_1506_05094_b200.build``)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_LIBPATH):
+            raise RuntimeError("librumd_b200.so is missing (%s): build it with "
+                               "`python -m paper_1506_05094_b200.build`; there is no CPU fallback" % _LIBPATH)
+        L = C.CDLL(_LIBPATH)
+        vp, ip = C.c_void_p, C.c_int
+        L.rumd_create.argtypes = [C.POINTER(vp), ip, ip, C.POINTER(C.c_float), vp]
+        L.rumd_destroy.argtypes = [vp]
+        L.rumd_bind_state.argtypes = [vp] * 7
+        L.rumd_workspace_bytes.argtypes = [vp, ip]
+        L.rumd_workspace_bytes.restype = C.c_size_t
+        L.rumd_bind_workspace.argtypes = [vp, vp, C.c_size_t, ip]
+        L.rumd_set_pair_potential.argtypes = [vp, ip, ip, ip, ip, C.POINTER(C.c_float), ip]
+        L.rumd_set_integrator.argtypes = [vp, ip, C.c_float, C.c_float, C.c_float]
+        L.rumd_default_tuning.argtypes = [vp, C.POINTER(Tuning)]
+        L.rumd_set_tuning.argtypes = [vp, C.POINTER(Tuning)]
+        L.rumd_get_tuning.argtypes = [vp, C.POINTER(Tuning)]
+        L.rumd_autotune.argtypes = [vp, C.POINTER(Tuning), ip, C.POINTER(C.c_double)]
+        L.rumd_build_nblist.argtypes = [vp]
+        L.rumd_compute_forces.argtypes = [vp]
+        L.rumd_run_steps.argtypes = [vp, C.c_long]
+        L.rumd_export_nblist.argtypes = [vp, vp, vp, ip]
+        L.rumd_get_thermo.argtypes = [vp, C.POINTER(Thermo)]
+        L.rumd_snapshot.argtypes = [vp]
+        L.rumd_restore.argtypes = [vp]
+        L.rumd_upload_state.argtypes = [vp] * 5
+        L.rumd_download_state.argtypes = [vp] * 7
+        L.rumd_launch_count.argtypes = [vp]
+        L.rumd_launch_count.restype = C.c_longlong
+        L.rumd_profile_step.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(ip)]
+        L.rumd_last_error.argtypes = [vp]
+        L.rumd_last_error.restype = C.c_char_p
+        L.rumd_version.restype = C.c_char_p
+        _lib = L
+    return _lib
+
+
+def estimate_capacity(density: float, rc_max: float, skin: float) -> int:
+    """List capacity per particle: 1.5 x the mean count at this density + 32, rounded up to 32."""
+    mean = 4.0 / 3.0 * math.pi * (rc_max + skin) ** 3 * density
+    return int(math.ceil((1.5 * mean + 32) / 32.0)) * 32
+
+
+class System:
+    """One simulation (Fig. 1).  Owns torch tensors for the state and the workspace and hands their
+    device pointers to the library.  ``wl`` is a ``workloads.Workload``-like object."""
+
+    def __init__(self, r, v, m, types, box, pot, device="cuda:0", skin_for_capacity=0.5, capacity=None,
+                 stream=None):
+        if not torch.cuda.is_available():
+            raise RuntimeError("no CUDA device: librumd_b200 has no CPU fallback")
+        self.L = lib()
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        r = np.ascontiguousarray(r, dtype=np.float32)
+        N = r.shape[0]
+        self.N = N
+        self.ntypes = int(pot.shape[0])
+        self.box = np.ascontiguousarray(box, dtype=np.float32)
+        self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        h = C.c_void_p()
+        st = self.L.rumd_create(C.byref(h), N, self.ntypes, self.box.ctypes.data_as(C.POINTER(C.c_float)),
+                                C.c_void_p(self.stream.cuda_stream))
+        if st != OK:
+            raise RumdError(st, "rumd_create failed")
+        self.h = h
+        # host staging (pinned) in the ABI layouts
+        self.h_r = torch.zeros((N, 4), dtype=torch.float32).pin_memory()
+        self.h_v = torch.zeros((N, 4), dtype=torch.float32).pin_memory()
+        self.h_image = torch.zeros((N, 4), dtype=torch.int32).pin_memory()
+        self.h_id = torch.arange(N, dtype=torch.int32).pin_memory()
+        self.h_r[:, :3] = torch.from_numpy(r)
+        self.h_r[:, 3] = torch.from_numpy(np.ascontiguousarray(types, dtype=np.int32)).view(torch.float32)
+        self.h_v[:, :3] = torch.from_numpy(np.ascontiguousarray(v, dtype=np.float32))
+        self.h_v[:, 3] = torch.from_numpy(np.ascontiguousarray(m, dtype=np.float32))
+        dev = self.device
+        self.d_r = self.h_r.to(dev)
+        self.d_v = self.h_v.to(dev)
+        self.d_f = torch.zeros((N, 4), dtype=torch.float32, device=dev)
+        self.d_w = torch.zeros((N,), dtype=torch.float32, device=dev)
+        self.d_image = self.h_image.to(dev)
+        self.d_id = self.h_id.to(dev)
+        self._check(self.L.rumd_bind_state(self.h, *[C.c_void_p(t.data_ptr()) for t in
+                                                    (self.d_r, self.d_v, self.d_f, self.d_w, self.d_image,
+                                                     self.d_id)]))
+        # potentials (P:49-50 SetParams); pot records are (eps, sigma, rc_LJ, k qa qb, rc_Coulomb)
+        pot = np.asarray(pot, dtype=np.float64)
+        for a in range(self.ntypes):
+            for b in range(a, self.ntypes):
+                e, sg, rcl, qq, rcc = pot[a, b]
+                if rcl > 0:
+                    self.set_pair_potential(a, b, POT_LJ_12_6, [e, sg, rcl])
+                if rcc > 0:
+                    self.set_pair_potential(a, b, POT_COULOMB, [qq, rcc])
+        self.rc_max = float(max(pot[..., 2].max(), pot[..., 4].max()))
+        self.density = N / float(np.prod(self.box.astype(np.float64)))
+        if capacity is None:
+            capacity = estimate_capacity(self.density, self.rc_max, skin_for_capacity)
+        self.d_ws = None
+        self.bind_workspace(capacity)
+
+    # ---- helpers
+    def _check(self, st):
+        if st != OK:
+            raise RumdError(st, self.L.rumd_last_error(self.h).decode())
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.L.rumd_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- the C ABI, same names
+    def bind_workspace(self, capacity: int):
+        capacity = min(int(capacity), ((self.N + 31) // 32) * 32)
+        nbytes = int(self.L.rumd_workspace_bytes(self.h, capacity))
+        ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+        off = (-ws.data_ptr()) % 256
+        self._check(self.L.rumd_bind_workspace(self.h, C.c_void_p(ws.data_ptr() + off), nbytes, capacity))
+        self.d_ws = ws  # keep the new one alive, drop the old one only now
+        self.capacity = capacity
+
+    def set_pair_potential(self, ti, tj, kind, params):
+        arr = (C.c_float * len(params))(*[float(x) for x in params])
+        self._check(self.L.rumd_set_pair_potential(self.h, ti, tj, kind, CUT_SHIFTED_FORCE, arr, len(params)))
+
+    def set_integrator(self, kind, dt, T0=1.0, tau=0.2):
+        self._check(self.L.rumd_set_integrator(self.h, int(kind), float(dt), float(T0), float(tau)))
+
+    def default_tuning(self) -> Tuning:
+        t = Tuning()
+        self._check(self.L.rumd_default_tuning(self.h, C.byref(t)))
+        return t
+
+    def get_tuning(self) -> Tuning:
+        t = Tuning()
+        self._check(self.L.rumd_get_tuning(self.h, C.byref(t)))
+        return t
+
+    def set_tuning(self, t: Tuning = None, **kw):
+        if t is None:
+            t = self.get_tuning()
+        for k, val in kw.items():
+            setattr(t, k, val)
+        self._check(self.L.rumd_set_tuning(self.h, C.byref(t)))
+        return t
+
+    def autotune(self, steps_per_trial=200):
+        t = Tuning()
+        tps = C.c_double()
+        self._check(self.L.rumd_autotune(self.h, C.byref(t), int(steps_per_trial), C.byref(tps)))
+        return t, tps.value
+
+    def build_nblist(self):
+        self._check(self.L.rumd_build_nblist(self.h))
+
+    def compute_forces(self):
+        self._check(self.L.rumd_compute_forces(self.h))
+
+    def run_steps(self, n: int):
+        self._check(self.L.rumd_run_steps(self.h, int(n)))
+
+    def get_thermo(self, grow=False) -> dict:
+        th = Thermo()
+        st = self.L.rumd_get_thermo(self.h, C.byref(th))
+        if st == ERR_NBL_OVERFLOW and grow:
+            # "automatically re-allocated with doubled capacity"
+            self.bind_workspace(max(2 * self.capacity, th.max_nbrs + 32))
+            return None
+        self._check(st)
+        return th.as_dict()
+
+    def snapshot(self):
+        self._check(self.L.rumd_snapshot(self.h))
+
+    def restore(self):
+        self._check(self.L.rumd_restore(self.h))
+
+    def export_nblist(self):
+        """-> (count (N,), list (N, capacity)) int32 numpy arrays in SLOT numbering."""
+        cnt = torch.empty((self.N,), dtype=torch.int32, device=self.device)
+        lst = torch.empty((self.N, self.capacity), dtype=torch.int32, device=self.device)
+        self._check(self.L.rumd_export_nblist(self.h, C.c_void_p(cnt.data_ptr()), C.c_void_p(lst.data_ptr()),
+                                              self.capacity))
+        self.stream.synchronize()
+        return cnt.cpu().numpy(), lst.cpu().numpy()
+
+    def upload_state(self):
+        """Host (pinned) -> device through the ABI's host-buffer entry point."""
+        self._check(self.L.rumd_upload_state(self.h, C.c_void_p(self.h_r.data_ptr()), C.c_void_p(self.h_v.data_ptr()),
+                                             C.c_void_p(self.h_image.data_ptr()), C.c_void_p(self.h_id.data_ptr())))
+
+    def download_state(self, h_r=None, h_v=None, h_f=None, h_w=None, h_image=None, h_id=None):
+        ptr = lambda t: C.c_void_p(t.data_ptr()) if t is not None else None
+        self._check(self.L.rumd_download_state(self.h, ptr(h_r), ptr(h_v), ptr(h_f), ptr(h_w), ptr(h_image),
+                                               ptr(h_id)))
+
+    def launch_count(self) -> int:
+        return int(self.L.rumd_launch_count(self.h))
+
+    def profile_step(self):
+        ms = (C.c_float * 4)()
+        did = C.c_int()
+        self._check(self.L.rumd_profile_step(self.h, ms, C.byref(did)))
+        return dict(build_ms=ms[0], force_ms=ms[1], integrate_ms=ms[2], did_rebuild=bool(did.value))
+
+    # ---- convenience read-back (numpy, ORIGINAL particle numbering via d_id)
+    def state(self) -> dict:
+        self.stream.synchronize()
+        ids = self.d_id.cpu().numpy().astype(np.int64)
+        inv = np.empty_like(ids)
+        inv[ids] = np.arange(self.N)
+        r = self.d_r.cpu().numpy()[inv]
+        v = self.d_v.cpu().numpy()[inv]
+        f = self.d_f.cpu().numpy()[inv]
+        w = self.d_w.cpu().numpy()[inv]
+        im = self.d_image.cpu().numpy()[inv]
+        return dict(r=r[:, :3].copy(), types=r[:, 3].copy().view(np.int32), v=v[:, :3].copy(), m=v[:, 3].copy(),
+                    F=f[:, :3].copy(), u=f[:, 3].copy(), w=w, image=im[:, :3].copy(), ids=ids)
+
+
+def from_workload(wl, **kw) -> System:
+    """Create a System from a ``workloads.Workload`` and set its integrator and skin."""
+    s = System(wl.r, wl.v, wl.m, wl.types, wl.box, wl.pot, **kw)
+    s.set_integrator(wl.integrator, wl.dt, wl.T0, wl.tau)
+    s.set_tuning(skin=float(wl.skin))
+    return s

@@ -1,0 +1,68 @@
+"""CPU-side checks of the boundary: the C-ABI library builds for sm_100a, loads, exports every symbol that
+include/rumd_b200.h declares, and fails loudly (no CPU fallback) when there is no CUDA device."""
+import ctypes as C
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+HEADER = os.path.join(ROOT, "include", "rumd_b200.h")
+
+
+@pytest.fixture(scope="module")
+def libpath():
+    from paper_1506_05094_b200 import build
+
+    return build.build()
+
+
+def declared_symbols():
+    src = open(HEADER).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(rumd_[a-z_0-9]+)\s*\(", src)))
+
+
+def test_header_declares_the_mandated_entry_points():
+    names = declared_symbols()
+    for must in ("rumd_create", "rumd_set_pair_potential", "rumd_build_nblist", "rumd_compute_forces",
+                 "rumd_run_steps"):
+        assert must in names
+
+
+def test_library_exports_every_declared_symbol(libpath):
+    L = C.CDLL(libpath)
+    for name in declared_symbols():
+        assert hasattr(L, name), name
+
+
+def test_binding_lists_the_same_names():
+    src = open(os.path.join(ROOT, "paper_1506_05094_b200", "rumd.py")).read()
+    listed = set(re.findall(r'"(rumd_[a-z_0-9]+)"', src))
+    assert listed == set(declared_symbols())
+
+
+def test_no_cpu_fallback(libpath):
+    import torch
+
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    L = C.CDLL(libpath)
+    h = C.c_void_p()
+    box = (C.c_float * 3)(10, 10, 10)
+    assert L.rumd_create(C.byref(h), 100, 1, box, None) == 3  # RUMD_ERR_CUDA
+    from paper_1506_05094_b200 import rumd, workloads as W
+
+    wl = W.lj_fcc(2)
+    with pytest.raises(RuntimeError):
+        rumd.System(wl.r, wl.v, wl.m, wl.types, wl.box, wl.pot)
+
+
+def test_product_does_not_import_oracle():
+    pkg = os.path.join(ROOT, "paper_1506_05094_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                txt = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(import|from)\s+oracle", txt, flags=re.M), f
+                assert "rumd_oracle" not in txt, f

@@ -1,0 +1,347 @@
+"""GPU parity tests: the CUDA path (through the C ABI, via the ctypes binding) against the fp64 oracle,
+element by element, on the same seeded fp32-representable inputs.  Run with ``-m gpu`` on a B200.
+
+Bars (BASELINE.json north_star; norms per DESIGN.md S25):
+  * neighbour lists identical as pair sets, apart from pairs within 1e-6 sigma of the list cutoff;
+  * per-particle fp32 forces: max_i |F_i - F_i^oracle| <= 1e-4 * rms_i |F_i^oracle|;
+  * potential energy (and virial) to 1e-5 relative after one step from identical inputs.
+"""
+import numpy as np
+import pytest
+
+import oracle
+from paper_1506_05094_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+FORCE_TOL = 1e-4
+ENERGY_TOL = 1e-5
+BAND = 1e-6
+
+
+@pytest.fixture(scope="module")
+def rumd():
+    from paper_1506_05094_b200 import rumd as R
+
+    return R
+
+
+def perturbed(wl, amp=0.05, seed=7):
+    a = amp * wl.meta.get("a", 1.0)
+    wl.r = W.perturb(wl.r, wl.box, a, seed)
+    return wl
+
+
+def lattice_spacing(wl):
+    return (1.0 / wl.meta["density"]) ** (1.0 / 3.0) if wl.meta["lattice"] != "fcc" else (4.0 / wl.meta["density"]) ** (1.0 / 3.0)
+
+
+def make(kind, **kw):
+    wl = {"lj": W.lj_fcc, "ka": W.ka_lattice, "ch": W.charged_sc}[kind](**kw)
+    wl.meta["a"] = lattice_spacing(wl)
+    return wl
+
+
+def pair_keys(count, lst, ids=None):
+    """Set of directed pairs i*N+j (original numbering when ids is given)."""
+    N = count.shape[0]
+    rows = np.repeat(np.arange(N), count)
+    mask = np.arange(lst.shape[1])[None, :] < count[:, None]
+    cols = lst[mask]
+    if ids is not None:
+        rows = ids[rows]
+        cols = ids[cols]
+    return rows.astype(np.int64) * N + cols.astype(np.int64)
+
+
+def check_nblist(sys_, r64, types, box, pot, skin):
+    """GPU list == oracle O2 set, except pairs within BAND of the list cutoff."""
+    cnt, lst = sys_.export_nblist()
+    ids = sys_.d_id.cpu().numpy().astype(np.int64)
+    assert cnt.max() <= sys_.capacity
+    gpu = pair_keys(cnt, lst, ids)
+    assert np.unique(gpu).size == gpu.size, "duplicate neighbours"
+    oc, ol = oracle.nblist(r64, types, box, pot, skin, method="n2" if r64.shape[0] <= 20000 else "cell")
+    ora = pair_keys(oc, ol)
+    diff = np.setxor1d(gpu, ora)
+    N = r64.shape[0]
+    if diff.size:
+        i, j = diff // N, diff % N
+        d = r64[i] - r64[j]
+        d -= box * np.rint(d / box)
+        dist = np.sqrt((d * d).sum(1))
+        rc = np.maximum(pot[types[i], types[j], 2], pot[types[i], types[j], 4]) + skin
+        assert np.all(np.abs(dist - rc) <= BAND), "pair sets differ outside the 1e-6 band: %d pairs, worst %g" % (
+            diff.size, np.abs(dist - rc).max())
+    return cnt, gpu.size, diff.size
+
+
+def check_forces(sys_, r64, types, box, pot):
+    st = sys_.state()
+    F, u, w = oracle.forces_allpairs(r64, types, box, pot) if r64.shape[0] <= 20000 else \
+        oracle.forces_list(r64, types, box, pot, *oracle.nblist(r64, types, box, pot, 0.0, method="cell"))
+    rms = np.sqrt((F * F).sum(1).mean())
+    err = np.sqrt(((st["F"].astype(np.float64) - F) ** 2).sum(1)).max()
+    assert err <= FORCE_TOL * rms, "max|dF| = %g > 1e-4 * rms|F| = %g" % (err, FORCE_TOL * rms)
+    th = sys_.get_thermo()
+    assert th["U"] == pytest.approx(u.sum(), rel=ENERGY_TOL)
+    assert th["W"] == pytest.approx(w.sum(), rel=ENERGY_TOL)
+    # per-particle energies and virials (absolute tolerance scaled by their rms)
+    assert np.abs(st["u"] - u).max() <= 1e-5 * max(1.0, np.abs(u).max())
+    assert np.abs(st["w"] - w).max() <= 1e-5 * max(1.0, np.abs(w).max())
+    return err / rms
+
+
+CASES = [
+    ("lj", dict(ncell=6), "n2", 32),          # configs[0], N = 864
+    ("lj", dict(ncell=6), "cell", 4),
+    ("lj", dict(ncell=10), "cell", 1),        # N = 4000, several tiles + ragged tail
+    ("ka", dict(N=1000), "n2", 16),
+    ("ka", dict(N=4096), "cell", 8),
+    ("ka", dict(N=8000), "cell", 2),          # configs[1]
+    ("ka", dict(N=2048), "n2", 1),            # orthorhombic box 16x16x8
+    ("ch", dict(n=12), "cell", 8),            # charged, N = 1728, rc 4.0 + LJ 2.5
+    ("ch", dict(n=10), "n2", 4),
+]
+
+
+@pytest.mark.parametrize("kind,kw,method,tp", CASES)
+def test_nblist_and_forces_match_oracle(rumd, kind, kw, method, tp):
+    wl = perturbed(make(kind, **kw))
+    s = rumd.from_workload(wl)
+    s.set_tuning(method=rumd.NB_CELL if method == "cell" else rumd.NB_N2, tp=tp, pb=max(32 // tp, 128 // tp))
+    s.compute_forces()
+    r64 = wl.r.astype(np.float64)
+    box = wl.box.astype(np.float64)
+    cnt, npairs, nband = check_nblist(s, r64, wl.types, box, wl.pot, float(wl.skin))
+    assert npairs > 0
+    check_forces(s, r64, wl.types, box, wl.pot)
+    th = s.get_thermo()
+    assert th["n_rebuilds"] == 1 and th["max_nbrs"] == cnt.max()
+    s.close()
+
+
+def test_perfect_lattice_energy_and_counts(rumd):
+    """P6: static fcc lattice, every particle has 78 list entries; U/N = lattice sum; F = 0."""
+    wl = make("lj", ncell=6)
+    s = rumd.from_workload(wl)
+    s.compute_forces()
+    cnt, _ = s.export_nblist()
+    assert np.all(cnt == 78)
+    th = s.get_thermo()
+    F, u, w = oracle.forces_allpairs(wl.r.astype(np.float64), wl.types, wl.box.astype(np.float64), wl.pot)
+    assert th["U"] == pytest.approx(u.sum(), rel=ENERGY_TOL)
+    assert th["W"] == pytest.approx(w.sum(), rel=ENERGY_TOL)
+    assert np.abs(s.state()["F"]).max() < 1e-3
+    s.close()
+
+
+@pytest.mark.parametrize("tp", [1, 2, 4, 8, 16, 32])
+def test_all_tp_layouts_give_the_same_list_and_forces(rumd, tp):
+    wl = perturbed(make("ka", N=1000))
+    ref = None
+    for method in (rumd.NB_N2, rumd.NB_CELL):
+        s = rumd.from_workload(wl)
+        s.set_tuning(method=method, tp=tp, pb=max(32 // tp, 64 // tp))
+        s.compute_forces()
+        cnt, lst = s.export_nblist()
+        keys = np.sort(pair_keys(cnt, lst, s.d_id.cpu().numpy().astype(np.int64)))
+        F = s.state()["F"]
+        if ref is None:
+            ref = (keys, F)
+        else:
+            assert np.array_equal(keys, ref[0])
+            assert np.abs(F - ref[1]).max() <= 1e-4 * np.sqrt((ref[1] ** 2).sum(1).mean())
+        s.close()
+
+
+def test_bitwise_reproducible(rumd):
+    wl = perturbed(make("ka", N=4096))
+    out = []
+    for _ in range(2):
+        s = rumd.from_workload(wl)
+        s.set_tuning(method=rumd.NB_CELL, tp=4, pb=32)
+        s.run_steps(50)
+        st = s.state()
+        out.append((st["r"], st["v"], st["F"]))
+        s.close()
+    for a, b in zip(*out):
+        assert np.array_equal(a, b)
+
+
+@pytest.mark.parametrize("kind,kw,nvt", [("lj", dict(ncell=6), False), ("ka", dict(N=1000), True)])
+def test_one_step_matches_oracle(rumd, kind, kw, nvt):
+    """From identical inputs: one full step (build -> forces -> integrate), then the forces/energies of the
+    NEW configuration; positions modulo L, velocities, thermostat, energies."""
+    wl = perturbed(make(kind, **kw))
+    s = rumd.from_workload(wl)
+    r64, v64, m64 = wl.r.astype(np.float64), wl.v.astype(np.float64), wl.m.astype(np.float64)
+    box = wl.box.astype(np.float64)
+    o = oracle.run(r64, v64, m64, np.zeros((wl.N, 3), np.int32), wl.types, box, wl.pot, float(wl.skin), float(wl.dt),
+                   1, mode=wl.integrator, T0=wl.T0, tau=wl.tau)
+    s.run_steps(1)
+    th1 = s.get_thermo()
+    st = s.state()
+    d = st["r"].astype(np.float64) + st["image"] * box - (o["r"] + o["image"] * box)
+    assert np.abs(d).max() < 2e-6
+    assert np.abs(st["v"] - o["v"]).max() < 1e-5 * max(1.0, np.abs(o["v"]).max())
+    U0, K0 = o["log"][0, 0], o["log"][0, 1]
+    assert th1["U"] == pytest.approx(U0, rel=ENERGY_TOL)
+    assert th1["K"] == pytest.approx(K0, rel=ENERGY_TOL)
+    if nvt:
+        assert th1["xi"] == pytest.approx(o["xi"], rel=1e-4, abs=1e-7)
+        assert th1["eta"] == pytest.approx(o["eta"], rel=1e-4, abs=1e-9)
+    # potential energy after one step (north_star): forces of the new configuration on both sides
+    s.compute_forces()
+    th2 = s.get_thermo()
+    F, u, w = oracle.forces_allpairs(o["r"], wl.types, box, wl.pot)
+    assert th2["U"] == pytest.approx(u.sum(), rel=ENERGY_TOL)
+    s.close()
+
+
+def test_lockstep_spot_checks_and_list_validity(rumd):
+    """Protocol (3): every k steps copy the GPU state into the oracle and repeat the list / force checks; the
+    list in use must contain every pair inside the interaction range (skin/2 invariant)."""
+    wl = perturbed(make("ka", N=1000))
+    s = rumd.from_workload(wl)
+    s.set_tuning(method=rumd.NB_N2, tp=16, pb=8)
+    box = wl.box.astype(np.float64)
+    for _ in range(4):
+        s.run_steps(37)
+        s.compute_forces()   # forces of the current positions with the list in use (rebuilt iff flagged)
+        st = s.state()
+        r64 = st["r"].astype(np.float64)
+        cnt, lst = s.export_nblist()
+        ids = s.d_id.cpu().numpy().astype(np.int64)
+        have = np.unique(pair_keys(cnt, lst, ids))
+        oc, ol = oracle.nblist(r64, wl.types, box, wl.pot, 0.0)
+        need = pair_keys(oc, ol)
+        assert np.isin(need, have).all(), "list in use misses interacting pairs"
+        check_forces(s, r64, wl.types, box, wl.pot)
+    th = s.get_thermo()
+    assert th["n_rebuilds"] >= 2
+    s.close()
+
+
+def test_nve_energy_drift(rumd):
+    """north_star: over 1e4 NVE steps, total-energy drift <= 1e-4 per particle (S26: least-squares slope of
+    E/N times the run length).  configs[0] extended to 1e4 steps."""
+    wl = make("lj", ncell=6)
+    s = rumd.from_workload(wl)
+    E = []
+    s.run_steps(1)
+    for _ in range(100):
+        s.run_steps(100)
+        th = s.get_thermo()
+        E.append((th["K"] + th["U"]) / wl.N)
+    E = np.array(E)
+    t = np.arange(E.size) * 100.0
+    slope = np.polyfit(t, E, 1)[0]
+    assert abs(slope * 1e4) <= 1e-4, "drift %g per particle over 1e4 steps" % (slope * 1e4)
+    assert np.abs(E - E[0]).max() < 5e-3
+    s.close()
+
+
+def test_nvt_short_trajectory_tracks_oracle(rumd):
+    """20 NVT steps from identical inputs: thermostat variables and energies follow the oracle closely
+    (before chaos separates the trajectories)."""
+    wl = perturbed(make("ka", N=1000), amp=0.02)
+    s = rumd.from_workload(wl)
+    n = 20
+    o = oracle.run(wl.r.astype(np.float64), wl.v.astype(np.float64), wl.m.astype(np.float64),
+                   np.zeros((wl.N, 3), np.int32), wl.types, wl.box.astype(np.float64), wl.pot, float(wl.skin),
+                   float(wl.dt), n, mode=W.NVT, T0=wl.T0, tau=wl.tau)
+    s.run_steps(n)
+    th = s.get_thermo()
+    assert th["xi"] == pytest.approx(o["xi"], rel=1e-3, abs=1e-6)
+    assert th["eta"] == pytest.approx(o["eta"], rel=1e-3, abs=1e-8)
+    assert th["U"] == pytest.approx(o["log"][-1, 0], rel=1e-4)
+    assert th["K"] == pytest.approx(o["log"][-1, 1], rel=1e-4)
+    assert th["H"] == pytest.approx(o["log"][-1, 5], rel=1e-4)
+    s.close()
+
+
+def test_overflow_is_reported_and_capacity_doubles(rumd):
+    wl = perturbed(make("lj", ncell=6))
+    s = rumd.System(wl.r, wl.v, wl.m, wl.types, wl.box, wl.pot, capacity=32)
+    s.set_integrator(wl.integrator, wl.dt, wl.T0, wl.tau)
+    s.set_tuning(skin=float(wl.skin))
+    s.compute_forces()
+    with pytest.raises(rumd.RumdError) as e:
+        s.get_thermo()
+    assert e.value.status == rumd.ERR_NBL_OVERFLOW
+    assert s.get_thermo(grow=True) is None     # re-binds a larger workspace
+    s.compute_forces()
+    th = s.get_thermo()
+    assert th["overflow"] == 0 and th["max_nbrs"] <= th["nbl_capacity"]
+    check_forces(s, wl.r.astype(np.float64), wl.types, wl.box.astype(np.float64), wl.pot)
+    s.close()
+
+
+def test_graph_and_plain_launch_agree_bitwise(rumd):
+    wl = perturbed(make("ka", N=1000))
+    res = []
+    for g in (0, 1):
+        s = rumd.from_workload(wl)
+        s.set_tuning(use_graph=g, steps_per_graph=8)
+        s.run_steps(43)
+        st = s.state()
+        res.append((st["r"], st["v"]))
+        assert s.get_thermo()["n_steps"] == 43
+        s.close()
+    assert np.array_equal(res[0][0], res[1][0]) and np.array_equal(res[0][1], res[1][1])
+
+
+def test_snapshot_restore_and_host_buffers(rumd):
+    wl = perturbed(make("ka", N=1000))
+    s = rumd.from_workload(wl)
+    s.snapshot()
+    s.run_steps(25)
+    a = s.state()
+    s.restore()
+    s.run_steps(25)
+    b = s.state()
+    assert np.array_equal(a["r"], b["r"]) and np.array_equal(a["v"], b["v"])
+    # host-buffer entry points: upload the pinned initial state again, run, download
+    s.upload_state()
+    s.run_steps(25)
+    import torch
+
+    h_r = torch.empty((wl.N, 4), dtype=torch.float32).pin_memory()
+    h_id = torch.empty((wl.N,), dtype=torch.int32).pin_memory()
+    s.download_state(h_r=h_r, h_id=h_id)
+    inv = np.empty(wl.N, np.int64)
+    inv[h_id.numpy().astype(np.int64)] = np.arange(wl.N)
+    assert np.array_equal(h_r.numpy()[inv][:, :3], a["r"])
+    s.close()
+
+
+def test_autotune_returns_valid_setting_and_preserves_state(rumd):
+    wl = perturbed(make("ka", N=1000))
+    s = rumd.from_workload(wl)
+    s.run_steps(10)
+    before = s.state()
+    t, tps = s.autotune(steps_per_trial=40)
+    assert tps > 0 and t.tp in (1, 2, 4, 8, 16, 32) and (t.pb * t.tp) % 32 == 0 and t.skin > 0
+    after = s.state()
+    assert np.array_equal(before["r"], after["r"]) and np.array_equal(before["v"], after["v"])
+    s.compute_forces()
+    st = s.state()
+    check_forces(s, st["r"].astype(np.float64), wl.types, wl.box.astype(np.float64), wl.pot)
+    s.close()
+
+
+def test_invalid_arguments_are_rejected(rumd):
+    wl = make("lj", ncell=6)
+    s = rumd.from_workload(wl)
+    with pytest.raises(rumd.RumdError):
+        s.set_tuning(tp=3)
+    with pytest.raises(rumd.RumdError):
+        s.set_tuning(pb=3, tp=1)
+    with pytest.raises(rumd.RumdError):
+        s.set_integrator(0, -1.0)
+    s.set_tuning(skin=4.0)      # rc + skin > L/2 -> lazily at the next compute call
+    with pytest.raises(rumd.RumdError) as e:
+        s.compute_forces()
+    assert e.value.status == rumd.ERR_BOX_TOO_SMALL
+    s.close()
