@@ -173,6 +173,11 @@ long long rumd_launch_count(const rumd_system* s);
  * did_rebuild_out: host int.  Synchronizes. */
 rumd_status rumd_profile_step(rumd_system* s, float* ms_out, int* did_rebuild_out);
 
+/* Average device time, in microseconds, of one launch of the pair-force kernel with the current tuning and the
+ * current list: reps launches replayed from one CUDA graph between two CUDA events on the library's stream
+ * (roofline measurement; the outputs d_f, d_w are simply recomputed).  us_per_launch: host.  Synchronizes. */
+rumd_status rumd_time_force(rumd_system* s, int reps, float* us_per_launch);
+
 const char* rumd_last_error(const rumd_system* s);
 const char* rumd_version(void);
 

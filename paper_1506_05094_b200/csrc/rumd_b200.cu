@@ -791,6 +791,41 @@ extern "C" rumd_status rumd_profile_step(rumd_system* s, float* ms_out, int* did
     return RUMD_OK;
 }
 
+// Average device time of ONE force-kernel launch (current tuning, current list): `reps` launches captured in
+// a graph (no host launch gaps), bracketed by CUDA events on the library's stream.  The list must exist.
+extern "C" rumd_status rumd_time_force(rumd_system* s, int reps, float* us_per_launch)
+{
+    rumd_status st = ready(s, false);
+    if (st != RUMD_OK) return st;
+    if (reps < 1 || !us_per_launch) return fail(s, RUMD_ERR_INVALID_ARG, "bad arguments");
+    cudaGraph_t g = nullptr;
+    cudaGraphExec_t ex = nullptr;
+    CUDA_TRY(s, cudaStreamBeginCapture(s->stream, cudaStreamCaptureModeThreadLocal));
+    for (int q = 0; q < reps; ++q) launch_force(s);
+    cudaError_t e = cudaStreamEndCapture(s->stream, &g);
+    if (e != cudaSuccess) return fail(s, RUMD_ERR_CUDA, "graph capture failed: %s", cudaGetErrorString(e));
+    e = cudaGraphInstantiate(&ex, g, 0);
+    cudaGraphDestroy(g);
+    if (e != cudaSuccess) return fail(s, RUMD_ERR_CUDA, "graph instantiate failed: %s", cudaGetErrorString(e));
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0);
+    cudaEventCreate(&e1);
+    cudaGraphLaunch(ex, s->stream); // warm-up
+    cudaEventRecord(e0, s->stream);
+    cudaGraphLaunch(ex, s->stream);
+    cudaEventRecord(e1, s->stream);
+    cudaError_t es = cudaStreamSynchronize(s->stream);
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaGraphExecDestroy(ex);
+    s->launches += 2LL * reps;
+    if (es != cudaSuccess) return fail(s, RUMD_ERR_CUDA, "force timing failed: %s", cudaGetErrorString(es));
+    *us_per_launch = 1000.f * ms / (float)reps;
+    return RUMD_OK;
+}
+
 // ---------------------------------------------------------------------------------------------- A8: autotuner
 
 // One trial (every trial restarts from the same stored state): restore, warm up (includes the first

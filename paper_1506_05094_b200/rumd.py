@@ -27,7 +27,7 @@ EXPORTS = [
     "rumd_set_pair_potential", "rumd_set_integrator", "rumd_default_tuning", "rumd_set_tuning",
     "rumd_get_tuning", "rumd_autotune", "rumd_build_nblist", "rumd_compute_forces", "rumd_run_steps",
     "rumd_export_nblist", "rumd_get_thermo", "rumd_snapshot", "rumd_restore", "rumd_upload_state",
-    "rumd_download_state", "rumd_launch_count", "rumd_profile_step", "rumd_last_error", "rumd_version",
+    "rumd_download_state", "rumd_launch_count", "rumd_profile_step", "rumd_time_force", "rumd_last_error", "rumd_version",
 ]
 
 
@@ -92,6 +92,7 @@ def lib():
         L.rumd_launch_count.argtypes = [vp]
         L.rumd_launch_count.restype = C.c_longlong
         L.rumd_profile_step.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(ip)]
+        L.rumd_time_force.argtypes = [vp, ip, C.POINTER(C.c_float)]
         L.rumd_last_error.argtypes = [vp]
         L.rumd_last_error.restype = C.c_char_p
         L.rumd_version.restype = C.c_char_p
@@ -272,6 +273,12 @@ class System:
         did = C.c_int()
         self._check(self.L.rumd_profile_step(self.h, ms, C.byref(did)))
         return dict(build_ms=ms[0], force_ms=ms[1], integrate_ms=ms[2], did_rebuild=bool(did.value))
+
+    def time_force(self, reps=100) -> float:
+        """Average device time of one force-kernel launch, microseconds."""
+        us = C.c_float()
+        self._check(self.L.rumd_time_force(self.h, int(reps), C.byref(us)))
+        return float(us.value)
 
     # ---- convenience read-back (numpy, ORIGINAL particle numbering via d_id)
     def state(self) -> dict:
