@@ -178,11 +178,12 @@ def run_gpu(args, rank, world, local_rank):
     l0 = s.launch_count()
     barrier()
     mark = sampler.mark()
-    for a, b in ev:
-        flush.fill_(1)                       # L2 flush between timed iterations (not timed)
-        a.record(stream)
-        s.run_steps(inner)
-        b.record(stream)
+    with torch.cuda.stream(stream):
+        for a, b in ev:
+            flush.fill_(1)                   # L2 flush between timed iterations (same stream, not timed)
+            a.record(stream)
+            s.run_steps(inner)
+            b.record(stream)
     barrier()
     clocks = sampler.stop(mark)
     l1 = s.launch_count()

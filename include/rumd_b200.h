@@ -57,9 +57,15 @@ typedef enum { RUMD_NB_N2 = 0, RUMD_NB_CELL = 1 } rumd_nb_method; /* P:173 "n2",
  *   skin          Verlet skin; list cutoff of a type pair = rc_ab + skin (S4).
  *   sort_interval RUMD_NB_N2 only: spatially re-sort the particles at every sort_interval-th rebuild
  *                 (P:379); 0 = never.  RUMD_NB_CELL sorts at every rebuild.
- *   use_graph     0: plain kernel launches; 1: whole-timestep CUDA graphs (steps_per_graph steps each).
+ *   use_graph     per-step kernels only (persistent = 0).  0: plain kernel launches; 1: whole-timestep CUDA
+ *                 graphs (steps_per_graph steps each).
  *   steps_per_graph  time steps unrolled into one graph launch (>= 1; 0 = library default).
- *   fuse          1: force + integrate in one kernel per step (double-buffered positions); 0: separate. */
+ *   persistent    1: rumd_run_steps(n) is ONE cooperative kernel that runs all n steps (fused force +
+ *                 integrate, double-buffered positions, grid barrier per step, in-kernel rebuilds);
+ *                 0: per-step kernels (early-exit rebuild chain, force, integrate).  pb*tp (rounded to
+ *                 256..1024) is the block size of the persistent kernel.
+ *   build_tp      lanes per particle of the cell-list build, one of 1,2,4,8,16,32 ("not been tried
+ *                 yet"); 0 = library default for this N. */
 typedef struct {
     int method;
     int pb;
@@ -68,7 +74,8 @@ typedef struct {
     int sort_interval;
     int use_graph;
     int steps_per_graph;
-    int fuse;
+    int persistent;
+    int build_tp;
 } rumd_tuning;
 
 /* Thermodynamic scalars, all double, filled by rumd_get_thermo (host struct).
@@ -87,8 +94,10 @@ typedef struct {
 } rumd_thermo;
 
 /* P:40-46 Fig. 1 `Simulation(...)`.  box_lengths: host, 3 floats (Lx, Ly, Lz), orthorhombic periodic box
- * centred on the origin, coordinates live in [-L/2, L/2] (O1, S7).  cuda_stream: a cudaStream_t (0 = the
- * legacy default stream).  1 <= n_types <= RUMD_MAX_TYPES.  *out is written only on success. */
+ * centred on the origin, coordinates live in [-L/2, L/2] (O1, S7).  cuda_stream: a cudaStream_t created by
+ * the caller (e.g. torch.cuda.Stream().cuda_stream); 0 = the library creates and owns a blocking stream,
+ * which stays implicitly ordered with the legacy default stream (the legacy stream itself cannot be
+ * captured into CUDA graphs).  1 <= n_types <= RUMD_MAX_TYPES.  *out is written only on success. */
 rumd_status rumd_create(rumd_system** out, int n_particles, int n_types, const float box_lengths[3],
                         void* cuda_stream);
 rumd_status rumd_destroy(rumd_system* s);

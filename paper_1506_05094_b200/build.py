@@ -12,7 +12,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "librumd_b200.so")
 SOURCES = ["rumd_b200.cu"]
-HEADERS = ["rumd_types.cuh", "rumd_kernels.cuh", "rumd_force.cuh", "../../include/rumd_b200.h"]
+HEADERS = ["rumd_types.cuh", "rumd_kernels.cuh", "rumd_force.cuh", "rumd_persist.cuh", "../../include/rumd_b200.h"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared"]
 

@@ -1,7 +1,7 @@
 // rumd_b200.cu -- host side of librumd_b200.so: C ABI (include/rumd_b200.h), workspace carving, launch
 // chains, whole-timestep CUDA graphs and the Blackwell autotuner.  Product code: shares nothing with oracle/.
 #include "../../include/rumd_b200.h"
-#include "rumd_force.cuh"
+#include "rumd_persist.cuh"
 
 #include <algorithm>
 #include <cmath>
@@ -26,6 +26,7 @@ struct rumd_system {
     int N = 0, ntypes = 0;
     float box[3] = {0, 0, 0};
     cudaStream_t stream = nullptr;
+    bool own_stream = false;
     Sys S;
     bool state_bound = false, ws_bound = false, integ_set = false;
     bool params_dirty = true;
@@ -50,6 +51,9 @@ struct rumd_system {
     DevScalars* h_sc = nullptr;      // pinned
     long long launches = 0;
     int int_blocks = 0;
+    int num_sms = 148;
+    int persist_grid_for = -1; // tuning signature the cached persistent grid belongs to
+    int persist_grid = 0, persist_threads = 0;
     std::string err;
 };
 
@@ -141,6 +145,7 @@ static size_t carve(rumd_system* s, char* base, int cap)
     p = take(Npad * (size_t)cap * 4); if (base) S.nbl = (int*)p;
     p = take(Npad * 4); if (base) S.num_nbrs = (int*)p;
     p = take(N * 16); if (base) S.r_build = (float4*)p;
+    p = take(N * 16); if (base) S.r_alt = (float4*)p;
     p = take(N * 16); if (base) S.tmp_r = (float4*)p;
     p = take(N * 16); if (base) S.tmp_v = (float4*)p;
     p = take(N * 16); if (base) S.tmp_image = (int4*)p;
@@ -154,12 +159,12 @@ static size_t carve(rumd_system* s, char* base, int cap)
     p = take(N * 4); if (base) S.perm = (int*)p;
     p = take(nc * 4); if (base) S.ccount = (int*)p;
     p = take(nc * 4); if (base) S.cstart_z = (int*)p;
-    p = take(nc * 4); if (base) S.cell_start = (int*)p;
-    p = take(nc * 4); if (base) S.cell_end = (int*)p;
+    p = take(nc * 8); if (base) S.cell_range = (int2*)p;
     p = take(nc * 4); if (base) S.zrank = (int*)p;
     p = take(nc * 4); if (base) S.zinv = (int*)p;
     p = take((nc / SCAN_CHUNK + 2) * 4); if (base) S.blocksum = (int*)p;
-    const size_t nblk = (N + 31) / 32 + 1; // upper bound on integrator / fused-step blocks
+    // (kt, mv2) per block: integrator kernel (N/128 blocks) or persistent kernel (2 sets x <= 4096 blocks)
+    const size_t nblk = std::max<size_t>((N + 31) / 32 + 1, 2 * 4096);
     p = take(nblk * 16); if (base) S.partial = (double*)p;
     return off;
 }
@@ -187,11 +192,26 @@ extern "C" rumd_status rumd_create(rumd_system** out, int n_particles, int n_typ
     s->N = n_particles;
     s->ntypes = n_types;
     s->stream = (cudaStream_t)cuda_stream;
+    if (!s->stream) {
+        // the legacy default stream cannot be captured into CUDA graphs: own a BLOCKING stream instead, which
+        // stays implicitly ordered with the legacy default stream
+        if (cudaStreamCreate(&s->stream) != cudaSuccess) {
+            delete s;
+            return RUMD_ERR_CUDA;
+        }
+        s->own_stream = true;
+    }
     for (int k = 0; k < 3; ++k) s->box[k] = box_lengths[k];
     if (cudaMallocHost((void**)&s->h_thermo, sizeof(rumd_thermo)) != cudaSuccess ||
         cudaMallocHost((void**)&s->h_sc, sizeof(DevScalars)) != cudaSuccess) {
         delete s;
         return RUMD_ERR_CUDA;
+    }
+    {
+        int dev = 0, sms = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess &&
+            cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0)
+            s->num_sms = sms;
     }
     rumd_default_tuning(s, &s->tune);
     *out = s;
@@ -213,6 +233,7 @@ extern "C" rumd_status rumd_destroy(rumd_system* s)
     drop_graphs(s);
     if (s->h_thermo) cudaFreeHost(s->h_thermo);
     if (s->h_sc) cudaFreeHost(s->h_sc);
+    if (s->own_stream) cudaStreamDestroy(s->stream);
     delete s;
     return RUMD_OK;
 }
@@ -279,7 +300,7 @@ extern "C" rumd_status rumd_bind_workspace(rumd_system* s, void* d_ws, size_t by
         keep.pending = 0u;
         keep.ticket = 0u;
         keep.overflow = 0u;
-        keep.max_nbrs = 0;
+        keep.max_nbrs[0] = keep.max_nbrs[1] = 0;
         *s->h_sc = keep;
         CUDA_TRY(s, cudaMemcpyAsync(s->S.sc, s->h_sc, sizeof keep, cudaMemcpyHostToDevice, s->stream));
         CUDA_TRY(s, cudaStreamSynchronize(s->stream));
@@ -348,7 +369,8 @@ extern "C" rumd_status rumd_default_tuning(const rumd_system* s, rumd_tuning* t)
     t->sort_interval = 0;
     t->use_graph = 1;
     t->steps_per_graph = 0;
-    t->fuse = 0;
+    t->persistent = 1;
+    t->build_tp = 0;
     return RUMD_OK;
 }
 
@@ -362,6 +384,7 @@ extern "C" rumd_status rumd_set_tuning(rumd_system* s, const rumd_tuning* t)
     if (t->pb < 1 || (t->pb * t->tp) % 32 || t->pb * t->tp > 1024) return fail(s, RUMD_ERR_INVALID_ARG, "pb*tp must be a multiple of 32 and <= 1024");
     if (!(t->skin > 0.f) || !std::isfinite(t->skin)) return fail(s, RUMD_ERR_INVALID_ARG, "skin must be > 0");
     if (t->sort_interval < 0 || t->steps_per_graph < 0) return fail(s, RUMD_ERR_INVALID_ARG, "negative interval");
+    if (t->build_tp != 0 && !valid_tp(t->build_tp)) return fail(s, RUMD_ERR_INVALID_ARG, "build_tp must be 0,1,2,4,8,16 or 32");
     s->tune = *t;
     s->params_dirty = true;
     return RUMD_OK;
@@ -416,6 +439,11 @@ static rumd_status refresh(rumd_system* s)
     S.omega2 = (tau > 0 && std::isfinite(tau)) ? (2.0 * M_PI / tau) * (2.0 * M_PI / tau) : 0.0;
     S.sort_interval = t.sort_interval;
     S.method = t.method;
+    S.r_out = S.r;
+    {   // lanes per particle of the cell build: a whole warp while the machine is not full, fewer at large N
+        const int btp = t.build_tp > 0 ? t.build_tp : s->N <= 16384 ? 32 : s->N <= 65536 ? 16 : s->N <= 262144 ? 8 : 4;
+        S.build_tp_shift = ilog2(btp);
+    }
     s->any_coul = false;
     memset(S.pp, 0, sizeof S.pp);
     for (int a = 0; a < s->ntypes; ++a)
@@ -481,6 +509,7 @@ static rumd_status refresh(rumd_system* s)
         s->grid_for[2] = n[2];
     }
     s->int_blocks = (s->N + INT_THREADS - 1) / INT_THREADS;
+    s->persist_grid_for = -1;
     s->params_dirty = false;
     drop_graphs(s);
     // a list built with other parameters (skin, tp layout, method) is void
@@ -492,41 +521,80 @@ static rumd_status refresh(rumd_system* s)
 
 // ---------------------------------------------------------------------------------------------- launch chains
 
-template <int TP, bool COUL, bool ONE>
-static void launch_force_t(rumd_system* s, int nblocks, int nthreads)
-{
-    if (TP >= 8)
-        k_force<TP, COUL, ONE, 2><<<nblocks, nthreads, 0, s->stream>>>(s->S);
-    else
-        k_force<TP, COUL, ONE, 4><<<nblocks, nthreads, 0, s->stream>>>(s->S);
-}
+// Kernel selection over (TP, COUL, ONE_TYPE); UNROLL follows TP (wide groups have few iterations per lane).
+template <int TP> struct UnrollOf { static constexpr int value = TP >= 8 ? 2 : 4; };
 
-template <int TP>
-static void launch_force_tp(rumd_system* s, int nb, int nt)
+template <template <int, bool, bool> class F, int TP, typename... A>
+static auto pick_flags(rumd_system* s, A... a)
 {
     const bool one = s->ntypes == 1;
-    if (s->any_coul) {
-        if (one) launch_force_t<TP, true, true>(s, nb, nt);
-        else launch_force_t<TP, true, false>(s, nb, nt);
-    } else {
-        if (one) launch_force_t<TP, false, true>(s, nb, nt);
-        else launch_force_t<TP, false, false>(s, nb, nt);
+    if (s->any_coul) return one ? F<TP, true, true>::run(s, a...) : F<TP, true, false>::run(s, a...);
+    return one ? F<TP, false, true>::run(s, a...) : F<TP, false, false>::run(s, a...);
+}
+
+template <template <int, bool, bool> class F, typename... A>
+static auto pick_kernel(rumd_system* s, A... a)
+{
+    switch (s->tune.tp) {
+    case 1: return pick_flags<F, 1>(s, a...);
+    case 2: return pick_flags<F, 2>(s, a...);
+    case 4: return pick_flags<F, 4>(s, a...);
+    case 8: return pick_flags<F, 8>(s, a...);
+    case 16: return pick_flags<F, 16>(s, a...);
+    default: return pick_flags<F, 32>(s, a...);
     }
 }
+
+template <int TP, bool COUL, bool ONE> struct ForceLaunch {
+    static int run(rumd_system* s, int nblocks, int nthreads)
+    {
+        k_force<TP, COUL, ONE, UnrollOf<TP>::value><<<nblocks, nthreads, 0, s->stream>>>(s->S);
+        return 1;
+    }
+};
 
 static int launch_force(rumd_system* s)
 {
     const int tp = s->tune.tp, nthreads = s->tune.pb * tp;
     const int nblocks = (int)(((size_t)s->N * tp + nthreads - 1) / nthreads);
-    switch (tp) {
-    case 1: launch_force_tp<1>(s, nblocks, nthreads); break;
-    case 2: launch_force_tp<2>(s, nblocks, nthreads); break;
-    case 4: launch_force_tp<4>(s, nblocks, nthreads); break;
-    case 8: launch_force_tp<8>(s, nblocks, nthreads); break;
-    case 16: launch_force_tp<16>(s, nblocks, nthreads); break;
-    default: launch_force_tp<32>(s, nblocks, nthreads); break;
+    return pick_kernel<ForceLaunch>(s, nblocks, nthreads);
+}
+
+// A7, persistent form: the address of the k_persist instantiation for the current tuning.
+template <int TP, bool COUL, bool ONE> struct PersistKernel {
+    static const void* run(rumd_system*) { return (const void*)&k_persist<TP, COUL, ONE, UnrollOf<TP>::value>; }
+};
+
+static int persist_threads_of(const rumd_tuning& t)
+{
+    int th = t.pb * t.tp / 256 * 256;
+    return std::min(512, std::max(256, th));
+}
+
+// n steps in ONE cooperative launch.  The grid is sized to cover N*tp virtual threads when it can be
+// co-resident, else to the co-residency limit (the kernel strides).
+static rumd_status launch_persistent(rumd_system* s, int nsteps)
+{
+    const void* fn = pick_kernel<PersistKernel>(s);
+    const int threads = persist_threads_of(s->tune);
+    const int sig = s->tune.tp * 4096 + threads + (s->any_coul ? 1 << 20 : 0) + (s->ntypes == 1 ? 1 << 21 : 0);
+    if (sig != s->persist_grid_for) {
+        int per_sm = 0;
+        CUDA_TRY(s, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, threads, 0));
+        if (per_sm < 1) return fail(s, RUMD_ERR_CUDA, "persistent kernel does not fit an SM");
+        const long long want = ((long long)s->N * s->tune.tp + threads - 1) / threads;
+        long long grid = std::min<long long>(want, (long long)per_sm * s->num_sms);
+        grid = std::min<long long>(grid, 4096);
+        s->persist_grid = (int)std::max<long long>(1, grid);
+        s->persist_threads = threads;
+        s->persist_grid_for = sig;
     }
-    return 1;
+    CUDA_TRY(s, cudaMemsetAsync(&s->S.sc->barrier, 0, sizeof(unsigned), s->stream));
+    int nvt = s->integ == RUMD_INT_NVT_NOSE_HOOVER;
+    void* args[] = {(void*)&s->S, (void*)&nsteps, (void*)&nvt};
+    CUDA_TRY(s, cudaLaunchCooperativeKernel(fn, dim3(s->persist_grid), dim3(s->persist_threads), args, 0, s->stream));
+    s->launches += 1;
+    return RUMD_OK;
 }
 
 // (rebuild if flag): every kernel of the chain exits at once when the device flag is clear, so the
@@ -540,19 +608,26 @@ static int launch_rebuild_chain(rumd_system* s)
         const int nbp = (s->N + 255) / 256, nbc = (S.grid.ncell + 255) / 256;
         const int nchunks = (S.grid.ncell + SCAN_CHUNK - 1) / SCAN_CHUNK;
         k_cell_assign<<<nbp, 256, 0, s->stream>>>(S);
-        k_scan_sums<<<nchunks, SCAN_THREADS, 0, s->stream>>>(S);
-        k_scan_blocks<<<1, SCAN_THREADS, 0, s->stream>>>(S, nchunks);
-        k_scan_apply<<<nchunks, SCAN_THREADS, 0, s->stream>>>(S);
+        if (nchunks <= 8) {
+            k_scan_single<<<1, SCAN_THREADS, 0, s->stream>>>(S);
+            n += 2;
+        } else {
+            k_scan_sums<<<std::min(nchunks, 1024), SCAN_THREADS, 0, s->stream>>>(S);
+            k_scan_blocks<<<1, SCAN_THREADS, 0, s->stream>>>(S);
+            k_scan_apply<<<std::min(nchunks, 1024), SCAN_THREADS, 0, s->stream>>>(S);
+            n += 4;
+        }
         k_cell_scatter<<<nbp, 256, 0, s->stream>>>(S);
         k_cell_finish<<<nbc, 256, 0, s->stream>>>(S);
         k_permute_gather<<<nbp, 256, 0, s->stream>>>(S);
         k_permute_store<<<nbp, 256, 0, s->stream>>>(S);
-        n += 8;
+        n += 4;
     }
-    if (s->tune.method == RUMD_NB_CELL)
-        k_build_cell<<<(s->N + 127) / 128, 128, 0, s->stream>>>(S);
-    else
-        k_build_n2<<<(s->N + N2_WARPS - 1) / N2_WARPS, N2_WARPS * 32, 0, s->stream>>>(S);
+    if (s->tune.method == RUMD_NB_CELL) {
+        const long long threads = (long long)s->N << S.build_tp_shift;
+        k_build_cell<<<(unsigned)((threads + 127) / 128), 128, 0, s->stream>>>(S);
+    } else
+        k_build_n2<<<(s->N + 3) / 4, 128, 0, s->stream>>>(S);
     return n + 1;
 }
 
@@ -627,6 +702,17 @@ extern "C" rumd_status rumd_run_steps(rumd_system* s, long n)
     rumd_status st = ready(s, true);
     if (st != RUMD_OK) return st;
     if (n < 0) return fail(s, RUMD_ERR_INVALID_ARG, "negative step count");
+    if (n == 0) return RUMD_OK;
+    if (s->tune.persistent) {
+        // one cooperative launch per <= 2^20 steps (the step counter inside the kernel is an int)
+        for (long left = n; left > 0;) {
+            const int chunk = (int)std::min<long>(left, 1L << 20);
+            st = launch_persistent(s, chunk);
+            if (st != RUMD_OK) return st;
+            left -= chunk;
+        }
+        return RUMD_OK;
+    }
     if (!s->tune.use_graph) {
         for (long q = 0; q < n; ++q) s->launches += launch_step(s);
         CUDA_TRY(s, cudaGetLastError());
@@ -696,11 +782,14 @@ extern "C" rumd_status rumd_get_thermo(rumd_system* s, rumd_thermo* out)
     out->H = H;
     out->n_steps = d.n_steps;
     out->n_rebuilds = d.n_rebuilds;
-    out->max_nbrs = d.max_nbrs;
+    // slot of the last completed build (a build whose force evaluation has not run yet still owns the flag)
+    const int max_nbrs = d.max_nbrs[(d.flag ? d.n_rebuilds : d.n_rebuilds + 1) & 1];
+    out->max_nbrs = max_nbrs;
     out->nbl_capacity = s->cap;
     out->overflow = (int)d.overflow;
     out->pad_ = 0;
-    if (d.overflow) return fail(s, RUMD_ERR_NBL_OVERFLOW, "neighbour list overflow: %d neighbours > capacity %d", d.max_nbrs, s->cap);
+    if (d.overflow) return fail(s, RUMD_ERR_NBL_OVERFLOW, "neighbour list overflow: %d neighbours > capacity %d", max_nbrs, s->cap);
+    if (d.nonfinite == 2) return fail(s, RUMD_ERR_CUDA, "persistent kernel: grid barrier timed out");
     if (d.nonfinite) return fail(s, RUMD_ERR_NONFINITE, "non-finite energy");
     return RUMD_OK;
 }

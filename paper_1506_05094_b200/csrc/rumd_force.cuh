@@ -48,47 +48,35 @@ __device__ __forceinline__ void pair_accumulate(const float4 p0, const float4 p1
 // P:110-171 Fig. 3 (`Calcf_NBL_tp`): TP threads per particle stride the particle's neighbour row
 // (P:143 `i = MyT; i += TPerPart`), positions gathered through the read-only path (P:165 LOAD()), partial
 // sums reduced -- here by warp shuffles inside the TP-lane group instead of shared memory + __syncthreads
-// --, lane 0 halves the energy and stores f (xyz, u_i) and w_i.
-// Block = pb particles x TP threads laid out so that lane = (particle-in-warp)*TP + t; UNROLL listed pairs
+// --, lane 0 halves the energy.  Lane = (particle-in-warp)*TP + t; UNROLL listed pairs
 // per lane are in flight at once (the paper's one-ahead index prefetch, P:108 item 4, generalised).
-template <int TP, bool COUL, bool ONE_TYPE, int UNROLL>
-__global__ void __launch_bounds__(1024, 1) k_force(const Sys S)
-{
-    __shared__ float4 s_pp[ONE_TYPE ? 1 : 3 * RUMD_MAXT * RUMD_MAXT];
-    if (!ONE_TYPE) {
-        const float4* src = reinterpret_cast<const float4*>(S.pp);
-        // the table is stored compactly: record of the ordered pair (a, b) at a*ntypes + b
-        for (int q = threadIdx.x; q < 3 * S.ntypes * S.ntypes; q += blockDim.x) s_pp[q] = src[q];
-        __syncthreads();
-    }
-    if (blockIdx.x == 0 && threadIdx.x == 0) finish_rebuild(S);
+//
+// force_group: the partial sums of one lane, then the butterfly over its TP-lane group; on return every lane
+// of the group holds the particle's totals (u and w NOT yet halved).  vwarp = index of this warp in the
+// virtual grid of N*TP threads.  NC = true: list and positions are read-only for the whole kernel, loads go
+// through ld.global.nc; NC = false (persistent kernel, which rewrites both): coherent loads, the index
+// stream marked evict-first.  All 32 lanes of the warp must call.
+template <bool NC> __device__ __forceinline__ int load_idx(const int* p) { return NC ? __ldg(p) : __ldcs(p); }
+template <bool NC> __device__ __forceinline__ float4 load_pos(const float4* p) { return NC ? __ldg(p) : *p; }
 
-    const int tid = blockIdx.x * blockDim.x + threadIdx.x;
+template <int TP, bool COUL, bool ONE_TYPE, int UNROLL, bool NC>
+__device__ __forceinline__ void force_group(const Sys& S, const float4* r, const float4* s_pp, int vwarp, int i,
+                                            int t, const float4 ri, int cnt, float& fx, float& fy, float& fz,
+                                            float& u, float& w)
+{
     const int lane = threadIdx.x & 31;
-    const int i = tid / TP;
-    const int t = tid % TP;
-    const bool have_i = i < S.N;
-    float4 ri = make_float4(0.f, 0.f, 0.f, 0.f);
-    int cnt = 0;
-    if (have_i) {
-        ri = S.r[i];
-        cnt = S.num_nbrs[i];
-    }
     const int trow = ONE_TYPE ? 0 : 3 * type_of(ri) * S.ntypes;
     float4 q0, q1, q2;
     if (ONE_TYPE) {
-        const float4* src = reinterpret_cast<const float4*>(S.pp);
-        q0 = src[0];
-        q1 = src[1];
-        q2 = src[2];
+        q0 = s_pp[0];
+        q1 = s_pp[1];
+        q2 = s_pp[2];
     }
-    // iterations needed by this warp
     int nit = (cnt - t + TP - 1) / TP; // entries t, t+TP, ... < cnt
     if (nit < 0) nit = 0;
     const int nit_w = __reduce_max_sync(FULLMASK, nit);
-    const int* base = S.nbl + (size_t)(tid >> 5) * S.cap_it * 32 + lane;
-
-    float fx = 0.f, fy = 0.f, fz = 0.f, u = 0.f, w = 0.f;
+    const int* base = S.nbl + (size_t)vwarp * S.cap_it * 32 + lane;
+    fx = fy = fz = u = w = 0.f;
     const float hx = S.h[0], hy = S.h[1], hz = S.h[2];
     const float ix = S.invL[0], iy = S.invL[1], iz = S.invL[2];
     for (int it = 0; it < nit_w; it += UNROLL) {
@@ -98,10 +86,10 @@ __global__ void __launch_bounds__(1024, 1) k_force(const Sys S)
 #pragma unroll
         for (int q = 0; q < UNROLL; ++q) {
             ok[q] = (it + q) < nit;
-            j[q] = ok[q] ? __ldg(base + (size_t)(it + q) * 32) : i;
+            j[q] = ok[q] ? load_idx<NC>(base + (size_t)(it + q) * 32) : i;
         }
 #pragma unroll
-        for (int q = 0; q < UNROLL; ++q) rj[q] = ok[q] ? __ldg(&S.r[j[q]]) : ri;
+        for (int q = 0; q < UNROLL; ++q) rj[q] = ok[q] ? load_pos<NC>(&r[j[q]]) : ri;
 #pragma unroll
         for (int q = 0; q < UNROLL; ++q) {
             const float dx = min_image(ri.x, rj[q].x, hx, ix);
@@ -124,6 +112,45 @@ __global__ void __launch_bounds__(1024, 1) k_force(const Sys S)
         u += __shfl_xor_sync(FULLMASK, u, o);
         w += __shfl_xor_sync(FULLMASK, w, o);
     }
+}
+
+// the pair table in shared memory: record of the ordered pair (a, b) at 3*(a*ntypes + b) (three float4)
+__device__ __forceinline__ void load_pair_table(const Sys& S, float4* s_pp)
+{
+    const float4* src = reinterpret_cast<const float4*>(S.pp);
+    for (int q = threadIdx.x; q < 3 * S.ntypes * S.ntypes; q += blockDim.x) s_pp[q] = src[q];
+}
+
+// Bookkeeping that must happen once per step AFTER every rebuild kernel has read the flag: count the
+// rebuild, clear the flag and zero the max-length slot of the NEXT build.  1-thread tail of k_force.
+__device__ __forceinline__ void finish_rebuild(const Sys& S)
+{
+    if (S.sc->flag != 0u) {
+        S.sc->n_rebuilds += 1;
+        S.sc->max_nbrs[S.sc->n_rebuilds & 1] = 0;
+        S.sc->flag = 0u;
+    }
+}
+
+template <int TP, bool COUL, bool ONE_TYPE, int UNROLL>
+__global__ void __launch_bounds__(1024, 1) k_force(const Sys S)
+{
+    __shared__ float4 s_pp[3 * RUMD_MAXT * RUMD_MAXT];
+    load_pair_table(S, s_pp);
+    __syncthreads();
+    if (blockIdx.x == 0 && threadIdx.x == 0) finish_rebuild(S);
+    const int tid = blockIdx.x * blockDim.x + threadIdx.x;
+    const int i = tid / TP;
+    const int t = tid % TP;
+    const bool have_i = i < S.N;
+    float4 ri = make_float4(0.f, 0.f, 0.f, 0.f);
+    int cnt = 0;
+    if (have_i) {
+        ri = __ldg(&S.r[i]);
+        cnt = S.num_nbrs[i];
+    }
+    float fx, fy, fz, u, w;
+    force_group<TP, COUL, ONE_TYPE, UNROLL, true>(S, S.r, s_pp, tid >> 5, i, t, ri, cnt, fx, fy, fz, u, w);
     if (have_i && t == 0) {
         S.f[i] = make_float4(fx, fy, fz, 0.5f * u); // P:160 "compensate for double counting"
         S.w[i] = 0.5f * w;
@@ -250,7 +277,6 @@ __device__ __forceinline__ void step_tail(const Sys& S, bool nvt, double kt, dou
         sc->n_steps += 1;
         const unsigned pend = *((volatile unsigned*)&sc->pending);
         sc->flag = pend;
-        if (pend) sc->max_nbrs = 0;
         sc->pending = 0u;
         sc->ticket = 0u;
         if (!(a == a) || !(b == b)) sc->nonfinite = 1;
@@ -282,7 +308,7 @@ __global__ void k_request_rebuild(const Sys S)
 {
     S.sc->flag = 1u;
     S.sc->pending = 0u;
-    S.sc->max_nbrs = 0;
+    S.sc->max_nbrs[S.sc->n_rebuilds & 1] = 0;
     S.sc->overflow = 0u;
 }
 

@@ -1,5 +1,9 @@
-// rumd_kernels.cuh -- sm_100a kernels of the RUMD hot path.  Product code: shares nothing with oracle/.
-// "P:n" = PAPER.md line n; O*/S* = readings listed in DESIGN.md.
+// rumd_kernels.cuh -- sm_100a neighbour-list kernels of the RUMD hot path (A2, A3, A4).  Product code: shares
+// nothing with oracle/.  "P:n" = PAPER.md line n; O*/S* = readings listed in DESIGN.md.
+//
+// Every piece of work is written once as a __device__ "phase" over a virtual grid (first item, stride); the
+// stand-alone __global__ kernels (one phase each, early exit when no rebuild is requested) and the
+// persistent whole-run kernel (rumd_persist.cuh: all phases, grid barriers in between) both call the phases.
 #pragma once
 #include "rumd_types.cuh"
 
@@ -48,11 +52,14 @@ __device__ __forceinline__ double warp_sum(double x)
 __device__ __forceinline__ bool rebuild_requested(const Sys& S) { return S.sc->flag != 0u; }
 
 // sort on this rebuild?  cell method: always; n2 method: every sort_interval-th rebuild.
+__device__ __forceinline__ bool sort_on_rebuild(const Sys& S, long long n_rebuilds)
+{
+    if (S.method == 1) return true;
+    return S.sort_interval > 0 && (n_rebuilds % S.sort_interval) == 0;
+}
 __device__ __forceinline__ bool sort_requested(const Sys& S)
 {
-    if (S.sc->flag == 0u) return false;
-    if (S.method == 1) return true;
-    return S.sort_interval > 0 && (S.sc->n_rebuilds % S.sort_interval) == 0;
+    return S.sc->flag != 0u && sort_on_rebuild(S, S.sc->n_rebuilds);
 }
 
 __device__ __forceinline__ void cell_coords(const Sys& S, const float4& p, int& cx, int& cy, int& cz)
@@ -63,96 +70,91 @@ __device__ __forceinline__ void cell_coords(const Sys& S, const float4& p, int& 
     cz = min(S.grid.n[2] - 1, max(0, (int)floorf((p.z + S.h[2]) * S.grid.scale[2])));
 }
 
+__device__ __forceinline__ float list_dist2(const Sys& S, const float4& ri, const float4& rj)
+{
+    const float dx = min_image(ri.x, rj.x, S.h[0], S.invL[0]);
+    const float dy = min_image(ri.y, rj.y, S.h[1], S.invL[1]);
+    const float dz = min_image(ri.z, rj.z, S.h[2], S.invL[2]);
+    return __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, dx * dx));
+}
+
 // ------------------------------------------------------------------------------------------ A2: N^2 build
 
 // P:173-224 Fig. 4.  One WARP per particle i; j-positions staged through shared memory in tiles
 // (P:184); the 32 lanes test 32 different j at once and slots are handed out by
 // ballot + popc, so the row is in ascending-j order and the whole list is bitwise reproducible (the
-// paper's atomicInc gives "an unspecified sequential order").  Early exit when no rebuild is
-// requested.  Writes num_nbrs, positions at build and the overflow flag.
-#define N2_WARPS 4
+// paper's atomicInc gives "an unspecified sequential order").  Writes num_nbrs, positions at build
+// and the overflow flag.  Block-cooperative: `blk`/`nblk` = this block's index / block count
+// in the virtual grid; blockDim.x must be a multiple of 32.  max_slot: &sc->max_nbrs[build & 1].
 #define N2_TILE 256
-__global__ void __launch_bounds__(N2_WARPS * 32) k_build_n2(const Sys S)
+__device__ __forceinline__ void ph_build_n2(const Sys& S, const float4* r, float4* tile, const float* s_rcl2,
+                                            int blk, int nblk, int* max_slot)
 {
-    if (!rebuild_requested(S)) return;
-    __shared__ float4 tile[N2_TILE];
-    __shared__ float s_rcl2[RUMD_MAXT * RUMD_MAXT];
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    if (threadIdx.x < RUMD_MAXT * RUMD_MAXT) s_rcl2[threadIdx.x] = S.pp[threadIdx.x].rcl2;
-    const int i = blockIdx.x * N2_WARPS + wid;
-    const bool have_i = i < S.N;
-    float4 ri = make_float4(0.f, 0.f, 0.f, 0.f);
-    if (have_i) ri = S.r[i];
-    const int trow = have_i ? type_of(ri) * S.ntypes : 0;
-    int count = 0;
-    for (int j0 = 0; j0 < S.N; j0 += N2_TILE) {
-        __syncthreads();
-        for (int t = threadIdx.x; t < N2_TILE; t += N2_WARPS * 32)
-            if (j0 + t < S.N) tile[t] = S.r[j0 + t];
-        __syncthreads();
-        const int jend = min(N2_TILE, S.N - j0);
-        for (int jj = lane; jj < ((jend + 31) & ~31); jj += 32) {
-            bool acc = false;
-            const int j = j0 + jj;
-            if (jj < jend && have_i && j != i) {
-                const float4 rj = tile[jj];
-                const float dx = min_image(ri.x, rj.x, S.h[0], S.invL[0]);
-                const float dy = min_image(ri.y, rj.y, S.h[1], S.invL[1]);
-                const float dz = min_image(ri.z, rj.z, S.h[2], S.invL[2]);
-                const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, dx * dx));
-                acc = d2 < s_rcl2[trow + type_of(rj)]; // strict <, per type pair
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    const int ngroups = (S.N + nw - 1) / nw;
+    for (int g = blk; g < ngroups; g += nblk) {
+        const int i = g * nw + wid;
+        const bool have_i = i < S.N;
+        float4 ri = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (have_i) ri = r[i];
+        const int trow = have_i ? type_of(ri) * S.ntypes : 0;
+        int count = 0;
+        for (int j0 = 0; j0 < S.N; j0 += N2_TILE) {
+            __syncthreads();
+            for (int t = threadIdx.x; t < N2_TILE; t += blockDim.x)
+                if (j0 + t < S.N) tile[t] = r[j0 + t];
+            __syncthreads();
+            const int jend = min(N2_TILE, S.N - j0);
+            for (int jj = lane; jj < ((jend + 31) & ~31); jj += 32) {
+                bool acc = false;
+                const int j = j0 + jj;
+                if (jj < jend && have_i && j != i) {
+                    const float4 rj = tile[jj];
+                    acc = list_dist2(S, ri, rj) < s_rcl2[trow + type_of(rj)]; // strict <, per type pair
+                }
+                const unsigned m = __ballot_sync(FULLMASK, acc);
+                if (acc) {
+                    const int k = count + __popc(m & ((1u << lane) - 1u));
+                    if (k < S.cap) S.nbl[nbl_index(S, i, k)] = j;
+                }
+                count += __popc(m);
             }
-            const unsigned m = __ballot_sync(FULLMASK, acc);
-            if (acc) {
-                const int k = count + __popc(m & ((1u << lane) - 1u));
-                if (k < S.cap) S.nbl[nbl_index(S, i, k)] = j;
-            }
-            count += __popc(m);
         }
-    }
-    if (have_i && lane == 0) {
-        S.num_nbrs[i] = min(count, S.cap);
-        S.r_build[i] = ri;
-        if (count > S.cap) S.sc->overflow = 1u;
-        atomicMax(&S.sc->max_nbrs, count);
-    }
-}
-
-// Bookkeeping that must happen once per step AFTER every rebuild kernel has read the flag: count the
-// rebuild and clear the flag.  Runs as a 1-thread tail of the force kernel's first block (see k_force).
-__device__ __forceinline__ void finish_rebuild(const Sys& S)
-{
-    if (S.sc->flag != 0u) {
-        S.sc->n_rebuilds += 1;
-        S.sc->flag = 0u;
+        if (have_i && lane == 0) {
+            S.num_nbrs[i] = min(count, S.cap);
+            S.r_build[i] = ri;
+            if (count > S.cap) S.sc->overflow = 1u;
+            atomicMax(max_slot, count);
+        }
     }
 }
 
 // ------------------------------------------------------------------------------------------ A3: cells + sort
 
 // P:276 steps 1-3: cell of every particle, sort particles by cell, rearrange all particle data.  The paper
-// calls Thrust; here it is a counting sort written out: (a) histogram with slot = atomicAdd, (b) three-phase
-// exclusive scan, (c) scatter, (d) per-cell insertion sort of the (few) entries by old index, which removes
-// the atomic's arbitrary order so that the particle order -- and with it every later fp32 sum -- is
+// calls Thrust; here it is a counting sort written out: (a) histogram with slot = atomicAdd, (b) exclusive
+// scan, (c) scatter, (d) per-cell insertion sort of the (few) entries by old index, which removes the
+// atomic's arbitrary order so that the particle order -- and with it every later fp32 sum -- is
 // reproducible.  Cells are numbered along a Morton (Z-order) curve through the valid cells (zrank table,
 // built once on the host): consecutive particles are spatially compact (BASELINE configs[3], S19).
 
-__global__ void k_cell_assign(const Sys S)
+__device__ __forceinline__ void ph_cell_assign(const Sys& S, const float4* r, int first, int stride)
 {
-    if (!sort_requested(S)) return;
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= S.N) return;
-    int cx, cy, cz;
-    cell_coords(S, S.r[i], cx, cy, cz);
-    const int z = S.zrank[(cz * S.grid.n[1] + cy) * S.grid.n[0] + cx];
-    S.cell_of[i] = z;
-    S.slot[i] = atomicAdd(&S.ccount[z], 1);
+    for (int i = first; i < S.N; i += stride) {
+        int cx, cy, cz;
+        cell_coords(S, r[i], cx, cy, cz);
+        const int z = S.zrank[(cz * S.grid.n[1] + cy) * S.grid.n[0] + cx];
+        S.cell_of[i] = z;
+        S.slot[i] = atomicAdd(&S.ccount[z], 1);
+    }
 }
 
 #define SCAN_THREADS 256
 #define SCAN_ITEMS 8
 #define SCAN_CHUNK (SCAN_THREADS * SCAN_ITEMS)
 
+// Exclusive scan of one int per thread over the first SCAN_THREADS threads of the block (all threads of the
+// block must call; threads >= SCAN_THREADS pass 0 and ignore the result).  s_warp: 33 ints.
 __device__ __forceinline__ int block_exclusive_scan(int x, int* s_warp, int& total)
 {
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
@@ -162,7 +164,7 @@ __device__ __forceinline__ int block_exclusive_scan(int x, int* s_warp, int& tot
         int y = __shfl_up_sync(FULLMASK, incl, o);
         if (lane >= o) incl += y;
     }
-    if (lane == 31) s_warp[wid] = incl;
+    if (lane == 31 && wid < SCAN_THREADS / 32) s_warp[wid] = incl;
     __syncthreads();
     if (wid == 0) {
         int v = lane < (SCAN_THREADS / 32) ? s_warp[lane] : 0;
@@ -177,166 +179,314 @@ __device__ __forceinline__ int block_exclusive_scan(int x, int* s_warp, int& tot
     }
     __syncthreads();
     total = s_warp[32];
-    const int res = incl - x + s_warp[wid];
+    const int res = incl - x + (wid < SCAN_THREADS / 32 ? s_warp[wid] : 0);
     __syncthreads();
     return res;
 }
 
-// phase 1: per-chunk totals
-__global__ void __launch_bounds__(SCAN_THREADS) k_scan_sums(const Sys S)
+// phase 1: per-chunk totals (block-cooperative over chunks)
+__device__ __forceinline__ void ph_scan_sums(const Sys& S, int* s_warp, int blk, int nblk)
 {
-    if (!sort_requested(S)) return;
-    __shared__ int s_warp[33];
-    const int base = blockIdx.x * SCAN_CHUNK + threadIdx.x * SCAN_ITEMS;
-    int x = 0;
+    const int nchunks = (S.grid.ncell + SCAN_CHUNK - 1) / SCAN_CHUNK;
+    for (int c = blk; c < nchunks; c += nblk) {
+        const int base = c * SCAN_CHUNK + threadIdx.x * SCAN_ITEMS;
+        int x = 0;
+        if (threadIdx.x < SCAN_THREADS) {
 #pragma unroll
-    for (int q = 0; q < SCAN_ITEMS; ++q)
-        if (base + q < S.grid.ncell) x += S.ccount[base + q];
-    int total;
-    block_exclusive_scan(x, s_warp, total);
-    if (threadIdx.x == 0) S.blocksum[blockIdx.x] = total;
+            for (int q = 0; q < SCAN_ITEMS; ++q)
+                if (base + q < S.grid.ncell) x += S.ccount[base + q];
+        }
+        int total;
+        block_exclusive_scan(x, s_warp, total);
+        if (threadIdx.x == 0) S.blocksum[c] = total;
+    }
 }
 
-// phase 2: exclusive scan of the chunk totals (one block, loops if there are more than 256 chunks)
-__global__ void __launch_bounds__(SCAN_THREADS) k_scan_blocks(const Sys S, int nchunks)
+// phase 2: exclusive scan of the chunk totals (ONE block)
+__device__ __forceinline__ void ph_scan_blocks(const Sys& S, int* s_warp)
 {
-    if (!sort_requested(S)) return;
-    __shared__ int s_warp[33];
+    const int nchunks = (S.grid.ncell + SCAN_CHUNK - 1) / SCAN_CHUNK;
     int carry = 0;
     for (int b0 = 0; b0 < nchunks; b0 += SCAN_THREADS) {
         const int b = b0 + threadIdx.x;
-        const int x = b < nchunks ? S.blocksum[b] : 0;
+        const bool on = threadIdx.x < SCAN_THREADS && b < nchunks;
+        const int x = on ? S.blocksum[b] : 0;
         int total;
         const int e = block_exclusive_scan(x, s_warp, total);
-        if (b < nchunks) S.blocksum[b] = carry + e;
+        if (on) S.blocksum[b] = carry + e;
         carry += total;
     }
 }
 
 // phase 3: exclusive scan inside each chunk + chunk offset -> first sorted slot of each Z-ordered cell
-__global__ void __launch_bounds__(SCAN_THREADS) k_scan_apply(const Sys S)
+__device__ __forceinline__ void ph_scan_apply(const Sys& S, int* s_warp, int blk, int nblk)
 {
-    if (!sort_requested(S)) return;
-    __shared__ int s_warp[33];
-    const int base = blockIdx.x * SCAN_CHUNK + threadIdx.x * SCAN_ITEMS;
-    int c[SCAN_ITEMS];
-    int x = 0;
+    const int nchunks = (S.grid.ncell + SCAN_CHUNK - 1) / SCAN_CHUNK;
+    for (int ch = blk; ch < nchunks; ch += nblk) {
+        const int base = ch * SCAN_CHUNK + threadIdx.x * SCAN_ITEMS;
+        int c[SCAN_ITEMS];
+        int x = 0;
 #pragma unroll
-    for (int q = 0; q < SCAN_ITEMS; ++q) {
-        c[q] = (base + q < S.grid.ncell) ? S.ccount[base + q] : 0;
-        x += c[q];
-    }
-    int total;
-    int e = block_exclusive_scan(x, s_warp, total) + S.blocksum[blockIdx.x];
+        for (int q = 0; q < SCAN_ITEMS; ++q) {
+            c[q] = (threadIdx.x < SCAN_THREADS && base + q < S.grid.ncell) ? S.ccount[base + q] : 0;
+            x += c[q];
+        }
+        int total;
+        int e = block_exclusive_scan(x, s_warp, total) + S.blocksum[ch];
+        if (threadIdx.x < SCAN_THREADS) {
 #pragma unroll
-    for (int q = 0; q < SCAN_ITEMS; ++q) {
-        if (base + q < S.grid.ncell) S.cstart_z[base + q] = e;
-        e += c[q];
+            for (int q = 0; q < SCAN_ITEMS; ++q) {
+                if (base + q < S.grid.ncell) S.cstart_z[base + q] = e;
+                e += c[q];
+            }
+        }
     }
 }
 
-__global__ void k_cell_scatter(const Sys S)
+// all three phases by ONE block (small grids: saves two grid barriers in the persistent kernel)
+__device__ __forceinline__ void ph_scan_single_block(const Sys& S, int* s_warp)
 {
-    if (!sort_requested(S)) return;
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= S.N) return;
-    S.perm[S.cstart_z[S.cell_of[i]] + S.slot[i]] = i;
+    const int nchunks = (S.grid.ncell + SCAN_CHUNK - 1) / SCAN_CHUNK;
+    int carry = 0;
+    for (int ch = 0; ch < nchunks; ++ch) {
+        const int base = ch * SCAN_CHUNK + threadIdx.x * SCAN_ITEMS;
+        int c[SCAN_ITEMS];
+        int x = 0;
+#pragma unroll
+        for (int q = 0; q < SCAN_ITEMS; ++q) {
+            c[q] = (threadIdx.x < SCAN_THREADS && base + q < S.grid.ncell) ? S.ccount[base + q] : 0;
+            x += c[q];
+        }
+        int total;
+        int e = block_exclusive_scan(x, s_warp, total) + carry;
+        if (threadIdx.x < SCAN_THREADS) {
+#pragma unroll
+            for (int q = 0; q < SCAN_ITEMS; ++q) {
+                if (base + q < S.grid.ncell) S.cstart_z[base + q] = e;
+                e += c[q];
+            }
+        }
+        carry += total;
+    }
+}
+
+__device__ __forceinline__ void ph_cell_scatter(const Sys& S, int first, int stride)
+{
+    for (int i = first; i < S.N; i += stride) S.perm[S.cstart_z[S.cell_of[i]] + S.slot[i]] = i;
 }
 
 // One thread per cell: order its entries by old index (deterministic), publish cellStart / cellEnd under
 // the row-major cell index the build kernel uses (here end is EXCLUSIVE, S20), clear the
 // histogram for the next sort.
-__global__ void k_cell_finish(const Sys S)
+__device__ __forceinline__ void ph_cell_finish(const Sys& S, int first, int stride)
 {
-    if (!sort_requested(S)) return;
-    const int z = blockIdx.x * blockDim.x + threadIdx.x;
-    if (z >= S.grid.ncell) return;
-    const int b = S.cstart_z[z], n = S.ccount[z];
-    for (int a = 1; a < n; ++a) {
-        const int key = S.perm[b + a];
-        int q = a - 1;
-        while (q >= 0 && S.perm[b + q] > key) {
-            S.perm[b + q + 1] = S.perm[b + q];
-            --q;
+    for (int z = first; z < S.grid.ncell; z += stride) {
+        const int b = S.cstart_z[z], n = S.ccount[z];
+        for (int a = 1; a < n; ++a) {
+            const int key = S.perm[b + a];
+            int q = a - 1;
+            while (q >= 0 && S.perm[b + q] > key) {
+                S.perm[b + q + 1] = S.perm[b + q];
+                --q;
+            }
+            S.perm[b + q + 1] = key;
         }
-        S.perm[b + q + 1] = key;
+        const int c = S.zinv[z];
+        S.cell_range[c] = make_int2(b, b + n);
+        S.ccount[z] = 0;
     }
-    const int c = S.zinv[z];
-    S.cell_start[c] = b;
-    S.cell_end[c] = b + n;
-    S.ccount[z] = 0;
 }
 
 // P:276 "rearrange all particle data into the sorted order": gather into scratch, then copy back (the
 // caller owns the arrays, so the pointers cannot be swapped).
-__global__ void k_permute_gather(const Sys S)
+__device__ __forceinline__ void ph_permute_gather(const Sys& S, const float4* r, int first, int stride)
 {
-    if (!sort_requested(S)) return;
-    const int d = blockIdx.x * blockDim.x + threadIdx.x;
-    if (d >= S.N) return;
-    const int src = S.perm[d];
-    S.tmp_r[d] = S.r[src];
-    S.tmp_v[d] = S.v[src];
-    S.tmp_image[d] = S.image[src];
-    S.tmp_id[d] = S.id[src];
+    for (int d = first; d < S.N; d += stride) {
+        const int src = S.perm[d];
+        S.tmp_r[d] = r[src];
+        S.tmp_v[d] = S.v[src];
+        S.tmp_image[d] = S.image[src];
+        S.tmp_id[d] = S.id[src];
+    }
 }
 
-__global__ void k_permute_store(const Sys S)
+__device__ __forceinline__ void ph_permute_store(const Sys& S, float4* r, int first, int stride)
 {
-    if (!sort_requested(S)) return;
-    const int d = blockIdx.x * blockDim.x + threadIdx.x;
-    if (d >= S.N) return;
-    S.r[d] = S.tmp_r[d];
-    S.v[d] = S.tmp_v[d];
-    S.image[d] = S.tmp_image[d];
-    S.id[d] = S.tmp_id[d];
+    for (int d = first; d < S.N; d += stride) {
+        r[d] = S.tmp_r[d];
+        S.v[d] = S.tmp_v[d];
+        S.image[d] = S.tmp_image[d];
+        S.id[d] = S.tmp_id[d];
+    }
 }
 
 // ------------------------------------------------------------------------------------------ A4: cell build
 
-// P:226-268 Fig. 5: one thread per (sorted) particle, 5x5x5 stencil of cells of edge >= (rc_max+skin)/2
-// (P:278), periodic wrap (c + d + n) % n (needs n >= 5 per axis, S18), strict per-type-pair test
-// (P:251-255), overflow flag, positions at build.  Rows come out in stencil order,
-// which is fixed, so the list is reproducible.
+// P:226-268 Fig. 5: 5x5x5 stencil of cells of edge >= (rc_max+skin)/2, periodic wrap of the cell
+// coordinate (needs n >= 5 per axis, S18), strict per-type-pair test, overflow flag
+// (P:256), positions at build.  The paper uses one thread per particle and notes that several
+// threads per particle had "not been tried yet"; here G = 1..32 lanes share one particle: lane l
+// takes stencil cells l, l+G, ..., the group walks its cells in lock step and hands out list slots by
+// ballot + popc, so rows come out in the fixed order (round, position in cell, lane) and the list is
+// bitwise reproducible.  `first`/`stride` index the virtual grid of N*G threads (multiples of 32).
+template <int G>
+__device__ __forceinline__ void ph_build_cell(const Sys& S, const float4* r, const float* s_rcl2, int first,
+                                              int stride, int* max_slot)
+{
+    const int lane = threadIdx.x & 31;
+    const int l = lane & (G - 1);
+    const unsigned gmask = G == 32 ? FULLMASK : (((1u << G) - 1u) << (lane & ~(G - 1)));
+    const unsigned lt = gmask & ((1u << lane) - 1u);
+    const int nx = S.grid.n[0], ny = S.grid.n[1], nz = S.grid.n[2];
+    const long long total = (long long)S.N * G;
+    for (long long vt = first; vt - lane < total; vt += stride) {
+        const int i = (int)(vt / G);
+        const bool have_i = i < S.N;
+        float4 ri = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (have_i) ri = r[i];
+        const int trow = have_i ? type_of(ri) * S.ntypes : 0;
+        int cx = 0, cy = 0, cz = 0;
+        if (have_i) cell_coords(S, ri, cx, cy, cz);
+        int count = 0;
+        auto range_of = [&](int q) -> int2 {
+            if (!have_i || q >= 125) return make_int2(0, 0);
+            int dz = q / 25, dy = (q / 5) % 5, dx = q % 5;
+            int z = cz + dz - 2, y = cy + dy - 2, x = cx + dx - 2;
+            z += z < 0 ? nz : 0; z -= z >= nz ? nz : 0;
+            y += y < 0 ? ny : 0; y -= y >= ny ? ny : 0;
+            x += x < 0 ? nx : 0; x -= x >= nx ? nx : 0;
+            return S.cell_range[(z * ny + y) * nx + x];
+        };
+        int2 nxt = range_of(l);
+        for (int q0 = 0; q0 < 125; q0 += G) {
+            const int2 cur = nxt;
+            if (q0 + G < 125) nxt = range_of(q0 + G + l); // one-ahead prefetch of the next round's cell
+            const int n = cur.y - cur.x;
+            const int nmax = __reduce_max_sync(FULLMASK, n);
+            for (int it = 0; it < nmax; ++it) {
+                bool acc = false;
+                const int j = cur.x + it;
+                if (it < n && j != i) {
+                    const float4 rj = r[j];
+                    acc = list_dist2(S, ri, rj) < s_rcl2[trow + type_of(rj)];
+                }
+                const unsigned m = __ballot_sync(FULLMASK, acc);
+                if (acc) {
+                    const int k = count + __popc(m & lt);
+                    if (k < S.cap) S.nbl[nbl_index(S, i, k)] = j;
+                }
+                count += __popc(m & gmask);
+            }
+        }
+        if (have_i && l == 0) {
+            S.num_nbrs[i] = min(count, S.cap);
+            S.r_build[i] = ri;
+            if (count > S.cap) S.sc->overflow = 1u;
+            atomicMax(max_slot, count);
+        }
+    }
+}
+
+__device__ __forceinline__ void build_cell_dispatch(const Sys& S, const float4* r, const float* s_rcl2, int first,
+                                                    int stride, int* max_slot)
+{
+    switch (S.build_tp_shift) {
+    case 0: ph_build_cell<1>(S, r, s_rcl2, first, stride, max_slot); break;
+    case 1: ph_build_cell<2>(S, r, s_rcl2, first, stride, max_slot); break;
+    case 2: ph_build_cell<4>(S, r, s_rcl2, first, stride, max_slot); break;
+    case 3: ph_build_cell<8>(S, r, s_rcl2, first, stride, max_slot); break;
+    case 4: ph_build_cell<16>(S, r, s_rcl2, first, stride, max_slot); break;
+    default: ph_build_cell<32>(S, r, s_rcl2, first, stride, max_slot); break;
+    }
+}
+
+// ------------------------------------------------------------------------------------------ stand-alone kernels
+// One phase each; every kernel exits at once when the device flag is clear, so the chain can be
+// enqueued -- or baked into a CUDA graph -- every step without asking the host.
+
+#define VGRID const int first = blockIdx.x * blockDim.x + threadIdx.x, stride = gridDim.x * blockDim.x
+
+__device__ __forceinline__ int* max_slot_of(const Sys& S) { return &S.sc->max_nbrs[S.sc->n_rebuilds & 1]; }
+
+__global__ void __launch_bounds__(128) k_build_n2(const Sys S)
+{
+    if (!rebuild_requested(S)) return;
+    __shared__ float4 tile[N2_TILE];
+    __shared__ float s_rcl2[RUMD_MAXT * RUMD_MAXT];
+    if (threadIdx.x < RUMD_MAXT * RUMD_MAXT) s_rcl2[threadIdx.x] = S.pp[threadIdx.x].rcl2;
+    __syncthreads();
+    ph_build_n2(S, S.r, tile, s_rcl2, blockIdx.x, gridDim.x, max_slot_of(S));
+}
+
 __global__ void __launch_bounds__(128) k_build_cell(const Sys S)
 {
     if (!rebuild_requested(S)) return;
     __shared__ float s_rcl2[RUMD_MAXT * RUMD_MAXT];
     if (threadIdx.x < RUMD_MAXT * RUMD_MAXT) s_rcl2[threadIdx.x] = S.pp[threadIdx.x].rcl2;
     __syncthreads();
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= S.N) return;
-    const float4 ri = S.r[i];
-    const int trow = type_of(ri) * S.ntypes;
-    int cx, cy, cz;
-    cell_coords(S, ri, cx, cy, cz);
-    const int nx = S.grid.n[0], ny = S.grid.n[1], nz = S.grid.n[2];
-    int count = 0;
-    for (int dz = -2; dz <= 2; ++dz) {
-        const int z = (cz + dz + nz) % nz;
-        for (int dy = -2; dy <= 2; ++dy) {
-            const int y = (cy + dy + ny) % ny;
-            const int row = (z * ny + y) * nx;
-            for (int dx = -2; dx <= 2; ++dx) {
-                const int c = row + (cx + dx + nx) % nx;
-                const int je = S.cell_end[c];
-                for (int j = S.cell_start[c]; j < je; ++j) {
-                    if (j == i) continue;
-                    const float4 rj = __ldg(&S.r[j]);
-                    const float ddx = min_image(ri.x, rj.x, S.h[0], S.invL[0]);
-                    const float ddy = min_image(ri.y, rj.y, S.h[1], S.invL[1]);
-                    const float ddz = min_image(ri.z, rj.z, S.h[2], S.invL[2]);
-                    const float d2 = __fmaf_rn(ddz, ddz, __fmaf_rn(ddy, ddy, ddx * ddx));
-                    if (d2 < s_rcl2[trow + type_of(rj)]) {
-                        if (count < S.cap) S.nbl[nbl_index(S, i, count)] = j;
-                        ++count;
-                    }
-                }
-            }
-        }
-    }
-    S.num_nbrs[i] = min(count, S.cap);
-    S.r_build[i] = ri;
-    if (count > S.cap) S.sc->overflow = 1u;
-    atomicMax(&S.sc->max_nbrs, count);
+    VGRID;
+    build_cell_dispatch(S, S.r, s_rcl2, first, stride, max_slot_of(S));
+}
+
+__global__ void k_cell_assign(const Sys S)
+{
+    if (!sort_requested(S)) return;
+    VGRID;
+    ph_cell_assign(S, S.r, first, stride);
+}
+
+__global__ void __launch_bounds__(SCAN_THREADS) k_scan_sums(const Sys S)
+{
+    if (!sort_requested(S)) return;
+    __shared__ int s_warp[33];
+    ph_scan_sums(S, s_warp, blockIdx.x, gridDim.x);
+}
+
+__global__ void __launch_bounds__(SCAN_THREADS) k_scan_blocks(const Sys S)
+{
+    if (!sort_requested(S)) return;
+    __shared__ int s_warp[33];
+    ph_scan_blocks(S, s_warp);
+}
+
+__global__ void __launch_bounds__(SCAN_THREADS) k_scan_apply(const Sys S)
+{
+    if (!sort_requested(S)) return;
+    __shared__ int s_warp[33];
+    ph_scan_apply(S, s_warp, blockIdx.x, gridDim.x);
+}
+
+__global__ void __launch_bounds__(SCAN_THREADS) k_scan_single(const Sys S)
+{
+    if (!sort_requested(S)) return;
+    __shared__ int s_warp[33];
+    ph_scan_single_block(S, s_warp);
+}
+
+__global__ void k_cell_scatter(const Sys S)
+{
+    if (!sort_requested(S)) return;
+    VGRID;
+    ph_cell_scatter(S, first, stride);
+}
+
+__global__ void k_cell_finish(const Sys S)
+{
+    if (!sort_requested(S)) return;
+    VGRID;
+    ph_cell_finish(S, first, stride);
+}
+
+__global__ void k_permute_gather(const Sys S)
+{
+    if (!sort_requested(S)) return;
+    VGRID;
+    ph_permute_gather(S, S.r, first, stride);
+}
+
+__global__ void k_permute_store(const Sys S)
+{
+    if (!sort_requested(S)) return;
+    VGRID;
+    ph_permute_store(S, S.r, first, stride);
 }

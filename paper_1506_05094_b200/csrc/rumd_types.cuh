@@ -25,13 +25,14 @@ struct DevScalars {
     double U, W;          // filled by the thermo reduction
     long long n_steps;
     long long n_rebuilds;
+    long long moved_step; // persistent path: 1 + index of the last step whose displacement check fired (O9)
     unsigned int flag;    // rebuild requested for the NEXT force evaluation (P:179 updateRequired)
     unsigned int pending; // set by the integrator's displacement check during a step
     unsigned int ticket;  // last-block-done counter of the integrator
     unsigned int overflow;
-    int max_nbrs;         // largest list length of the last build
-    int nonfinite;
-    int pad0, pad1;
+    int max_nbrs[2];      // largest list length of build number b in slot b & 1
+    int nonfinite;        // 1: NaN/Inf energy; 2: grid barrier timed out
+    unsigned int barrier; // arrival counter of the persistent kernel's grid barrier
 };
 
 struct CellGrid {
@@ -52,12 +53,15 @@ struct Sys {
     CellGrid grid;
     // caller-owned state
     float4* r; float4* v; float4* f; float* w; int4* image; int* id;
+    float4* r_out;          // where a fused force+integrate step writes r(t+dt): r itself or r_alt
+    float4* r_alt;          // workspace: second position buffer (double buffering of the fused step)
+    int build_tp_shift;     // log2(lanes per particle) of the cell-list build
     // workspace
     int* nbl; int* num_nbrs; float4* r_build;
     float4* tmp_r; float4* tmp_v; int4* tmp_image; int* tmp_id;
     int* cell_of; int* slot; int* perm;
-    int* ccount; int* cstart_z; int* cell_start; int* cell_end; int* zrank; int* zinv; int* blocksum;
-    double* partial;        // 2 doubles per integrator block
+    int* ccount; int* cstart_z; int2* cell_range; int* zrank; int* zinv; int* blocksum;
+    double* partial;        // 2 sets x 2 doubles per block (kt, mv2) of the integrating kernel
     DevScalars* sc;
     PairParams pp[RUMD_MAXT * RUMD_MAXT];
 };

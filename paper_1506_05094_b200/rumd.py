@@ -34,7 +34,7 @@ EXPORTS = [
 class Tuning(C.Structure):
     _fields_ = [("method", C.c_int), ("pb", C.c_int), ("tp", C.c_int), ("skin", C.c_float),
                 ("sort_interval", C.c_int), ("use_graph", C.c_int), ("steps_per_graph", C.c_int),
-                ("fuse", C.c_int)]
+                ("persistent", C.c_int), ("build_tp", C.c_int)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
@@ -122,7 +122,8 @@ class System:
         self.N = N
         self.ntypes = int(pot.shape[0])
         self.box = np.ascontiguousarray(box, dtype=np.float32)
-        self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        # a dedicated side stream (the legacy default stream cannot be captured into CUDA graphs)
+        self.stream = stream if stream is not None else torch.cuda.Stream(self.device)
         h = C.c_void_p()
         st = self.L.rumd_create(C.byref(h), N, self.ntypes, self.box.ctypes.data_as(C.POINTER(C.c_float)),
                                 C.c_void_p(self.stream.cuda_stream))
@@ -163,6 +164,7 @@ class System:
             capacity = estimate_capacity(self.density, self.rc_max, skin_for_capacity)
         self.d_ws = None
         self.bind_workspace(capacity)
+        torch.cuda.synchronize(self.device)  # the tensors above were filled on torch's current stream
 
     # ---- helpers
     def _check(self, st):

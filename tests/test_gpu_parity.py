@@ -84,8 +84,10 @@ def check_forces(sys_, r64, types, box, pot):
     err = np.sqrt(((st["F"].astype(np.float64) - F) ** 2).sum(1)).max()
     assert err <= FORCE_TOL * rms, "max|dF| = %g > 1e-4 * rms|F| = %g" % (err, FORCE_TOL * rms)
     th = sys_.get_thermo()
-    assert th["U"] == pytest.approx(u.sum(), rel=ENERGY_TOL)
-    assert th["W"] == pytest.approx(w.sum(), rel=ENERGY_TOL)
+    # 1e-5 relative; the scale is sum_i |u_i| (= |U| whenever all u_i have one sign, i.e. in every equilibrated
+    # state; on the sc-lattice KA start U nearly cancels and |U| itself is not a meaningful scale, S29)
+    assert abs(th["U"] - u.sum()) <= ENERGY_TOL * np.abs(u).sum()
+    assert abs(th["W"] - w.sum()) <= ENERGY_TOL * np.abs(w).sum()
     # per-particle energies and virials (absolute tolerance scaled by their rms)
     assert np.abs(st["u"] - u).max() <= 1e-5 * max(1.0, np.abs(u).max())
     assert np.abs(st["w"] - w).max() <= 1e-5 * max(1.0, np.abs(w).max())
@@ -130,8 +132,10 @@ def test_perfect_lattice_energy_and_counts(rumd):
     assert np.all(cnt == 78)
     th = s.get_thermo()
     F, u, w = oracle.forces_allpairs(wl.r.astype(np.float64), wl.types, wl.box.astype(np.float64), wl.pot)
-    assert th["U"] == pytest.approx(u.sum(), rel=ENERGY_TOL)
-    assert th["W"] == pytest.approx(w.sum(), rel=ENERGY_TOL)
+    # 1e-5 relative; the scale is sum_i |u_i| (= |U| whenever all u_i have one sign, i.e. in every equilibrated
+    # state; on the sc-lattice KA start U nearly cancels and |U| itself is not a meaningful scale, S29)
+    assert abs(th["U"] - u.sum()) <= ENERGY_TOL * np.abs(u).sum()
+    assert abs(th["W"] - w.sum()) <= ENERGY_TOL * np.abs(w).sum()
     assert np.abs(s.state()["F"]).max() < 1e-3
     s.close()
 
@@ -283,13 +287,62 @@ def test_graph_and_plain_launch_agree_bitwise(rumd):
     res = []
     for g in (0, 1):
         s = rumd.from_workload(wl)
-        s.set_tuning(use_graph=g, steps_per_graph=8)
+        s.set_tuning(persistent=0, use_graph=g, steps_per_graph=8)
         s.run_steps(43)
         st = s.state()
         res.append((st["r"], st["v"]))
         assert s.get_thermo()["n_steps"] == 43
         s.close()
     assert np.array_equal(res[0][0], res[1][0]) and np.array_equal(res[0][1], res[1][1])
+
+
+@pytest.mark.parametrize("kind,kw,method,tp,nsteps", [
+    ("lj", dict(ncell=6), "n2", 16, 61),        # odd step count: positions end in the alternate buffer
+    ("lj", dict(ncell=8), "cell", 4, 80),       # N = 2048
+    ("ch", dict(n=10), "cell", 8, 40),
+])
+def test_persistent_kernel_equals_per_step_kernels_bitwise_nve(rumd, kind, kw, method, tp, nsteps):
+    """A7: the one-launch cooperative kernel (fused force + integrate, grid barriers, in-kernel rebuilds) and
+    the per-step kernel chain run the same arithmetic in the same order: NVE trajectories are bit-identical,
+    including across list rebuilds and spatial sorts."""
+    wl = perturbed(make(kind, **kw))
+    wl.integrator = W.NVE
+    res = []
+    for persistent in (1, 0):
+        s = rumd.from_workload(wl)
+        s.set_tuning(method=rumd.NB_CELL if method == "cell" else rumd.NB_N2, tp=tp, pb=256 // tp,
+                     persistent=persistent, use_graph=0)
+        s.run_steps(nsteps)
+        s.run_steps(7)
+        th = s.get_thermo()
+        st = s.state()
+        res.append((st, th))
+        assert th["n_steps"] == nsteps + 7
+        s.close()
+    (a, ta), (b, tb) = res
+    assert ta["n_rebuilds"] == tb["n_rebuilds"] and ta["n_rebuilds"] >= 2
+    for key in ("r", "v", "F", "u", "w", "image"):
+        assert np.array_equal(a[key], b[key]), key
+    assert ta["U"] == tb["U"] and ta["max_nbrs"] == tb["max_nbrs"]
+    assert ta["K"] == pytest.approx(tb["K"], rel=1e-12)
+
+
+def test_persistent_kernel_nvt_tracks_per_step_kernels(rumd):
+    """NVT: both paths add the same per-particle fp64 terms but group them by different block sizes, so xi
+    agrees to rounding, not bitwise."""
+    wl = perturbed(make("ka", N=4096))
+    res = []
+    for persistent in (1, 0):
+        s = rumd.from_workload(wl)
+        s.set_tuning(method=rumd.NB_CELL, tp=8, pb=32, persistent=persistent)
+        s.run_steps(30)
+        th = s.get_thermo()
+        res.append((s.state(), th))
+        s.close()
+    (a, ta), (b, tb) = res
+    assert ta["xi"] == pytest.approx(tb["xi"], rel=1e-9)
+    assert ta["H"] == pytest.approx(tb["H"], rel=1e-7)
+    assert np.abs(a["r"] - b["r"]).max() < 1e-4
 
 
 def test_snapshot_restore_and_host_buffers(rumd):
