@@ -187,6 +187,12 @@ rumd_status rumd_profile_step(rumd_system* s, float* ms_out, int* did_rebuild_ou
  * (roofline measurement; the outputs d_f, d_w are simply recomputed).  us_per_launch: host.  Synchronizes. */
 rumd_status rumd_time_force(rumd_system* s, int reps, float* us_per_launch);
 
+/* Runs nsteps time steps in the persistent kernel with the per-phase SM-cycle counters of block 0 switched
+ * on.  out8: host, 8 doubles = microseconds PER STEP spent by block 0 in {rebuild phases, force + integrate,
+ * block reductions, grid barrier wait, post-barrier reduction}, whole kernel per step, number of rebuilds,
+ * grid size.  Advances the simulation by nsteps.  Synchronizes. */
+rumd_status rumd_profile_persistent(rumd_system* s, int nsteps, double* out8);
+
 const char* rumd_last_error(const rumd_system* s);
 const char* rumd_version(void);
 

@@ -54,6 +54,7 @@ struct rumd_system {
     int num_sms = 148;
     int persist_grid_for = -1; // tuning signature the cached persistent grid belongs to
     int persist_grid = 0, persist_threads = 0;
+    long long* prof_buf = nullptr;
     std::string err;
 };
 
@@ -166,6 +167,7 @@ static size_t carve(rumd_system* s, char* base, int cap)
     // (kt, mv2) per block: integrator kernel (N/128 blocks) or persistent kernel (2 sets x <= 4096 blocks)
     const size_t nblk = std::max<size_t>((N + 31) / 32 + 1, 2 * 4096);
     p = take(nblk * 16); if (base) S.partial = (double*)p;
+    p = take(8 * 8); if (base) s->prof_buf = (long long*)p;
     return off;
 }
 
@@ -426,6 +428,7 @@ static rumd_status refresh(rumd_system* s)
         S.L[k] = s->box[k];
         S.h[k] = 0.5f * s->box[k];
         S.invL[k] = (float)(1.0 / (double)s->box[k]);
+        S.hin[k] = (float)(0.5 * (double)s->box[k] - (rcm + 2.0 * skin) - 1e-3);
         if (rcm + skin > 0.5 * (double)s->box[k])
             return fail(s, RUMD_ERR_BOX_TOO_SMALL, "rc_max + skin = %g exceeds L/2 = %g on axis %d", rcm + skin,
                         0.5 * s->box[k], k);
@@ -458,6 +461,8 @@ static rumd_status refresh(rumd_system* s)
                 const double fc = (12 * c12 * ri6 * ri6 - 6 * c6 * ri6) / p.rc_lj;
                 q.c12 = (float)c12;
                 q.c6 = (float)c6;
+                q.c12x12 = (float)(12.0 * c12);
+                q.c6x6 = (float)(6.0 * c6);
                 q.rc2_lj = (float)(p.rc_lj * p.rc_lj);
                 q.fc_lj = (float)fc;
                 q.k0_lj = (float)(uc + p.rc_lj * fc);
@@ -565,11 +570,7 @@ template <int TP, bool COUL, bool ONE> struct PersistKernel {
     static const void* run(rumd_system*) { return (const void*)&k_persist<TP, COUL, ONE, UnrollOf<TP>::value>; }
 };
 
-static int persist_threads_of(const rumd_tuning& t)
-{
-    int th = t.pb * t.tp / 256 * 256;
-    return std::min(512, std::max(256, th));
-}
+static int persist_threads_of(const rumd_tuning&) { return PERSIST_THREADS; }
 
 // n steps in ONE cooperative launch.  The grid is sized to cover N*tp virtual threads when it can be
 // co-resident, else to the co-residency limit (the kernel strides).
@@ -589,7 +590,7 @@ static rumd_status launch_persistent(rumd_system* s, int nsteps)
         s->persist_threads = threads;
         s->persist_grid_for = sig;
     }
-    CUDA_TRY(s, cudaMemsetAsync(&s->S.sc->barrier, 0, sizeof(unsigned), s->stream));
+    CUDA_TRY(s, cudaMemsetAsync(s->S.sc->bar, 0, 2 * sizeof(unsigned long long), s->stream));
     int nvt = s->integ == RUMD_INT_NVT_NOSE_HOOVER;
     void* args[] = {(void*)&s->S, (void*)&nsteps, (void*)&nvt};
     CUDA_TRY(s, cudaLaunchCooperativeKernel(fn, dim3(s->persist_grid), dim3(s->persist_threads), args, 0, s->stream));
@@ -704,9 +705,9 @@ extern "C" rumd_status rumd_run_steps(rumd_system* s, long n)
     if (n < 0) return fail(s, RUMD_ERR_INVALID_ARG, "negative step count");
     if (n == 0) return RUMD_OK;
     if (s->tune.persistent) {
-        // one cooperative launch per <= 2^20 steps (the step counter inside the kernel is an int)
+        // one cooperative launch per <= 2^16 steps (keeps the 32-bit arrival count of the grid barrier in range)
         for (long left = n; left > 0;) {
-            const int chunk = (int)std::min<long>(left, 1L << 20);
+            const int chunk = (int)std::min<long>(left, 1L << 16);
             st = launch_persistent(s, chunk);
             if (st != RUMD_OK) return st;
             left -= chunk;
@@ -912,6 +913,39 @@ extern "C" rumd_status rumd_time_force(rumd_system* s, int reps, float* us_per_l
     s->launches += 2LL * reps;
     if (es != cudaSuccess) return fail(s, RUMD_ERR_CUDA, "force timing failed: %s", cudaGetErrorString(es));
     *us_per_launch = 1000.f * ms / (float)reps;
+    return RUMD_OK;
+}
+
+// Where the time of the persistent kernel goes: runs n steps with the cycle counters of block 0 switched on.
+extern "C" rumd_status rumd_profile_persistent(rumd_system* s, int nsteps, double* out8)
+{
+    rumd_status st = ready(s, true);
+    if (st != RUMD_OK) return st;
+    if (nsteps < 1 || !out8) return fail(s, RUMD_ERR_INVALID_ARG, "bad arguments");
+    CUDA_TRY(s, cudaMemsetAsync(s->prof_buf, 0, 64, s->stream));
+    s->S.prof = s->prof_buf;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0);
+    cudaEventCreate(&e1);
+    cudaEventRecord(e0, s->stream);
+    st = launch_persistent(s, nsteps);
+    cudaEventRecord(e1, s->stream);
+    s->S.prof = nullptr;
+    long long h[8];
+    cudaError_t e = cudaMemcpyAsync(h, s->prof_buf, 64, cudaMemcpyDeviceToHost, s->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    if (st != RUMD_OK) return st;
+    if (e != cudaSuccess) return fail(s, RUMD_ERR_CUDA, "profiling run failed: %s", cudaGetErrorString(e));
+    // convert cycles to microseconds per step with the kernel's own total (cycles <-> event time)
+    const double us_total = 1000.0 * ms, cyc_total = (double)h[5];
+    for (int q = 0; q < 5; ++q) out8[q] = cyc_total > 0 ? (double)h[q] / cyc_total * us_total / nsteps : 0.0;
+    out8[5] = us_total / nsteps;
+    out8[6] = (double)h[6];
+    out8[7] = (double)h[7];
     return RUMD_OK;
 }
 

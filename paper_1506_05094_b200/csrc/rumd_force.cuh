@@ -5,42 +5,48 @@
 
 // ------------------------------------------------------------------------------------------ pair function
 
-// O3/O4/O5 for one listed pair: adds f_SF(r) d/r to (fx,fy,fz), u_SF to u and r f_SF to w (the halving of u
-// and w is done once per particle).  Every term applies its own cutoff (S5, strict <, S3).
-// 1/r^2 comes from MUFU.RCP plus one Newton step (the r^-12 term amplifies its error six-fold); 1/r, used
-// only in the small shifted-force terms and Coulomb, from MUFU.RSQ plus one Newton step.
-template <bool COUL>
-__device__ __forceinline__ void pair_accumulate(const float4 p0, const float4 p1, const float4 p2, bool ok,
+// O3/O4/O5 for one listed pair: adds f_SF(r) d/r to (fx,fy,fz) and -- only when ENERGY -- u_SF to u and
+// r f_SF to w (the halving of u and w is done once per particle).  Every term applies its own cutoff
+// (S5, strict <, S3).  Branch-free: a warp almost never has all 32 pairs outside the cutoff, so the terms are
+// computed for every pair and selected.  1/r = MUFU.RSQ + one Newton step (the r^-14 force term amplifies its
+// error 14-fold); 1/r^2 = (1/r)^2.
+//   pf = (12 c12, 6 c6, rc_lj^2, fc_lj)   pc = (qq, rc_c^2, fc_c, -)   pe = (c12, c6, k0_lj, k0_c)
+template <bool COUL, bool ENERGY>
+__device__ __forceinline__ void pair_accumulate(const float4 pf, const float4 pc, const float4 pe, bool ok,
                                                 float dx, float dy, float dz, float& fx, float& fy, float& fz,
                                                 float& u, float& w)
 {
     const float r2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, dx * dx));
-    if (!(ok && r2 < p2.z)) return; // p2.z = max rc^2 of the pair's terms
     float y = rsqrtf(r2);
     y = y * __fmaf_rn(-0.5f * r2, y * y, 1.5f); // Newton: y <- y (3 - r2 y^2)/2
-    const float rinv = y;
-    float q = __fdividef(1.0f, r2);
-    q = __fmaf_rn(q, __fmaf_rn(-r2, q, 1.0f), q); // Newton: q <- q + q (1 - r2 q)
-    const float rinv2 = q;
-    const float r = r2 * rinv;
-    float fr = 0.f, uu = 0.f; // fr = f_SF(r) / r
-    if (r2 < p0.z) {          // LJ term, p0 = (c12, c6, rc2_lj, fc_lj), p1.x = k0_lj
-        const float rinv6 = rinv2 * rinv2 * rinv2;
-        const float t12 = p0.x * rinv6;
-        uu = __fmaf_rn(rinv6, t12 - p0.y, __fmaf_rn(p0.w, r, -p1.x));
-        fr = __fmaf_rn(rinv6 * rinv2, __fmaf_rn(12.0f, t12, -6.0f * p0.y), -p0.w * rinv);
+    const float rinv2 = y * y;
+    const float rinv6 = rinv2 * rinv2 * rinv2;
+    const float r = r2 * y;
+    const bool in_lj = ok && r2 < pf.z;
+    // f_SF / r = (12 c12 r^-12 - 6 c6 r^-6) r^-2 - fc / r
+    float fr = __fmaf_rn(rinv6 * rinv2, __fmaf_rn(pf.x, rinv6, -pf.y), -pf.w * y);
+    fr = in_lj ? fr : 0.f;
+    float uu = 0.f;
+    if (ENERGY) { // u_SF = c12 r^-12 - c6 r^-6 + fc r - k0
+        uu = __fmaf_rn(rinv6, __fmaf_rn(pe.x, rinv6, -pe.y), __fmaf_rn(pf.w, r, -pe.z));
+        uu = in_lj ? uu : 0.f;
     }
-    if (COUL) { // p1 = (k0_lj, qq, rc2_c, fc_c), p2.x = k0_c
-        if (r2 < p1.z) {
-            uu += __fmaf_rn(p1.y, rinv, __fmaf_rn(p1.w, r, -p2.x));
-            fr += __fmaf_rn(p1.y * rinv, rinv2, -p1.w * rinv);
+    if (COUL) {
+        const bool in_c = ok && r2 < pc.y;
+        const float fc = __fmaf_rn(pc.x * y, rinv2, -pc.z * y); // qq r^-3 - fc / r
+        fr += in_c ? fc : 0.f;
+        if (ENERGY) {
+            const float uc = __fmaf_rn(pc.x, y, __fmaf_rn(pc.z, r, -pe.w)); // qq / r + fc r - k0
+            uu += in_c ? uc : 0.f;
         }
     }
     fx = __fmaf_rn(fr, dx, fx);
     fy = __fmaf_rn(fr, dy, fy);
     fz = __fmaf_rn(fr, dz, fz);
-    u += uu;
-    w = __fmaf_rn(fr, r2, w);
+    if (ENERGY) {
+        u += uu;
+        w = __fmaf_rn(fr, r2, w);
+    }
 }
 
 // ------------------------------------------------------------------------------------------ A5: forces
@@ -52,31 +58,31 @@ __device__ __forceinline__ void pair_accumulate(const float4 p0, const float4 p1
 // per lane are in flight at once (the paper's one-ahead index prefetch, P:108 item 4, generalised).
 //
 // force_group: the partial sums of one lane, then the butterfly over its TP-lane group; on return every lane
-// of the group holds the particle's totals (u and w NOT yet halved).  vwarp = index of this warp in the
-// virtual grid of N*TP threads.  NC = true: list and positions are read-only for the whole kernel, loads go
-// through ld.global.nc; NC = false (persistent kernel, which rewrites both): coherent loads, the index
-// stream marked evict-first.  All 32 lanes of the warp must call.
+// of the group holds the particle's totals (u and w NOT yet halved; only computed when ENERGY).  vwarp =
+// index of this warp in the virtual grid of N*TP threads.  NC = true: list and positions are read-only for
+// the whole kernel, loads go through ld.global.nc; NC = false (persistent kernel, which rewrites both):
+// coherent loads, the index stream marked evict-first.  All 32 lanes of the warp must call.
+//
+// Minimum image: a particle further than rc_max + 2 skin from every face of the box cannot have a listed
+// neighbour across a periodic boundary (the pair was within rc + skin at the build and neither particle has
+// moved more than skin/2 since, O9), so when this holds for ALL particles of the warp (WRAP = false) the
+// displacement is the plain difference; otherwise the exact shifted form of min_image is used.
 template <bool NC> __device__ __forceinline__ int load_idx(const int* p) { return NC ? __ldg(p) : __ldcs(p); }
 template <bool NC> __device__ __forceinline__ float4 load_pos(const float4* p) { return NC ? __ldg(p) : *p; }
 
-template <int TP, bool COUL, bool ONE_TYPE, int UNROLL, bool NC>
-__device__ __forceinline__ void force_group(const Sys& S, const float4* r, const float4* s_pp, int vwarp, int i,
-                                            int t, const float4 ri, int cnt, float& fx, float& fy, float& fz,
-                                            float& u, float& w)
+template <int TP, bool COUL, bool ONE_TYPE, int UNROLL, bool NC, bool ENERGY, bool WRAP>
+__device__ __forceinline__ void force_loop(const Sys& S, const float4* r, const float4* s_pp, const int* base, int i,
+                                           int nit, int nit_w, const float4 ri, float& fx, float& fy, float& fz,
+                                           float& u, float& w)
 {
-    const int lane = threadIdx.x & 31;
-    const int trow = ONE_TYPE ? 0 : 3 * type_of(ri) * S.ntypes;
-    float4 q0, q1, q2;
+    const int trow = ONE_TYPE ? 0 : 4 * type_of(ri) * S.ntypes;
+    float4 pf, pc, pe;
+    pc = pe = make_float4(0.f, 0.f, 0.f, 0.f);
     if (ONE_TYPE) {
-        q0 = s_pp[0];
-        q1 = s_pp[1];
-        q2 = s_pp[2];
+        pf = s_pp[0];
+        if (COUL) pc = s_pp[1];
+        if (ENERGY) pe = s_pp[2];
     }
-    int nit = (cnt - t + TP - 1) / TP; // entries t, t+TP, ... < cnt
-    if (nit < 0) nit = 0;
-    const int nit_w = __reduce_max_sync(FULLMASK, nit);
-    const int* base = S.nbl + (size_t)vwarp * S.cap_it * 32 + lane;
-    fx = fy = fz = u = w = 0.f;
     const float hx = S.h[0], hy = S.h[1], hz = S.h[2];
     const float ix = S.invL[0], iy = S.invL[1], iz = S.invL[2];
     for (int it = 0; it < nit_w; it += UNROLL) {
@@ -86,39 +92,66 @@ __device__ __forceinline__ void force_group(const Sys& S, const float4* r, const
 #pragma unroll
         for (int q = 0; q < UNROLL; ++q) {
             ok[q] = (it + q) < nit;
-            j[q] = ok[q] ? load_idx<NC>(base + (size_t)(it + q) * 32) : i;
+            j[q] = ok[q] ? load_idx<NC>(base + (size_t)(it + q) * 32) : 0; // masked lanes gather slot 0 (always valid)
         }
 #pragma unroll
-        for (int q = 0; q < UNROLL; ++q) rj[q] = ok[q] ? load_pos<NC>(&r[j[q]]) : ri;
+        for (int q = 0; q < UNROLL; ++q) rj[q] = load_pos<NC>(&r[j[q]]);
 #pragma unroll
         for (int q = 0; q < UNROLL; ++q) {
-            const float dx = min_image(ri.x, rj[q].x, hx, ix);
-            const float dy = min_image(ri.y, rj[q].y, hy, iy);
-            const float dz = min_image(ri.z, rj[q].z, hz, iz);
-            if (!ONE_TYPE) {
-                const int o = trow + 3 * type_of(rj[q]);
-                q0 = s_pp[o];
-                q1 = s_pp[o + 1];
-                q2 = s_pp[o + 2];
+            float dx, dy, dz;
+            if (WRAP) {
+                dx = min_image(ri.x, rj[q].x, hx, ix);
+                dy = min_image(ri.y, rj[q].y, hy, iy);
+                dz = min_image(ri.z, rj[q].z, hz, iz);
+            } else {
+                dx = ri.x - rj[q].x;
+                dy = ri.y - rj[q].y;
+                dz = ri.z - rj[q].z;
             }
-            pair_accumulate<COUL>(q0, q1, q2, ok[q], dx, dy, dz, fx, fy, fz, u, w);
+            if (!ONE_TYPE) {
+                const int o = trow + 4 * type_of(rj[q]);
+                pf = s_pp[o];
+                if (COUL) pc = s_pp[o + 1];
+                if (ENERGY) pe = s_pp[o + 2];
+            }
+            pair_accumulate<COUL, ENERGY>(pf, pc, pe, ok[q], dx, dy, dz, fx, fy, fz, u, w);
         }
     }
+}
+
+template <int TP, bool COUL, bool ONE_TYPE, int UNROLL, bool NC, bool ENERGY>
+__device__ __forceinline__ void force_group(const Sys& S, const float4* r, const float4* s_pp, int vwarp, int i,
+                                            int t, bool have_i, const float4 ri, int cnt, float& fx, float& fy,
+                                            float& fz, float& u, float& w)
+{
+    const int lane = threadIdx.x & 31;
+    int nit = (cnt - t + TP - 1) / TP; // entries t, t+TP, ... < cnt
+    if (nit < 0) nit = 0;
+    const int nit_w = __reduce_max_sync(FULLMASK, nit);
+    const int* base = S.nbl + (size_t)vwarp * S.cap_it * 32 + lane;
+    fx = fy = fz = u = w = 0.f;
+    const bool interior = fabsf(ri.x) < S.hin[0] && fabsf(ri.y) < S.hin[1] && fabsf(ri.z) < S.hin[2];
+    if (__any_sync(FULLMASK, have_i && !interior))
+        force_loop<TP, COUL, ONE_TYPE, UNROLL, NC, ENERGY, true>(S, r, s_pp, base, i, nit, nit_w, ri, fx, fy, fz, u, w);
+    else
+        force_loop<TP, COUL, ONE_TYPE, UNROLL, NC, ENERGY, false>(S, r, s_pp, base, i, nit, nit_w, ri, fx, fy, fz, u, w);
 #pragma unroll
     for (int o = TP / 2; o; o >>= 1) {
         fx += __shfl_xor_sync(FULLMASK, fx, o);
         fy += __shfl_xor_sync(FULLMASK, fy, o);
         fz += __shfl_xor_sync(FULLMASK, fz, o);
-        u += __shfl_xor_sync(FULLMASK, u, o);
-        w += __shfl_xor_sync(FULLMASK, w, o);
+        if (ENERGY) {
+            u += __shfl_xor_sync(FULLMASK, u, o);
+            w += __shfl_xor_sync(FULLMASK, w, o);
+        }
     }
 }
 
-// the pair table in shared memory: record of the ordered pair (a, b) at 3*(a*ntypes + b) (three float4)
+// the pair table in shared memory: record of the ordered pair (a, b) at 4*(a*ntypes + b) (four float4)
 __device__ __forceinline__ void load_pair_table(const Sys& S, float4* s_pp)
 {
     const float4* src = reinterpret_cast<const float4*>(S.pp);
-    for (int q = threadIdx.x; q < 3 * S.ntypes * S.ntypes; q += blockDim.x) s_pp[q] = src[q];
+    for (int q = threadIdx.x; q < 4 * S.ntypes * S.ntypes; q += blockDim.x) s_pp[q] = src[q];
 }
 
 // Bookkeeping that must happen once per step AFTER every rebuild kernel has read the flag: count the
@@ -135,7 +168,7 @@ __device__ __forceinline__ void finish_rebuild(const Sys& S)
 template <int TP, bool COUL, bool ONE_TYPE, int UNROLL>
 __global__ void __launch_bounds__(1024, 1) k_force(const Sys S)
 {
-    __shared__ float4 s_pp[3 * RUMD_MAXT * RUMD_MAXT];
+    __shared__ float4 s_pp[4 * RUMD_MAXT * RUMD_MAXT];
     load_pair_table(S, s_pp);
     __syncthreads();
     if (blockIdx.x == 0 && threadIdx.x == 0) finish_rebuild(S);
@@ -150,7 +183,7 @@ __global__ void __launch_bounds__(1024, 1) k_force(const Sys S)
         cnt = S.num_nbrs[i];
     }
     float fx, fy, fz, u, w;
-    force_group<TP, COUL, ONE_TYPE, UNROLL, true>(S, S.r, s_pp, tid >> 5, i, t, ri, cnt, fx, fy, fz, u, w);
+    force_group<TP, COUL, ONE_TYPE, UNROLL, true, true>(S, S.r, s_pp, tid >> 5, i, t, have_i, ri, cnt, fx, fy, fz, u, w);
     if (have_i && t == 0) {
         S.f[i] = make_float4(fx, fy, fz, 0.5f * u); // P:160 "compensate for double counting"
         S.w[i] = 0.5f * w;

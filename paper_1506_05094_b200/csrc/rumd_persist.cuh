@@ -13,96 +13,119 @@
 #pragma once
 #include "rumd_force.cuh"
 
-#define PERSIST_SPIN_LIMIT (1u << 27)
+#ifndef PERSIST_THREADS
+#define PERSIST_THREADS 256
+#endif
+#ifndef PERSIST_MINB
+#define PERSIST_MINB 2
+#endif
+#define PERSIST_SPIN_LIMIT (1u << 24)
 
-__device__ __forceinline__ unsigned ld_acquire_u32(const unsigned* p)
-{
-    unsigned v;
-    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-    return v;
-}
+// Grid barrier.  Two monotone 64-bit arrival counters (zeroed by the host before the launch) are used in
+// turn, so a block that is already arriving at the NEXT barrier never touches the counter a slow block is
+// still polling.  Low word: arrivals; high word: how many arriving blocks reported "some particle moved more
+// than skin/2" (O9) -- the displacement flag travels with the barrier and costs no extra round trip.
+// Thread 0 of each block arrives with a release reduction (publishes the block's writes, which it has
+// observed through the preceding __syncthreads) and polls with acquire loads (the compiler follows them by
+// CCTL.IVALL, dropping stale L1 lines of data other blocks rewrote); the closing __syncthreads hands the
+// ordering on to the rest of the block.  Returns false if the spin limit was hit (the kernel then winds
+// down instead of hanging).  `any_moved`: did the high word change since this counter was last used.
+struct BarrierState {
+    unsigned n = 0;            // barriers passed so far
+    unsigned seen_hi0 = 0, seen_hi1 = 0;
+};
 
-// Grid barrier over a monotone arrival counter (zeroed by the host before the launch).  Thread 0 of every
-// block publishes the block's writes (fence), arrives, spins with acquire loads until all nblocks blocks of
-// this epoch have arrived, and fences again (which also drops stale L1 lines of data other blocks rewrote).
-// Returns false if the spin limit was hit (a block is missing: the kernel then winds down instead of hanging).
-__device__ __forceinline__ bool grid_barrier(unsigned* counter, unsigned& epoch, unsigned nblocks, int* s_ok)
+__device__ __forceinline__ bool barrier_arrive_wait(unsigned long long* counters, BarrierState& bs, unsigned nblocks,
+                                                    bool moved, bool& any_moved)
 {
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        epoch += 1;
-        __threadfence();
-        atomicAdd(counter, 1u);
-        const unsigned target = epoch * nblocks;
-        unsigned spins = 0;
-        bool ok = true;
-        while (ld_acquire_u32(counter) < target) {
-            if (++spins > PERSIST_SPIN_LIMIT) {
-                ok = false;
-                break;
-            }
+    const unsigned p = bs.n & 1u;
+    const unsigned target = ((bs.n >> 1) + 1u) * nblocks;
+    bs.n += 1;
+    unsigned long long* c = counters + p;
+    const unsigned long long inc = 1ull | (moved ? (1ull << 32) : 0ull);
+    asm volatile("red.release.gpu.global.add.u64 [%0], %1;" ::"l"(c), "l"(inc) : "memory");
+    unsigned long long v;
+    unsigned spins = 0;
+    bool ok = true;
+    for (;;) {
+        asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(c) : "memory");
+        if ((unsigned)v >= target) break;
+        if (++spins > PERSIST_SPIN_LIMIT) {
+            ok = false;
+            break;
         }
-        __threadfence();
-        *s_ok = ok ? 1 : 0;
     }
-    __syncthreads();
-    return *s_ok != 0;
+    const unsigned hi = (unsigned)(v >> 32);
+    any_moved = hi != (p ? bs.seen_hi1 : bs.seen_hi0);
+    if (p) bs.seen_hi1 = hi; else bs.seen_hi0 = hi;
+    return ok;
 }
 
-// Fixed-order block sum of one double per thread; result valid in every thread.  s_red: 33 doubles.
-__device__ __forceinline__ double block_sum(double x, double* s_red)
-{
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
-    x = warp_sum(x);
-    __syncthreads();
-    if (lane == 0) s_red[wid] = x;
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        double a = 0.0;
-        for (int q = 0; q < nw; ++q) a += s_red[q];
-        s_red[32] = a;
-    }
-    __syncthreads();
-    return s_red[32];
-}
-
-#define PB(call)                                                                                         \
+// plain grid barrier between rebuild phases
+#define PB()                                                                                             \
     do {                                                                                                 \
-        if (!grid_barrier(&S.sc->barrier, epoch, gridDim.x, &s_ok)) {                                    \
-            if (threadIdx.x == 0) S.sc->nonfinite = 2;                                                   \
+        __syncthreads();                                                                                 \
+        if (threadIdx.x == 0) {                                                                          \
+            bool any_;                                                                                   \
+            s_ok = barrier_arrive_wait(sc->bar, bs, gridDim.x, false, any_) ? 1 : 0;                     \
+        }                                                                                                \
+        __syncthreads();                                                                                 \
+        if (!s_ok) {                                                                                     \
+            if (threadIdx.x == 0) sc->nonfinite = 2;                                                     \
             return;                                                                                      \
         }                                                                                                \
     } while (0)
 
-template <int TP, bool COUL, bool ONE_TYPE, int UNROLL>
-__global__ void __launch_bounds__(512, 1) k_persist(const Sys S, const int nsteps, const int nvt)
+// Fixed-order sum over the per-block partials of one step by ONE warp; every lane returns the total.
+__device__ __forceinline__ double warp_sum_partials(const double* p, int n)
 {
-    __shared__ float4 s_pp[3 * RUMD_MAXT * RUMD_MAXT];
+    double a = 0.0;
+    for (int q = threadIdx.x & 31; q < n; q += 32) a += __ldcg(&p[2 * q]);
+    return warp_sum(a);
+}
+
+template <int TP, bool COUL, bool ONE_TYPE, int UNROLL>
+__global__ void __launch_bounds__(PERSIST_THREADS, PERSIST_MINB) k_persist(const Sys S, const int nsteps, const int nvt)
+{
+    __shared__ float4 s_pp[4 * RUMD_MAXT * RUMD_MAXT];
     __shared__ float s_rcl2[RUMD_MAXT * RUMD_MAXT];
     __shared__ float4 s_tile[N2_TILE];
     __shared__ int s_warp[33];
-    __shared__ double s_red[33];
-    __shared__ int s_ok, s_moved;
+    __shared__ double s_redm[PERSIST_THREADS / 32], s_redk[PERSIST_THREADS / 32];
+    __shared__ int s_ok, s_moved, s_flag;
+    __shared__ float s_ab[2];
+    __shared__ int s_ab_step; // s_ab holds the leap-frog factors of every step < s_ab_step
 
     load_pair_table(S, s_pp);
     if (threadIdx.x < RUMD_MAXT * RUMD_MAXT) s_rcl2[threadIdx.x] = S.pp[threadIdx.x].rcl2;
-    unsigned epoch = 0;
     const int first = blockIdx.x * blockDim.x + threadIdx.x, stride = gridDim.x * blockDim.x;
-    const int lane = threadIdx.x & 31;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
     DevScalars* sc = S.sc;
+    BarrierState bs;
 
     // state every block carries identically (read before the first barrier, written back by block 0 at the end)
-    const long long step0 = sc->n_steps;
-    long long n_rebuilds = sc->n_rebuilds;
+    const long long n_rebuilds0 = sc->n_rebuilds;
+    long long n_rebuilds = n_rebuilds0;
     bool flag = sc->flag != 0u;
-    double xi = sc->xi, eta = sc->eta, xi_t = sc->xi_t, eta_t = sc->eta_t;
+    double xi = sc->xi, eta = sc->eta, xi_t = sc->xi_t, eta_t = sc->eta_t; // advanced by warp 0 of every block
     float4* rc = S.r;     // positions r(t) of the current step
     float4* rn = S.r_alt; // where r(t+dt) goes
     const int nchunks = (S.grid.ncell + SCAN_CHUNK - 1) / SCAN_CHUNK;
     const long long nvt_threads = (long long)S.N * TP;
+    if (threadIdx.x == 0) {
+        s_moved = 0;
+        s_ab[0] = 1.0f;
+        s_ab[1] = S.dt;
+        s_ab_step = nvt ? 0 : 0x7fffffff; // NVE: a = 1, b = dt for good
+    }
     __syncthreads();
+    // profiling (S.prof != nullptr): block 0 / thread 0 adds up SM cycles per phase
+    const bool prof = S.prof != nullptr && blockIdx.x == 0 && threadIdx.x == 0;
+    long long c_reb = 0, c_force = 0, c_bar = 0, t0 = 0, t1 = 0;
+    const long long c_begin = clock64();
 
     for (int k = 0; k < nsteps; ++k) {
+        if (prof) t0 = clock64();
         // ---------------------------------------------------------------- (rebuild if flag) A2 / A3 / A4
         if (flag) {
             int* max_slot = &sc->max_nbrs[n_rebuilds & 1];
@@ -136,17 +159,35 @@ __global__ void __launch_bounds__(512, 1) k_persist(const Sys S, const int nstep
             n_rebuilds += 1;
             PB();
         }
+        if (prof) {
+            t1 = clock64();
+            c_reb += t1 - t0;
+            t0 = t1;
+        }
+
+        // ---------------------------------------------------------------- Nose-Hoover factors of this step (O7)
+        // Warp 0 of EVERY block adds the previous step's per-block sums of m v^2 in the same fixed order and
+        // advances xi identically; the other warps start on the forces and pick the factors up from shared
+        // memory only when they integrate.
+        if (nvt && wid == 0) {
+            if (k > 0) {
+                const double sm = warp_sum_partials(S.partial + (size_t)((k - 1) & 1) * gridDim.x * 2 + 1, gridDim.x);
+                const double xin = xi + S.dt_d * S.omega2 * (sm / S.g / S.T0 - 1.0); // xi += dt w^2 (T_kin/T0 - 1)
+                xi_t = xi;
+                eta_t = eta;
+                eta += 0.5 * S.dt_d * (xi + xin);                                    // eta += dt/2 (xi_old + xi_new)
+                xi = xin;
+            }
+            if (lane == 0) {
+                const double hx = 0.5 * xi * S.dt_d;
+                ((volatile float*)s_ab)[0] = (float)((1.0 - hx) / (1.0 + hx));
+                ((volatile float*)s_ab)[1] = (float)(S.dt_d / (1.0 + hx));
+                __threadfence_block();
+                *((volatile int*)&s_ab_step) = k + 1;
+            }
+        }
 
         // ---------------------------------------------------------------- A5 + A6 fused: forces, leap-frog
-        float a, b;
-        if (nvt) {
-            const double hx = 0.5 * xi * S.dt_d;
-            a = (float)((1.0 - hx) / (1.0 + hx));
-            b = (float)(S.dt_d / (1.0 + hx));
-        } else {
-            a = 1.0f;
-            b = S.dt;
-        }
         const bool last = k == nsteps - 1;
         double kt = 0.0, mv2 = 0.0;
         bool moved = false;
@@ -161,8 +202,14 @@ __global__ void __launch_bounds__(512, 1) k_persist(const Sys S, const int nstep
                 cnt = S.num_nbrs[i];
             }
             float fx, fy, fz, u, w;
-            force_group<TP, COUL, ONE_TYPE, UNROLL, false>(S, rc, s_pp, (int)(vt >> 5), i, t, ri, cnt, fx, fy, fz, u, w);
+            if (last) // energies and virials are outputs of the LAST force evaluation only
+                force_group<TP, COUL, ONE_TYPE, UNROLL, false, true>(S, rc, s_pp, (int)(vt >> 5), i, t, have_i, ri, cnt, fx, fy, fz, u, w);
+            else
+                force_group<TP, COUL, ONE_TYPE, UNROLL, false, false>(S, rc, s_pp, (int)(vt >> 5), i, t, have_i, ri, cnt, fx, fy, fz, u, w);
             if (have_i && t == 0) {
+                while (*((volatile int*)&s_ab_step) <= k) {} // factors of step k published? (warp 0, above)
+                __threadfence_block();
+                const float a = ((volatile float*)s_ab)[0], b = ((volatile float*)s_ab)[1];
                 const float4 f = make_float4(fx, fy, fz, 0.5f * u);
                 float4 v = S.v[i];
                 int4 im = S.image[i];
@@ -181,63 +228,89 @@ __global__ void __launch_bounds__(512, 1) k_persist(const Sys S, const int nstep
                 mv2 += mv2i;
             }
         }
-        // per-block results: kinetic sums (needed every step for NVT, at the last step for the thermo read-out)
-        if (threadIdx.x == 0) s_moved = 0;
+        if (prof) {
+            t1 = clock64();
+            c_force += t1 - t0;
+            t0 = t1;
+        }
+
+        // ---------------------------------------------------------------- block sums, then the step's barrier
+        {
+            const double wm = (nvt || last) ? warp_sum(mv2) : 0.0;
+            const double wk = last ? warp_sum(kt) : 0.0;
+            const bool wmoved = __any_sync(FULLMASK, moved);
+            if (lane == 0) {
+                s_redm[wid] = wm;
+                s_redk[wid] = wk;
+                if (wmoved) s_moved = 1;
+            }
+        }
         __syncthreads();
-        if (moved) s_moved = 1;
-        if (nvt || last) {
-            const double bm = block_sum(mv2, s_red);
-            const double bk = last ? block_sum(kt, s_red) : 0.0;
-            if (threadIdx.x == 0) {
+        if (threadIdx.x == 0) {
+            if (nvt || last) {
+                double bk = 0.0, bm = 0.0;
+                for (int q = 0; q < nw; ++q) {
+                    bk += s_redk[q];
+                    bm += s_redm[q];
+                }
                 double* p = S.partial + ((size_t)(k & 1) * gridDim.x + blockIdx.x) * 2;
                 p[0] = bk;
                 p[1] = bm;
             }
+            const bool mvd = s_moved != 0;
+            s_moved = 0;
+            bool any;
+            s_ok = barrier_arrive_wait(sc->bar, bs, gridDim.x, mvd, any) ? 1 : 0;
+            s_flag = any ? 1 : 0; // O9 / P:270: rebuild before the next force evaluation
         }
         __syncthreads();
-        if (threadIdx.x == 0 && s_moved) atomicMax(&sc->moved_step, step0 + k + 1);
-        PB();
-
-        // ---------------------------------------------------------------- after the barrier: next step's inputs
-        flag = *((volatile long long*)&sc->moved_step) == step0 + k + 1; // O9 / P:270
-        if (nvt || last) {
-            const double* p = S.partial + (size_t)(k & 1) * gridDim.x * 2;
-            double sm = 0.0, sk = 0.0;
-            for (int q = threadIdx.x; q < (int)gridDim.x; q += blockDim.x) {
-                sk += __ldcg(&p[2 * q]);
-                sm += __ldcg(&p[2 * q + 1]);
-            }
-            sm = block_sum(sm, s_red);
-            if (last) sk = block_sum(sk, s_red);
-            if (nvt) { // O7: xi += dt w^2 (T_kin/T0 - 1), eta += dt/2 (xi_old + xi_new)
-                const double xin = xi + S.dt_d * S.omega2 * (sm / S.g / S.T0 - 1.0);
-                xi_t = xi;
-                eta_t = eta;
-                eta += 0.5 * S.dt_d * (xi + xin);
-                xi = xin;
-            }
-            if (last && blockIdx.x == 0 && threadIdx.x == 0) {
-                sc->K = sk;
-                sc->mv2 = sm;
-                if (!(sk == sk) || !(sm == sm)) sc->nonfinite = 1;
-            }
+        if (!s_ok) {
+            if (threadIdx.x == 0) sc->nonfinite = 2;
+            return;
         }
+        flag = s_flag != 0;
         float4* tmp = rc;
         rc = rn;
         rn = tmp;
+        if (prof) c_bar += clock64() - t0;
     }
 
     // ---------------------------------------------------------------- wind down
     if (rc != S.r) // odd number of steps: the current positions sit in the alternate buffer
         for (int i = first; i < S.N; i += stride) S.r[i] = rc[i];
-    if (blockIdx.x == 0 && threadIdx.x == 0) {
-        sc->xi = xi;
-        sc->eta = eta;
-        sc->xi_t = xi_t;
-        sc->eta_t = eta_t;
-        sc->n_steps = step0 + nsteps;
-        sc->n_rebuilds = n_rebuilds;
-        sc->flag = flag ? 1u : 0u;
-        sc->pending = 0u;
+    if (blockIdx.x == 0 && wid == 0 && nsteps > 0) {
+        const double* p = S.partial + (size_t)((nsteps - 1) & 1) * gridDim.x * 2;
+        const double sk = warp_sum_partials(p, gridDim.x);
+        const double sm = warp_sum_partials(p + 1, gridDim.x);
+        if (nvt) {
+            const double xin = xi + S.dt_d * S.omega2 * (sm / S.g / S.T0 - 1.0);
+            xi_t = xi;
+            eta_t = eta;
+            eta += 0.5 * S.dt_d * (xi + xin);
+            xi = xin;
+        }
+        if (lane == 0) {
+            sc->K = sk;
+            sc->mv2 = sm;
+            if (!(sk == sk) || !(sm == sm)) sc->nonfinite = 1;
+            sc->xi = xi;
+            sc->eta = eta;
+            sc->xi_t = xi_t;
+            sc->eta_t = eta_t;
+            sc->n_steps += nsteps;
+            sc->n_rebuilds = n_rebuilds;
+            sc->flag = flag ? 1u : 0u;
+            sc->pending = 0u;
+        }
+    }
+    if (prof) {
+        S.prof[0] = c_reb;
+        S.prof[1] = c_force;
+        S.prof[2] = 0;
+        S.prof[3] = c_bar;
+        S.prof[4] = 0;
+        S.prof[5] = clock64() - c_begin;
+        S.prof[6] = n_rebuilds - n_rebuilds0;
+        S.prof[7] = gridDim.x;
     }
 }

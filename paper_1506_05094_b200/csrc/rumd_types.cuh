@@ -12,9 +12,10 @@
 //   shifted force: u_SF = u(r) + fc*r - k0,  f_SF/r = f(r)/r - fc/r,  fc = f(rc), k0 = u(rc) + rc*fc
 //   Coulomb (O4):  u = qq/r, same shift with fc = qq/rc^2, k0 = 2 qq/rc
 struct __align__(16) PairParams {
-    float c12, c6, rc2_lj, fc_lj;   // float4 #0
-    float k0_lj, qq, rc2_c, fc_c;   // float4 #1
-    float k0_c, rcl2, rc2_max, pad; // float4 #2: rcl2 = (rc_ab + skin)^2 list cutoff (S4), rc2_max = max rc^2
+    float c12x12, c6x6, rc2_lj, fc_lj; // float4 #0: force, LJ term
+    float qq, rc2_c, fc_c, rc2_max;    // float4 #1: force, Coulomb term; rc2_max = max rc^2 of the pair's terms
+    float c12, c6, k0_lj, k0_c;        // float4 #2: energies
+    float rcl2, pad0, pad1, pad2;      // float4 #3: rcl2 = (rc_ab + skin)^2 list cutoff (S4)
 };
 
 // Device scalars living in the workspace.
@@ -25,14 +26,14 @@ struct DevScalars {
     double U, W;          // filled by the thermo reduction
     long long n_steps;
     long long n_rebuilds;
-    long long moved_step; // persistent path: 1 + index of the last step whose displacement check fired (O9)
+    unsigned long long bar[2]; // persistent kernel: the two arrival counters of its grid barrier
     unsigned int flag;    // rebuild requested for the NEXT force evaluation (P:179 updateRequired)
     unsigned int pending; // set by the integrator's displacement check during a step
     unsigned int ticket;  // last-block-done counter of the integrator
     unsigned int overflow;
     int max_nbrs[2];      // largest list length of build number b in slot b & 1
     int nonfinite;        // 1: NaN/Inf energy; 2: grid barrier timed out
-    unsigned int barrier; // arrival counter of the persistent kernel's grid barrier
+    int pad0;
 };
 
 struct CellGrid {
@@ -47,6 +48,7 @@ struct Sys {
     int cap, cap_it;        // list capacity per particle (multiple of 32), cap / tp
     int tp_shift, ppw_shift;// log2(tp), log2(32/tp)
     float L[3], h[3], invL[3];
+    float hin[3];           // h - (rc_max + 2 skin): inside this no listed neighbour is across a boundary
     float dt, half_skin2;   // (skin/2)^2
     double dt_d, T0, omega2, g;
     int sort_interval, method;
@@ -61,6 +63,7 @@ struct Sys {
     float4* tmp_r; float4* tmp_v; int4* tmp_image; int* tmp_id;
     int* cell_of; int* slot; int* perm;
     int* ccount; int* cstart_z; int2* cell_range; int* zrank; int* zinv; int* blocksum;
+    long long* prof;        // nullptr, or 8 cycle counters filled by block 0 of the persistent kernel (profiling run)
     double* partial;        // 2 sets x 2 doubles per block (kt, mv2) of the integrating kernel
     DevScalars* sc;
     PairParams pp[RUMD_MAXT * RUMD_MAXT];

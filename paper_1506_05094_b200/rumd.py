@@ -14,7 +14,7 @@ import numpy as np
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_LIBPATH = os.path.join(_HERE, "librumd_b200.so")
+_LIBPATH = os.environ.get("RUMD_B200_LIB") or os.path.join(_HERE, "librumd_b200.so")  # override: A/B builds
 
 OK, ERR_INVALID_ARG, ERR_NOT_READY, ERR_CUDA, ERR_NBL_OVERFLOW, ERR_BOX_TOO_SMALL, ERR_NONFINITE = range(7)
 POT_LJ_12_6, POT_COULOMB = 0, 1
@@ -27,7 +27,7 @@ EXPORTS = [
     "rumd_set_pair_potential", "rumd_set_integrator", "rumd_default_tuning", "rumd_set_tuning",
     "rumd_get_tuning", "rumd_autotune", "rumd_build_nblist", "rumd_compute_forces", "rumd_run_steps",
     "rumd_export_nblist", "rumd_get_thermo", "rumd_snapshot", "rumd_restore", "rumd_upload_state",
-    "rumd_download_state", "rumd_launch_count", "rumd_profile_step", "rumd_time_force", "rumd_last_error", "rumd_version",
+    "rumd_download_state", "rumd_launch_count", "rumd_profile_step", "rumd_time_force", "rumd_profile_persistent", "rumd_last_error", "rumd_version",
 ]
 
 
@@ -93,6 +93,7 @@ def lib():
         L.rumd_launch_count.restype = C.c_longlong
         L.rumd_profile_step.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(ip)]
         L.rumd_time_force.argtypes = [vp, ip, C.POINTER(C.c_float)]
+        L.rumd_profile_persistent.argtypes = [vp, ip, C.POINTER(C.c_double)]
         L.rumd_last_error.argtypes = [vp]
         L.rumd_last_error.restype = C.c_char_p
         L.rumd_version.restype = C.c_char_p
@@ -281,6 +282,15 @@ class System:
         us = C.c_float()
         self._check(self.L.rumd_time_force(self.h, int(reps), C.byref(us)))
         return float(us.value)
+
+    def profile_persistent(self, nsteps=1000) -> dict:
+        out = (C.c_double * 8)()
+        self._check(self.L.rumd_profile_persistent(self.h, int(nsteps), out))
+        keys = ("rebuild_us", "force_integrate_us", "block_reduce_us", "barrier_us", "post_us", "step_us")
+        d = {k: out[q] for q, k in enumerate(keys)}
+        d["rebuilds"] = int(out[6])
+        d["grid"] = int(out[7])
+        return d
 
     # ---- convenience read-back (numpy, ORIGINAL particle numbering via d_id)
     def state(self) -> dict:
