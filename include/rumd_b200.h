@@ -188,9 +188,9 @@ rumd_status rumd_profile_step(rumd_system* s, float* ms_out, int* did_rebuild_ou
 rumd_status rumd_time_force(rumd_system* s, int reps, float* us_per_launch);
 
 /* Runs nsteps time steps in the persistent kernel with the per-phase SM-cycle counters of block 0 switched
- * on.  out8: host, 8 doubles = microseconds PER STEP spent by block 0 in {rebuild phases, force + integrate,
- * block reductions, grid barrier wait, post-barrier reduction}, whole kernel per step, number of rebuilds,
- * grid size.  Advances the simulation by nsteps.  Synchronizes. */
+ * on.  out8: host, 8 doubles = microseconds PER STEP spent by block 0 in {rebuild phases (sort + build),
+ * force + integrate, the sort part of the rebuild, block sums + grid barrier wait, unused}, whole kernel per
+ * step, number of rebuilds, grid size.  Advances the simulation by nsteps.  Synchronizes. */
 rumd_status rumd_profile_persistent(rumd_system* s, int nsteps, double* out8);
 
 const char* rumd_last_error(const rumd_system* s);

@@ -118,13 +118,13 @@ static size_t max_cells(const rumd_system* s)
     return t;
 }
 
-static uint32_t part1by2(uint32_t x)
+static uint32_t part1by1(uint32_t x) // spread the low 16 bits to the even bit positions
 {
-    x &= 0x000003ff;
-    x = (x ^ (x << 16)) & 0xff0000ff;
-    x = (x ^ (x << 8)) & 0x0300f00f;
-    x = (x ^ (x << 4)) & 0x030c30c3;
-    x = (x ^ (x << 2)) & 0x09249249;
+    x &= 0x0000ffff;
+    x = (x ^ (x << 8)) & 0x00ff00ff;
+    x = (x ^ (x << 4)) & 0x0f0f0f0f;
+    x = (x ^ (x << 2)) & 0x33333333;
+    x = (x ^ (x << 1)) & 0x55555555;
     return x;
 }
 
@@ -159,10 +159,8 @@ static size_t carve(rumd_system* s, char* base, int cap)
     p = take(N * 4); if (base) S.slot = (int*)p;
     p = take(N * 4); if (base) S.perm = (int*)p;
     p = take(nc * 4); if (base) S.ccount = (int*)p;
-    p = take(nc * 4); if (base) S.cstart_z = (int*)p;
-    p = take(nc * 8); if (base) S.cell_range = (int2*)p;
-    p = take(nc * 4); if (base) S.zrank = (int*)p;
-    p = take(nc * 4); if (base) S.zinv = (int*)p;
+    p = take((nc + 1) * 4); if (base) S.cstart_z = (int*)p;
+    p = take(nc * 4); if (base) S.rowrank = (int*)p;
     p = take((nc / SCAN_CHUNK + 2) * 4); if (base) S.blocksum = (int*)p;
     // (kt, mv2) per block: integrator kernel (N/128 blocks) or persistent kernel (2 sets x <= 4096 blocks)
     const size_t nblk = std::max<size_t>((N + 31) / 32 + 1, 2 * 4096);
@@ -492,22 +490,19 @@ static rumd_status refresh(rumd_system* s)
     S.grid.ncell = (int)ncell;
     for (int k = 0; k < 3; ++k) S.grid.scale[k] = (float)((double)n[k] / (double)s->box[k]);
     if (n[0] != s->grid_for[0] || n[1] != s->grid_for[1] || n[2] != s->grid_for[2]) {
-        std::vector<std::pair<uint32_t, int>> keys(ncell);
+        // rank of every (y, z) cell column along a 2-D Morton curve (S19)
+        const size_t nrows = (size_t)n[1] * n[2];
+        std::vector<std::pair<uint32_t, int>> keys(nrows);
         for (int z = 0; z < n[2]; ++z)
-            for (int y = 0; y < n[1]; ++y)
-                for (int x = 0; x < n[0]; ++x) {
-                    const int c = (z * n[1] + y) * n[0] + x;
-                    keys[c] = {part1by2(x) | (part1by2(y) << 1) | (part1by2(z) << 2), c};
-                }
+            for (int y = 0; y < n[1]; ++y) {
+                const int c = z * n[1] + y;
+                keys[c] = {part1by1((uint32_t)y) | (part1by1((uint32_t)z) << 1), c};
+            }
         std::sort(keys.begin(), keys.end());
-        std::vector<int> zr(ncell), zi(ncell);
-        for (size_t q = 0; q < ncell; ++q) {
-            zr[keys[q].second] = (int)q;
-            zi[q] = keys[q].second;
-        }
+        std::vector<int> rr(nrows);
+        for (size_t q = 0; q < nrows; ++q) rr[keys[q].second] = (int)q;
         CUDA_TRY(s, cudaStreamSynchronize(s->stream));
-        CUDA_TRY(s, cudaMemcpyAsync(S.zrank, zr.data(), ncell * 4, cudaMemcpyHostToDevice, s->stream));
-        CUDA_TRY(s, cudaMemcpyAsync(S.zinv, zi.data(), ncell * 4, cudaMemcpyHostToDevice, s->stream));
+        CUDA_TRY(s, cudaMemcpyAsync(S.rowrank, rr.data(), nrows * 4, cudaMemcpyHostToDevice, s->stream));
         CUDA_TRY(s, cudaStreamSynchronize(s->stream));
         s->grid_for[0] = n[0];
         s->grid_for[1] = n[1];

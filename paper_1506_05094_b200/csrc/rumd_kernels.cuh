@@ -135,15 +135,18 @@ __device__ __forceinline__ void ph_build_n2(const Sys& S, const float4* r, float
 // calls Thrust; here it is a counting sort written out: (a) histogram with slot = atomicAdd, (b) exclusive
 // scan, (c) scatter, (d) per-cell insertion sort of the (few) entries by old index, which removes the
 // atomic's arbitrary order so that the particle order -- and with it every later fp32 sum -- is
-// reproducible.  Cells are numbered along a Morton (Z-order) curve through the valid cells (zrank table,
-// built once on the host): consecutive particles are spatially compact (BASELINE configs[3], S19).
+// reproducible.  Sort key of cell (x, y, z) = rowrank[z][y] * nx + x, where rowrank numbers the (y, z) cell
+// columns along a 2-D Morton (Z-order) curve (table built once on the host): consecutive particles are
+// spatially compact (BASELINE configs[3], S19) AND the cells of one x-row are contiguous in the sorted
+// order, so the 5 x-neighbour cells of a stencil row are ONE particle range (cellStart of the first cell to
+// cellStart of the cell after the last) -- the build then walks 25 ranges instead of 125 cells.
 
 __device__ __forceinline__ void ph_cell_assign(const Sys& S, const float4* r, int first, int stride)
 {
     for (int i = first; i < S.N; i += stride) {
         int cx, cy, cz;
         cell_coords(S, r[i], cx, cy, cz);
-        const int z = S.zrank[(cz * S.grid.n[1] + cy) * S.grid.n[0] + cx];
+        const int z = S.rowrank[cz * S.grid.n[1] + cy] * S.grid.n[0] + cx;
         S.cell_of[i] = z;
         S.slot[i] = atomicAdd(&S.ccount[z], 1);
     }
@@ -216,6 +219,7 @@ __device__ __forceinline__ void ph_scan_blocks(const Sys& S, int* s_warp)
         if (on) S.blocksum[b] = carry + e;
         carry += total;
     }
+    if (threadIdx.x == 0) S.cstart_z[S.grid.ncell] = S.N;
 }
 
 // phase 3: exclusive scan inside each chunk + chunk offset -> first sorted slot of each Z-ordered cell
@@ -268,6 +272,7 @@ __device__ __forceinline__ void ph_scan_single_block(const Sys& S, int* s_warp)
         }
         carry += total;
     }
+    if (threadIdx.x == 0) S.cstart_z[S.grid.ncell] = S.N;
 }
 
 __device__ __forceinline__ void ph_cell_scatter(const Sys& S, int first, int stride)
@@ -275,9 +280,9 @@ __device__ __forceinline__ void ph_cell_scatter(const Sys& S, int first, int str
     for (int i = first; i < S.N; i += stride) S.perm[S.cstart_z[S.cell_of[i]] + S.slot[i]] = i;
 }
 
-// One thread per cell: order its entries by old index (deterministic), publish cellStart / cellEnd under
-// the row-major cell index the build kernel uses (here end is EXCLUSIVE, S20), clear the
-// histogram for the next sort.
+// One thread per cell: order its entries by old index (deterministic) and clear the histogram for the next
+// sort.  cellStart is the scan output cstart_z[key]; cellEnd of a cell = cellStart of the next key
+// (EXCLUSIVE, S20; cstart_z[ncell] = N).
 __device__ __forceinline__ void ph_cell_finish(const Sys& S, int first, int stride)
 {
     for (int z = first; z < S.grid.ncell; z += stride) {
@@ -291,8 +296,6 @@ __device__ __forceinline__ void ph_cell_finish(const Sys& S, int first, int stri
             }
             S.perm[b + q + 1] = key;
         }
-        const int c = S.zinv[z];
-        S.cell_range[c] = make_int2(b, b + n);
         S.ccount[z] = 0;
     }
 }
@@ -326,9 +329,10 @@ __device__ __forceinline__ void ph_permute_store(const Sys& S, float4* r, int fi
 // coordinate (needs n >= 5 per axis, S18), strict per-type-pair test, overflow flag
 // (P:256), positions at build.  The paper uses one thread per particle and notes that several
 // threads per particle had "not been tried yet"; here G = 1..32 lanes share one particle: lane l
-// takes stencil cells l, l+G, ..., the group walks its cells in lock step and hands out list slots by
-// ballot + popc, so rows come out in the fixed order (round, position in cell, lane) and the list is
-// bitwise reproducible.  `first`/`stride` index the virtual grid of N*G threads (multiples of 32).
+// takes stencil rows l, l+G, ... of the 25 (dy, dz) rows; a row's 5 x-cells are one contiguous particle range
+// (two when the row wraps around the box in x).  The group walks its ranges in lock step and hands out list
+// slots by ballot + popc, so rows of the list come out in the fixed order (round, position in range, lane)
+// and the list is bitwise reproducible.  `first`/`stride` index the virtual grid of N*G threads.
 template <int G>
 __device__ __forceinline__ void ph_build_cell(const Sys& S, const float4* r, const float* s_rcl2, int first,
                                               int stride, int* max_slot)
@@ -347,35 +351,71 @@ __device__ __forceinline__ void ph_build_cell(const Sys& S, const float4* r, con
         const int trow = have_i ? type_of(ri) * S.ntypes : 0;
         int cx = 0, cy = 0, cz = 0;
         if (have_i) cell_coords(S, ri, cx, cy, cz);
+        // x extent of the stencil: main segment [x0, x1], wrapped segment [w0, w1] (empty if w0 > w1)
+        const int x0 = max(cx - 2, 0), x1 = min(cx + 2, nx - 1);
+        int w0 = 1, w1 = 0;
+        if (cx - 2 < 0) {
+            w0 = nx + cx - 2;
+            w1 = nx - 1;
+        } else if (cx + 2 >= nx) {
+            w0 = 0;
+            w1 = cx + 2 - nx;
+        }
         int count = 0;
-        auto range_of = [&](int q) -> int2 {
-            if (!have_i || q >= 125) return make_int2(0, 0);
-            int dz = q / 25, dy = (q / 5) % 5, dx = q % 5;
-            int z = cz + dz - 2, y = cy + dy - 2, x = cx + dx - 2;
-            z += z < 0 ? nz : 0; z -= z >= nz ? nz : 0;
-            y += y < 0 ? ny : 0; y -= y >= ny ? ny : 0;
-            x += x < 0 ? nx : 0; x -= x >= nx ? nx : 0;
-            return S.cell_range[(z * ny + y) * nx + x];
+        // particle ranges of stencil row q (0..24): main [a.x, a.y) and wrapped [b.x, b.y)
+        auto ranges_of = [&](int q, int2& a, int2& b) {
+            a = b = make_int2(0, 0);
+            if (!have_i || q >= 25) return;
+            int z = cz + q / 5 - 2, y = cy + q % 5 - 2;
+            z += z < 0 ? nz : 0;
+            z -= z >= nz ? nz : 0;
+            y += y < 0 ? ny : 0;
+            y -= y >= ny ? ny : 0;
+            const int* cs = S.cstart_z + S.rowrank[z * ny + y] * nx;
+            a = make_int2(cs[x0], cs[x1 + 1]);
+            if (w0 <= w1) b = make_int2(cs[w0], cs[w1 + 1]);
         };
-        int2 nxt = range_of(l);
-        for (int q0 = 0; q0 < 125; q0 += G) {
-            const int2 cur = nxt;
-            if (q0 + G < 125) nxt = range_of(q0 + G + l); // one-ahead prefetch of the next round's cell
-            const int n = cur.y - cur.x;
+        // A particle further than the list cutoff from every face has no listed neighbour across a periodic
+        // boundary, and a wrapped candidate's plain difference is ~L, which fails the test anyway: when this
+        // holds for the whole warp the plain difference replaces the minimum image (hin is a little stricter).
+        const bool interior = fabsf(ri.x) < S.hin[0] && fabsf(ri.y) < S.hin[1] && fabsf(ri.z) < S.hin[2];
+        const bool wrap = __any_sync(FULLMASK, have_i && !interior);
+        int2 na, nb;
+        ranges_of(l, na, nb);
+        for (int q0 = 0; q0 < 25; q0 += G) {
+            const int2 a = na, b = nb;
+            if (q0 + G < 25) ranges_of(q0 + G + l, na, nb); // one-ahead prefetch of the next round's ranges
+            const int n0 = a.y - a.x, n = n0 + (b.y - b.x);
             const int nmax = __reduce_max_sync(FULLMASK, n);
-            for (int it = 0; it < nmax; ++it) {
-                bool acc = false;
-                const int j = cur.x + it;
-                if (it < n && j != i) {
-                    const float4 rj = r[j];
-                    acc = list_dist2(S, ri, rj) < s_rcl2[trow + type_of(rj)];
+            constexpr int U = 4; // candidates in flight per lane
+            for (int it0 = 0; it0 < nmax; it0 += U) {
+                float4 rj[U];
+                int j[U];
+#pragma unroll
+                for (int q = 0; q < U; ++q) {
+                    const int it = it0 + q;
+                    j[q] = it < n0 ? a.x + it : b.x + (it - n0);
+                    if (it >= n) j[q] = i; // masked: gather the particle itself (always valid when n > 0)
+                    if (!have_i) j[q] = 0;
+                    rj[q] = r[j[q]];
                 }
-                const unsigned m = __ballot_sync(FULLMASK, acc);
-                if (acc) {
-                    const int k = count + __popc(m & lt);
-                    if (k < S.cap) S.nbl[nbl_index(S, i, k)] = j;
+#pragma unroll
+                for (int q = 0; q < U; ++q) {
+                    float d2;
+                    if (wrap)
+                        d2 = list_dist2(S, ri, rj[q]);
+                    else {
+                        const float dx = ri.x - rj[q].x, dy = ri.y - rj[q].y, dz = ri.z - rj[q].z;
+                        d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, dx * dx));
+                    }
+                    const bool acc = have_i && j[q] != i && d2 < s_rcl2[trow + type_of(rj[q])];
+                    const unsigned m = __ballot_sync(FULLMASK, acc);
+                    if (acc) {
+                        const int k = count + __popc(m & lt);
+                        if (k < S.cap) S.nbl[nbl_index(S, i, k)] = j[q];
+                    }
+                    count += __popc(m & gmask);
                 }
-                count += __popc(m & gmask);
             }
         }
         if (have_i && l == 0) {

@@ -17,7 +17,7 @@
 #define PERSIST_THREADS 256
 #endif
 #ifndef PERSIST_MINB
-#define PERSIST_MINB 2
+#define PERSIST_MINB 3
 #endif
 #define PERSIST_SPIN_LIMIT (1u << 24)
 
@@ -95,6 +95,8 @@ __global__ void __launch_bounds__(PERSIST_THREADS, PERSIST_MINB) k_persist(const
     __shared__ int s_ok, s_moved, s_flag;
     __shared__ float s_ab[2];
     __shared__ int s_ab_step; // s_ab holds the leap-frog factors of every step < s_ab_step
+    __shared__ double s_nh[4];       // xi, eta, xi_t, eta_t: kept by lane 0 of warp 0 (identical in every block)
+    __shared__ long long s_prof[6];  // cycle counters of block 0 / thread 0 (profiling runs only)
 
     load_pair_table(S, s_pp);
     if (threadIdx.x < RUMD_MAXT * RUMD_MAXT) s_rcl2[threadIdx.x] = S.pp[threadIdx.x].rcl2;
@@ -104,10 +106,9 @@ __global__ void __launch_bounds__(PERSIST_THREADS, PERSIST_MINB) k_persist(const
     BarrierState bs;
 
     // state every block carries identically (read before the first barrier, written back by block 0 at the end)
-    const long long n_rebuilds0 = sc->n_rebuilds;
-    long long n_rebuilds = n_rebuilds0;
+    const int n_rebuilds0 = (int)(sc->n_rebuilds & 0x3fffffff); // only its parity and value mod sort_interval matter
+    int n_rebuilds = n_rebuilds0;
     bool flag = sc->flag != 0u;
-    double xi = sc->xi, eta = sc->eta, xi_t = sc->xi_t, eta_t = sc->eta_t; // advanced by warp 0 of every block
     float4* rc = S.r;     // positions r(t) of the current step
     float4* rn = S.r_alt; // where r(t+dt) goes
     const int nchunks = (S.grid.ncell + SCAN_CHUNK - 1) / SCAN_CHUNK;
@@ -117,15 +118,25 @@ __global__ void __launch_bounds__(PERSIST_THREADS, PERSIST_MINB) k_persist(const
         s_ab[0] = 1.0f;
         s_ab[1] = S.dt;
         s_ab_step = nvt ? 0 : 0x7fffffff; // NVE: a = 1, b = dt for good
+        s_nh[0] = sc->xi;
+        s_nh[1] = sc->eta;
+        s_nh[2] = sc->xi_t;
+        s_nh[3] = sc->eta_t;
+        for (int q = 0; q < 6; ++q) s_prof[q] = 0;
     }
     __syncthreads();
     // profiling (S.prof != nullptr): block 0 / thread 0 adds up SM cycles per phase
     const bool prof = S.prof != nullptr && blockIdx.x == 0 && threadIdx.x == 0;
-    long long c_reb = 0, c_force = 0, c_bar = 0, t0 = 0, t1 = 0;
-    const long long c_begin = clock64();
+    if (prof) s_prof[5] = clock64();
+#define PROF_LAP(slot)                                                                                   \
+    if (prof) {                                                                                          \
+        const long long t_ = clock64();                                                                  \
+        s_prof[slot] += t_ - s_prof[4];                                                                  \
+        s_prof[4] = t_;                                                                                  \
+    }
 
     for (int k = 0; k < nsteps; ++k) {
-        if (prof) t0 = clock64();
+        if (prof) s_prof[4] = clock64();
         // ---------------------------------------------------------------- (rebuild if flag) A2 / A3 / A4
         if (flag) {
             int* max_slot = &sc->max_nbrs[n_rebuilds & 1];
@@ -152,6 +163,7 @@ __global__ void __launch_bounds__(PERSIST_THREADS, PERSIST_MINB) k_persist(const
                 ph_permute_store(S, rc, first, stride);
                 PB();
             }
+            if (prof) s_prof[2] += clock64() - s_prof[4];
             if (S.method == 1)
                 build_cell_dispatch(S, rc, s_rcl2, first, stride, max_slot);
             else
@@ -159,26 +171,24 @@ __global__ void __launch_bounds__(PERSIST_THREADS, PERSIST_MINB) k_persist(const
             n_rebuilds += 1;
             PB();
         }
-        if (prof) {
-            t1 = clock64();
-            c_reb += t1 - t0;
-            t0 = t1;
-        }
+        PROF_LAP(0)
 
         // ---------------------------------------------------------------- Nose-Hoover factors of this step (O7)
         // Warp 0 of EVERY block adds the previous step's per-block sums of m v^2 in the same fixed order and
         // advances xi identically; the other warps start on the forces and pick the factors up from shared
         // memory only when they integrate.
         if (nvt && wid == 0) {
-            if (k > 0) {
-                const double sm = warp_sum_partials(S.partial + (size_t)((k - 1) & 1) * gridDim.x * 2 + 1, gridDim.x);
-                const double xin = xi + S.dt_d * S.omega2 * (sm / S.g / S.T0 - 1.0); // xi += dt w^2 (T_kin/T0 - 1)
-                xi_t = xi;
-                eta_t = eta;
-                eta += 0.5 * S.dt_d * (xi + xin);                                    // eta += dt/2 (xi_old + xi_new)
-                xi = xin;
-            }
+            double sm = 0.0;
+            if (k > 0) sm = warp_sum_partials(S.partial + (size_t)((k - 1) & 1) * gridDim.x * 2 + 1, gridDim.x);
             if (lane == 0) {
+                double xi = s_nh[0];
+                if (k > 0) {
+                    const double xin = xi + S.dt_d * S.omega2 * (sm / S.g / S.T0 - 1.0); // xi += dt w^2 (T_kin/T0 - 1)
+                    s_nh[2] = xi;
+                    s_nh[3] = s_nh[1];
+                    s_nh[1] += 0.5 * S.dt_d * (xi + xin);                               // eta += dt/2 (xi_old + xi_new)
+                    s_nh[0] = xi = xin;
+                }
                 const double hx = 0.5 * xi * S.dt_d;
                 ((volatile float*)s_ab)[0] = (float)((1.0 - hx) / (1.0 + hx));
                 ((volatile float*)s_ab)[1] = (float)(S.dt_d / (1.0 + hx));
@@ -228,11 +238,7 @@ __global__ void __launch_bounds__(PERSIST_THREADS, PERSIST_MINB) k_persist(const
                 mv2 += mv2i;
             }
         }
-        if (prof) {
-            t1 = clock64();
-            c_force += t1 - t0;
-            t0 = t1;
-        }
+        PROF_LAP(1)
 
         // ---------------------------------------------------------------- block sums, then the step's barrier
         {
@@ -272,7 +278,7 @@ __global__ void __launch_bounds__(PERSIST_THREADS, PERSIST_MINB) k_persist(const
         float4* tmp = rc;
         rc = rn;
         rn = tmp;
-        if (prof) c_bar += clock64() - t0;
+        PROF_LAP(3)
     }
 
     // ---------------------------------------------------------------- wind down
@@ -282,35 +288,37 @@ __global__ void __launch_bounds__(PERSIST_THREADS, PERSIST_MINB) k_persist(const
         const double* p = S.partial + (size_t)((nsteps - 1) & 1) * gridDim.x * 2;
         const double sk = warp_sum_partials(p, gridDim.x);
         const double sm = warp_sum_partials(p + 1, gridDim.x);
-        if (nvt) {
-            const double xin = xi + S.dt_d * S.omega2 * (sm / S.g / S.T0 - 1.0);
-            xi_t = xi;
-            eta_t = eta;
-            eta += 0.5 * S.dt_d * (xi + xin);
-            xi = xin;
-        }
         if (lane == 0) {
+            if (nvt) {
+                const double xi = s_nh[0];
+                const double xin = xi + S.dt_d * S.omega2 * (sm / S.g / S.T0 - 1.0);
+                s_nh[2] = xi;
+                s_nh[3] = s_nh[1];
+                s_nh[1] += 0.5 * S.dt_d * (xi + xin);
+                s_nh[0] = xin;
+            }
             sc->K = sk;
             sc->mv2 = sm;
             if (!(sk == sk) || !(sm == sm)) sc->nonfinite = 1;
-            sc->xi = xi;
-            sc->eta = eta;
-            sc->xi_t = xi_t;
-            sc->eta_t = eta_t;
+            sc->xi = s_nh[0];
+            sc->eta = s_nh[1];
+            sc->xi_t = s_nh[2];
+            sc->eta_t = s_nh[3];
             sc->n_steps += nsteps;
-            sc->n_rebuilds = n_rebuilds;
+            sc->n_rebuilds += n_rebuilds - n_rebuilds0;
             sc->flag = flag ? 1u : 0u;
             sc->pending = 0u;
         }
     }
     if (prof) {
-        S.prof[0] = c_reb;
-        S.prof[1] = c_force;
-        S.prof[2] = 0;
-        S.prof[3] = c_bar;
+        S.prof[0] = s_prof[0];
+        S.prof[1] = s_prof[1];
+        S.prof[2] = s_prof[2];
+        S.prof[3] = s_prof[3];
         S.prof[4] = 0;
-        S.prof[5] = clock64() - c_begin;
+        S.prof[5] = clock64() - s_prof[5];
         S.prof[6] = n_rebuilds - n_rebuilds0;
         S.prof[7] = gridDim.x;
     }
+#undef PROF_LAP
 }

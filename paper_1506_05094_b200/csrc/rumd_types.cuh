@@ -62,7 +62,7 @@ struct Sys {
     int* nbl; int* num_nbrs; float4* r_build;
     float4* tmp_r; float4* tmp_v; int4* tmp_image; int* tmp_id;
     int* cell_of; int* slot; int* perm;
-    int* ccount; int* cstart_z; int2* cell_range; int* zrank; int* zinv; int* blocksum;
+    int* ccount; int* cstart_z; int* rowrank; int* blocksum; // cstart_z: ncell + 1 entries; rowrank: ny*nz
     long long* prof;        // nullptr, or 8 cycle counters filled by block 0 of the persistent kernel (profiling run)
     double* partial;        // 2 sets x 2 doubles per block (kt, mv2) of the integrating kernel
     DevScalars* sc;

@@ -286,7 +286,7 @@ class System:
     def profile_persistent(self, nsteps=1000) -> dict:
         out = (C.c_double * 8)()
         self._check(self.L.rumd_profile_persistent(self.h, int(nsteps), out))
-        keys = ("rebuild_us", "force_integrate_us", "block_reduce_us", "barrier_us", "post_us", "step_us")
+        keys = ("rebuild_us", "force_integrate_us", "sort_us", "barrier_us", "post_us", "step_us")
         d = {k: out[q] for q, k in enumerate(keys)}
         d["rebuilds"] = int(out[6])
         d["grid"] = int(out[7])
