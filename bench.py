@@ -241,14 +241,27 @@ def run_gpu(args, rank, world, local_rank):
         ach_tf = flop / (us * 1e-6) / 1e12
         alg_bytes = 4.0 * listed + (16 + 4 + 20) * N
         prof = s.profile_step()
-        roof = {"kernel": "k_force", "bound": "alu", "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s",
-                "frac": ach_tf / peak_tf, "traffic": None,
-                "peak_source": "derived: 148 SMs x 128 FP32 lanes x 2 x %.0f MHz (max SM clock, %s)" % (
-                    peaks["sm_max_mhz"], peaks["source"]),
-                "frac_at_observed_clock": ach_tf / fp32_peak_tflops(sm_mhz),
-                "us_per_launch": us, "listed_pairs": listed, "flop_per_listed_pair": flop / listed,
-                "hbm_equiv_gbs": alg_bytes / (us * 1e-6) / 1e9, "hbm_peak_gbs": peaks["hbm_gbs"],
-                "force_share_of_step": us * 1e-3 / (ms / tsteps), "unfused_step_ms": prof}
+        flop_pp = flop / listed
+        force_kernel = {"kernel": "k_force (stand-alone, current tuning)", "us_per_launch": us, "achieved": ach_tf,
+                        "frac": ach_tf / peak_tf, "hbm_equiv_gbs": alg_bytes / (us * 1e-6) / 1e9,
+                        "hbm_peak_gbs": peaks["hbm_gbs"], "unfused_step_ms": prof}
+        if tun["persistent"]:
+            # the dominant kernel IS the whole run: one k_persist launch = `inner` time steps; its duration is the
+            # CUDA-event time of the timed region itself
+            us_launch = 1e3 * ms / args.steps
+            ach = flop * inner / (us_launch * 1e-6) / 1e12
+            phases = s.profile_persistent(inner)
+            roof = {"kernel": "k_persist (one launch = %d time steps: rebuilds + forces + integration)" % inner,
+                    "bound": "alu", "achieved": ach, "peak": peak_tf, "unit": "TFLOP/s", "frac": ach / peak_tf,
+                    "traffic": None, "us_per_launch": us_launch, "phases_us_per_timestep": phases}
+        else:
+            roof = {"kernel": "k_force", "bound": "alu", "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s",
+                    "frac": ach_tf / peak_tf, "traffic": None, "us_per_launch": us,
+                    "force_share_of_step": us * 1e-3 / (ms / tsteps)}
+        roof.update({"peak_source": "derived: 148 SMs x 128 FP32 lanes x 2 x %.0f MHz (max SM clock, %s)" % (
+                         peaks["sm_max_mhz"], peaks["source"]),
+                     "frac_at_observed_clock": roof["achieved"] / fp32_peak_tflops(sm_mhz),
+                     "listed_pairs": listed, "flop_per_listed_pair": flop_pp, "force_kernel": force_kernel})
         out = {
             "metric": "timesteps/s", "value": tps, "unit": "timesteps/s", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
@@ -267,6 +280,64 @@ def run_gpu(args, rank, world, local_rank):
             "thermo": {k: th1[k] for k in ("U", "K", "H", "xi")},
         }
     s.close()
+    return out
+
+
+# ------------------------------------------------------------------------------------------------ N sweep
+
+SWEEP = ["lj864", "ka512", "ka1000", "ka2048", "ka4096", "ka8000", "ka8192", "ka16384", "ka32768", "ka65536",
+         "ka131072", "charged", "lj1m"]
+
+
+def run_sweep(args, names):
+    """BASELINE.json metric "timesteps/s and particle-steps/s vs N": device-resident arm only, one entry per
+    workload, each autotuned (configs[2]) after equilibration.  Not part of the default run."""
+    import torch
+
+    from paper_1506_05094_b200 import rumd
+
+    peaks = measured_peaks()
+    peak_tf = fp32_peak_tflops(peaks["sm_max_mhz"])
+    out = []
+    for name in names:
+        wl, desc = make_workload(name)
+        s = rumd.from_workload(wl)
+        N = wl.N
+        equilibrate(s, wl, args.equil if N < 500000 else 500)
+        info = {}
+        if args.autotune:
+            t, tps_trial = s.autotune(steps_per_trial=args.tune_steps if N < 500000 else 60)
+            info["trial_tps"] = tps_trial
+        inner = max(50, min(args.inner, int(2e8 / N)))
+        for _ in range(3):
+            s.run_steps(inner)
+        th0 = s.get_thermo()
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(5)]
+        with torch.cuda.stream(s.stream):
+            for a, b in ev:
+                a.record(s.stream)
+                s.run_steps(inner)
+                b.record(s.stream)
+        torch.cuda.synchronize()
+        ms = sum(a.elapsed_time(b) for a, b in ev)
+        th1 = s.get_thermo()
+        tps = 5 * inner / (ms * 1e-3)
+        s.compute_forces()
+        cnt, _ = s.export_nblist()
+        listed = int(cnt.sum())
+        us = s.time_force(reps=50)
+        coul = bool((wl.pot[..., 4] > 0).any())
+        flop = (FLOP_PER_LISTED_PAIR_COUL if coul else FLOP_PER_LISTED_PAIR_LJ) * listed
+        tun = s.get_tuning().as_dict()
+        phases = s.profile_persistent(inner) if tun["persistent"] else None
+        out.append({"workload": name, "N": N, "timesteps_per_s": tps, "particle_steps_per_s": tps * N,
+                    "us_per_timestep": 1e3 * ms / (5 * inner), "tuning": tun, **info,
+                    "rebuild_interval": 5 * inner / max(1, th1["n_rebuilds"] - th0["n_rebuilds"]),
+                    "mean_nbrs": listed / N, "whole_step_frac_fp32": flop / (1e-3 * ms / (5 * inner)) / 1e12 / peak_tf,
+                    "force_kernel_us": us, "force_kernel_frac_fp32": flop / (us * 1e-6) / 1e12 / peak_tf,
+                    "phases_us_per_timestep": phases})
+        print("sweep %s: %.0f timesteps/s" % (name, tps), file=sys.stderr, flush=True)
+        s.close()
     return out
 
 
@@ -339,6 +410,8 @@ def main():
     ap.add_argument("--no-autotune", dest="autotune", action="store_false")
     ap.add_argument("--tune-steps", type=int, default=300)
     ap.add_argument("--no-cpu-baseline", dest="cpu", action="store_false")
+    ap.add_argument("--sweep", nargs="*", default=None, metavar="WORKLOAD",
+                    help="also time the N sweep (all of configs[0..4] when no names are given) -> key 'sweep'")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
 
@@ -367,6 +440,8 @@ def main():
             out["cpu_baseline"] = cpu_baseline(wl)
         else:
             out["cpu_baseline"] = None
+        if args.sweep is not None and world == 1:
+            out["sweep"] = run_sweep(args, args.sweep or SWEEP)
         print(json.dumps(out), flush=True)
     if world > 1:
         torch.distributed.barrier()

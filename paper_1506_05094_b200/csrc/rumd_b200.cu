@@ -363,8 +363,8 @@ extern "C" rumd_status rumd_default_tuning(const rumd_system* s, rumd_tuning* t)
     if (!s || !t) return RUMD_ERR_INVALID_ARG;
     const int N = s->N;
     t->method = N <= 6000 ? RUMD_NB_N2 : RUMD_NB_CELL;
-    t->tp = N <= 2048 ? 32 : N <= 8192 ? 16 : N <= 32768 ? 8 : N <= 131072 ? 4 : 2;
-    t->pb = std::max(32 / t->tp, 128 / t->tp);
+    t->tp = N <= 2048 ? 32 : N <= 16384 ? 8 : N <= 32768 ? 4 : N <= 131072 ? 2 : 1;
+    t->pb = 256 / t->tp;
     t->skin = 0.3f;
     t->sort_interval = 0;
     t->use_graph = 1;
@@ -971,9 +971,40 @@ static double trial(rumd_system* s, const rumd_tuning& t, int steps)
     return 1000.0 * steps / ms;
 }
 
-// Coordinate descent over (method, tp, block size, skin).  The paper's empirical claim that the time has a
-// single minimum along each of pb, tp and skin is what makes this sound; the loop-breaking rules
-// follow P:386-391 in spirit (stop a direction once it is clearly worse than the best).
+// Coordinate descent over (method, tp, cell-build lanes, skin, persistent vs per-step kernels, block size).
+// The paper's empirical claim that the time has a single minimum along each of pb, tp and skin is
+// what makes this sound; the loop-breaking rules follow P:386-391 in spirit (stop a direction once it is
+// worse than the best).  The B200 dimensions the paper does not have: lanes per particle of the cell build
+// ("not been tried yet") and the persistent whole-run kernel vs per-step kernels in CUDA graphs.
+namespace {
+struct Tuner {
+    rumd_system* s;
+    int steps;
+    rumd_tuning cur;
+    double cur_tps = 0.0;
+    int trials = 0;
+    bool try_setting(const rumd_tuning& c)
+    {
+        ++trials;
+        const double tps = trial(s, c, steps);
+        if (tps > cur_tps) {
+            cur = c;
+            cur_tps = tps;
+            return true;
+        }
+        return false;
+    }
+    // walk one parameter both ways with `next(c, dir)` (returns false when out of range) until no gain
+    template <class Next> void descend(Next next)
+    {
+        for (int dir = -1; dir <= 1; dir += 2) {
+            rumd_tuning c = cur;
+            while (next(c, dir) && try_setting(c)) {}
+        }
+    }
+};
+} // namespace
+
 extern "C" rumd_status rumd_autotune(rumd_system* s, rumd_tuning* out, int steps_per_trial, double* tps_out)
 {
     rumd_status st = ready(s, true);
@@ -984,74 +1015,61 @@ extern "C" rumd_status rumd_autotune(rumd_system* s, rumd_tuning* out, int steps
     if (st != RUMD_OK) return st;
     const double rcm = rc_max_of(s);
     const double minL = std::min(s->box[0], std::min(s->box[1], s->box[2]));
-    const double skin_max = 0.5 * minL - rcm - 1e-4;
+    const float skin_max = (float)(0.5 * minL - rcm - 1e-4);
     rumd_tuning best = saved;
-    best.use_graph = 1;
     double best_tps = 0.0;
     std::vector<int> methods;
-    if (s->N <= 20000) methods.push_back(RUMD_NB_N2);
+    if (s->N <= 20000) methods.push_back(RUMD_NB_N2); // n2 is not tried for large systems
     methods.push_back(RUMD_NB_CELL);
     for (int method : methods) {
-        rumd_tuning cur = saved;
-        cur.use_graph = 1;
-        cur.method = method;
-        cur.skin = (float)std::min<double>(saved.skin, skin_max);
-        if (!(cur.skin > 0.f)) continue;
-        double cur_tps = trial(s, cur, steps_per_trial);
-        if (cur_tps <= 0.0 && method == RUMD_NB_CELL) continue; // grid too coarse for the stencil (S18)
+        rumd_tuning start;
+        rumd_default_tuning(s, &start);
+        start.method = method;
+        start.skin = std::min(saved.skin, skin_max);
+        if (!(start.skin > 0.f)) continue;
+        Tuner T{s, steps_per_trial, start};
+        if (!T.try_setting(start)) continue; // e.g. grid too coarse for the stencil (S18)
         for (int round = 0; round < 2; ++round) {
-            // threads per particle at fixed block size
-            const int threads = cur.pb * cur.tp;
-            for (int dir = -1; dir <= 1; dir += 2) {
-                rumd_tuning c = cur;
-                for (;;) {
-                    const int tp = dir < 0 ? c.tp / 2 : c.tp * 2;
-                    if (tp < 1 || tp > 32) break;
-                    c.tp = tp;
-                    c.pb = std::max(threads / tp, 32 / tp);
-                    if (c.pb * c.tp > 1024) break;
-                    const double tps = trial(s, c, steps_per_trial);
-                    if (tps > cur_tps) {
-                        cur = c;
-                        cur_tps = tps;
-                    } else
-                        break;
-                }
-            }
-            // block size at fixed tp
-            for (int dir = -1; dir <= 1; dir += 2) {
-                rumd_tuning c = cur;
-                for (;;) {
-                    const int th = dir < 0 ? c.pb * c.tp / 2 : c.pb * c.tp * 2;
-                    if (th < 32 || th > 1024) break;
-                    c.pb = th / c.tp;
-                    const double tps = trial(s, c, steps_per_trial);
-                    if (tps > cur_tps) {
-                        cur = c;
-                        cur_tps = tps;
-                    } else
-                        break;
-                }
-            }
-            // skin: +-15 % steps until the minimum is bracketed
-            for (int dir = -1; dir <= 1; dir += 2) {
-                rumd_tuning c = cur;
-                for (;;) {
-                    const float sk = c.skin * (dir < 0 ? 0.85f : 1.15f);
-                    if (sk < 0.05f || sk > skin_max) break;
-                    c.skin = sk;
-                    const double tps = trial(s, c, steps_per_trial);
-                    if (tps > cur_tps) {
-                        cur = c;
-                        cur_tps = tps;
-                    } else
-                        break;
-                }
-            }
+            const double before = T.cur_tps;
+            T.descend([](rumd_tuning& c, int dir) { // threads per particle
+                const int tp = dir < 0 ? c.tp / 2 : c.tp * 2;
+                if (tp < 1 || tp > 32) return false;
+                const int threads = std::max(32, c.pb * c.tp);
+                c.tp = tp;
+                c.pb = std::max(1, threads / tp);
+                return true;
+            });
+            T.descend([&](rumd_tuning& c, int dir) { // skin, +-15 % steps until the minimum is bracketed
+                const float sk = c.skin * (dir < 0 ? 0.85f : 1.15f);
+                if (sk < 0.05f || sk > skin_max) return false;
+                c.skin = sk;
+                return true;
+            });
+            if (method == RUMD_NB_CELL)
+                T.descend([&](rumd_tuning& c, int dir) { // lanes per particle of the cell build
+                    const int cur_b = c.build_tp > 0 ? c.build_tp : 1 << s->S.build_tp_shift;
+                    const int b = dir < 0 ? cur_b / 2 : cur_b * 2;
+                    if (b < 1 || b > 32) return false;
+                    c.build_tp = b;
+                    return true;
+                });
+            if (T.cur_tps < 1.02 * before) break;
         }
-        if (cur_tps > best_tps) {
-            best_tps = cur_tps;
-            best = cur;
+        {   // per-step kernels in CUDA graphs instead of the persistent kernel; there the block size matters
+            rumd_tuning c = T.cur;
+            c.persistent = 0;
+            c.use_graph = 1;
+            if (T.try_setting(c))
+                T.descend([](rumd_tuning& q, int dir) {
+                    const int th = dir < 0 ? q.pb * q.tp / 2 : q.pb * q.tp * 2;
+                    if (th < 32 || th > 1024 || th / q.tp < 1) return false;
+                    q.pb = th / q.tp;
+                    return true;
+                });
+        }
+        if (T.cur_tps > best_tps) {
+            best_tps = T.cur_tps;
+            best = T.cur;
         }
     }
     rumd_status r1 = rumd_set_tuning(s, best_tps > 0.0 ? &best : &saved);
