@@ -125,6 +125,26 @@ def fp32_peak_tflops(sm_mhz: float) -> float:
     return SM_COUNT * FP32_LANES_PER_SM * 2 * sm_mhz * 1e6 / 1e12
 
 
+# ------------------------------------------------------------------------------------------------ ranks
+
+
+def max_over_ranks(value: float, world: int, device="cpu") -> float:
+    """Max of a per-rank scalar over all ranks (torch.distributed must be initialised when world > 1)."""
+    if world <= 1:
+        return float(value)
+    import torch
+
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    torch.distributed.all_reduce(t, op=torch.distributed.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_rate(units_per_rank: float, seconds_local: float, world: int, device="cpu") -> float:
+    """Replicas only: every rank processes units_per_rank; the job's rate is the units all
+    ranks processed divided by the slowest rank's time."""
+    return world * units_per_rank / max_over_ranks(seconds_local, world, device)
+
+
 # ------------------------------------------------------------------------------------------------ GPU arm
 
 FLOP_PER_LISTED_PAIR_LJ = 42.0       # SURVEY.md 8(d) / DESIGN.md "Roofline": 21 always + 30 x 0.712 inside rc
@@ -189,10 +209,7 @@ def run_gpu(args, rank, world, local_rank):
     l1 = s.launch_count()
     ms = sum(a.elapsed_time(b) for a, b in ev)
     th1 = s.get_thermo()
-    if world > 1:
-        t = torch.tensor([ms], dtype=torch.float64, device=dev)
-        torch.distributed.all_reduce(t, op=torch.distributed.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(ms, world, dev)
     tsteps = args.steps * inner
     tps = world * tsteps / (ms * 1e-3)
 
@@ -219,12 +236,7 @@ def run_gpu(args, rank, world, local_rank):
         s.h_r.copy_(h_r), s.h_v.copy_(h_v), s.h_image.copy_(h_im), s.h_id.copy_(h_id)
         if it >= args.warmup:
             e2e_times.append(dt_)
-    e2e_s = sum(e2e_times)
-    if world > 1:
-        t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
-        torch.distributed.all_reduce(t, op=torch.distributed.ReduceOp.MAX)
-        e2e_s = float(t.item())
-    e2e_tps = world * tsteps / e2e_s
+    e2e_tps = whole_job_rate(tsteps, sum(e2e_times), world, dev)
 
     out = None
     if rank == 0:
