@@ -578,10 +578,12 @@ static rumd_status launch_persistent(rumd_system* s, int nsteps)
         int per_sm = 0;
         CUDA_TRY(s, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, threads, 0));
         if (per_sm < 1) return fail(s, RUMD_ERR_CUDA, "persistent kernel does not fit an SM");
+        // whole multiples of the SM count (every SM carries the same number of blocks; the kernel splits the
+        // work into equal contiguous chunks per block), as many as the work can fill, at most what is co-resident
         const long long want = ((long long)s->N * s->tune.tp + threads - 1) / threads;
-        long long grid = std::min<long long>(want, (long long)per_sm * s->num_sms);
-        grid = std::min<long long>(grid, 4096);
-        s->persist_grid = (int)std::max<long long>(1, grid);
+        long long per = std::min<long long>(per_sm, (want + s->num_sms - 1) / s->num_sms);
+        per = std::max<long long>(1, per);
+        s->persist_grid = (int)std::min<long long>(per * s->num_sms, 4096);
         s->persist_threads = threads;
         s->persist_grid_for = sig;
     }

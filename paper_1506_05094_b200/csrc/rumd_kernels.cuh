@@ -422,8 +422,9 @@ __device__ __forceinline__ void ph_build_cell(const Sys& S, const float4* r, con
             S.num_nbrs[i] = min(count, S.cap);
             S.r_build[i] = ri;
             if (count > S.cap) S.sc->overflow = 1u;
-            atomicMax(max_slot, count);
         }
+        const int wmax = __reduce_max_sync(FULLMASK, count); // one atomic per warp, not per particle
+        if (lane == 0) atomicMax(max_slot, wmax);
     }
 }
 

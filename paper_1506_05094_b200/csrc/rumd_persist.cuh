@@ -112,7 +112,8 @@ __global__ void __launch_bounds__(PERSIST_THREADS, PERSIST_MINB) k_persist(const
     float4* rc = S.r;     // positions r(t) of the current step
     float4* rn = S.r_alt; // where r(t+dt) goes
     const int nchunks = (S.grid.ncell + SCAN_CHUNK - 1) / SCAN_CHUNK;
-    const long long nvt_threads = (long long)S.N * TP;
+    const long long nvwarps = ((long long)S.N * TP + 31) / 32;
+    const long long vw0 = nvwarps * blockIdx.x / gridDim.x, vw1 = nvwarps * (blockIdx.x + 1) / gridDim.x;
     if (threadIdx.x == 0) {
         s_moved = 0;
         s_ab[0] = 1.0f;
@@ -201,7 +202,10 @@ __global__ void __launch_bounds__(PERSIST_THREADS, PERSIST_MINB) k_persist(const
         const bool last = k == nsteps - 1;
         double kt = 0.0, mv2 = 0.0;
         bool moved = false;
-        for (long long vt = first; vt - lane < nvt_threads; vt += stride) {
+        // the N*TP/32 warps of work are split into gridDim.x contiguous, equally long chunks (spatial locality
+        // inside a block, every SM equally loaded); the block's warps take the warps of its chunk in turn
+        for (long long vw = vw0 + wid; vw < vw1; vw += nw) {
+            const long long vt = vw * 32 + lane;
             const int i = (int)(vt / TP);
             const int t = (int)(vt % TP);
             const bool have_i = i < S.N;
@@ -213,9 +217,9 @@ __global__ void __launch_bounds__(PERSIST_THREADS, PERSIST_MINB) k_persist(const
             }
             float fx, fy, fz, u, w;
             if (last) // energies and virials are outputs of the LAST force evaluation only
-                force_group<TP, COUL, ONE_TYPE, UNROLL, false, true>(S, rc, s_pp, (int)(vt >> 5), i, t, have_i, ri, cnt, fx, fy, fz, u, w);
+                force_group<TP, COUL, ONE_TYPE, UNROLL, false, true>(S, rc, s_pp, (int)vw, i, t, have_i, ri, cnt, fx, fy, fz, u, w);
             else
-                force_group<TP, COUL, ONE_TYPE, UNROLL, false, false>(S, rc, s_pp, (int)(vt >> 5), i, t, have_i, ri, cnt, fx, fy, fz, u, w);
+                force_group<TP, COUL, ONE_TYPE, UNROLL, false, false>(S, rc, s_pp, (int)vw, i, t, have_i, ri, cnt, fx, fy, fz, u, w);
             if (have_i && t == 0) {
                 while (*((volatile int*)&s_ab_step) <= k) {} // factors of step k published? (warp 0, above)
                 __threadfence_block();

@@ -107,6 +107,72 @@ CASES = [
 ]
 
 
+def test_one_lane_build_wide_box_matches_oracle(rumd):
+    """A4 with one thread per particle (the paper's P:278 configuration) in a wide box: N = 42592 (22^3 fcc
+    cells, 26 cells per axis, interior fast path of the minimum image in play), whole list and all forces
+    against the oracle's cell search."""
+    wl = perturbed(make("lj", ncell=22))
+    s = rumd.from_workload(wl)
+    s.set_tuning(method=rumd.NB_CELL, tp=1, pb=256, build_tp=1)
+    s.compute_forces()
+    r64 = wl.r.astype(np.float64)
+    box = wl.box.astype(np.float64)
+    cnt, npairs, nband = check_nblist(s, r64, wl.types, box, wl.pot, float(wl.skin))
+    assert npairs > 3e6
+    check_forces(s, r64, wl.types, box, wl.pot)
+    # the same list as the several-lanes-per-particle build (as sets; row order differs)
+    keys_g1 = np.sort(pair_keys(*s.export_nblist(), s.d_id.cpu().numpy().astype(np.int64)))
+    s.set_tuning(build_tp=8)
+    s.build_nblist()
+    keys_g8 = np.sort(pair_keys(*s.export_nblist(), s.d_id.cpu().numpy().astype(np.int64)))
+    assert np.array_equal(keys_g1, keys_g8)
+    s.close()
+
+
+def test_full_size_million_particles_sampled_against_oracle(rumd):
+    """configs[3] at full size (N = 1 048 576) in the configuration bench.py times (autotuned defaults): list
+    rows and forces of 64 sampled particles against the oracle, each computed on the cluster of all particles
+    within rc + skin + 0.2 of the sample (which contains every interaction partner); plus properties that hold
+    at any size: symmetric list, zero total force."""
+    wl = perturbed(make("lj", ncell=64))
+    s = rumd.from_workload(wl)
+    s.compute_forces()
+    N = wl.N
+    r64 = wl.r.astype(np.float64)
+    box = wl.box.astype(np.float64)
+    cnt, lst = s.export_nblist()
+    ids = s.d_id.cpu().numpy().astype(np.int64)
+    slot_of = np.empty(N, np.int64)
+    slot_of[ids] = np.arange(N)
+    st = s.state()
+    rng = np.random.default_rng(5)
+    skin = float(wl.skin)
+    for i in rng.choice(N, 64, replace=False):
+        d = r64 - r64[i]
+        d -= box * np.rint(d / box)
+        near = np.flatnonzero((d * d).sum(1) < (2.5 + skin + 0.2) ** 2)   # contains i itself
+        sub = np.concatenate(([i], near[near != i]))
+        F, u, w = oracle.forces_allpairs(r64[sub], wl.types[sub], box, wl.pot)
+        oc, ol = oracle.nblist(r64[sub], wl.types[sub], box, wl.pot, skin, method="n2")
+        want = set(sub[ol[0, :oc[0]]].tolist())
+        row = slot_of[i]
+        got = set(ids[lst[row, :cnt[row]]].tolist())
+        for j in want ^ got:
+            dj = r64[j] - r64[i]
+            dj -= box * np.rint(dj / box)
+            assert abs(np.sqrt((dj * dj).sum()) - (2.5 + skin)) <= BAND
+        rmsF = np.sqrt((st["F"].astype(np.float64) ** 2).sum(1).mean())
+        assert np.sqrt(((st["F"][i] - F[0]) ** 2).sum()) <= FORCE_TOL * rmsF
+        assert abs(st["u"][i] - u[0]) <= 1e-5 * max(1.0, abs(u[0]))
+    # any-size properties
+    assert cnt.sum() % 2 == 0 and 70 < cnt.mean() < 90
+    Fsum = st["F"].astype(np.float64).sum(0)
+    assert np.abs(Fsum).max() <= 1e-3 * np.abs(st["F"]).sum()          # Newton's third law through a full list
+    th = s.get_thermo()
+    assert th["overflow"] == 0
+    s.close()
+
+
 @pytest.mark.parametrize("kind,kw,method,tp", CASES)
 def test_nblist_and_forces_match_oracle(rumd, kind, kw, method, tp):
     wl = perturbed(make(kind, **kw))
