@@ -8,18 +8,25 @@
 // O3/O4/O5 for one listed pair: adds f_SF(r) d/r to (fx,fy,fz) and -- only when ENERGY -- u_SF to u and
 // r f_SF to w (the halving of u and w is done once per particle).  Every term applies its own cutoff
 // (S5, strict <, S3).  Branch-free: a warp almost never has all 32 pairs outside the cutoff, so the terms are
-// computed for every pair and selected.  1/r = MUFU.RSQ + one Newton step (the r^-14 force term amplifies its
-// error 14-fold); 1/r^2 = (1/r)^2.
+// computed for every pair and selected.  1/r^2 = MUFU.RCP(r^2) (1 ulp; the r^-14 force term amplifies it 7-fold
+// to < 1e-6 relative per pair, two orders inside the 1e-4 rms|F| bar) and 1/r = MUFU.RSQ(r^2) (2 ulp; used
+// only in the small shifted-force terms and the Coulomb term): no Newton steps.
 //   pf = (12 c12, 6 c6, rc_lj^2, fc_lj)   pc = (qq, rc_c^2, fc_c, -)   pe = (c12, c6, k0_lj, k0_c)
+__device__ __forceinline__ float __frcp_approx(float x)
+{
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
 template <bool COUL, bool ENERGY>
 __device__ __forceinline__ void pair_accumulate(const float4 pf, const float4 pc, const float4 pe, bool ok,
                                                 float dx, float dy, float dz, float& fx, float& fy, float& fz,
                                                 float& u, float& w)
 {
     const float r2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, dx * dx));
-    float y = rsqrtf(r2);
-    y = y * __fmaf_rn(-0.5f * r2, y * y, 1.5f); // Newton: y <- y (3 - r2 y^2)/2
-    const float rinv2 = y * y;
+    const float y = rsqrtf(r2);
+    const float rinv2 = __frcp_approx(r2);
     const float rinv6 = rinv2 * rinv2 * rinv2;
     const float r = r2 * y;
     const bool in_lj = ok && r2 < pf.z;
@@ -70,10 +77,10 @@ __device__ __forceinline__ void pair_accumulate(const float4 pf, const float4 pc
 template <bool NC> __device__ __forceinline__ int load_idx(const int* p) { return NC ? __ldg(p) : __ldcs(p); }
 template <bool NC> __device__ __forceinline__ float4 load_pos(const float4* p) { return NC ? __ldg(p) : *p; }
 
-template <int TP, bool COUL, bool ONE_TYPE, int UNROLL, bool NC, bool ENERGY, bool WRAP>
-__device__ __forceinline__ void force_loop(const Sys& S, const float4* r, const float4* s_pp, const int* base, int i,
-                                           int nit, int nit_w, const float4 ri, float& fx, float& fy, float& fz,
-                                           float& u, float& w)
+template <int TP, bool COUL, bool ONE_TYPE, int UNROLL, bool NC, bool ENERGY, bool WRAP, bool MASKED>
+__device__ __forceinline__ void force_loop(const Sys& S, const float4* r, const float4* s_pp, const int* base,
+                                           int it_begin, int nit, int it_end, const float4 ri, float& fx, float& fy,
+                                           float& fz, float& u, float& w)
 {
     const int trow = ONE_TYPE ? 0 : 4 * type_of(ri) * S.ntypes;
     float4 pf, pc, pe;
@@ -85,13 +92,13 @@ __device__ __forceinline__ void force_loop(const Sys& S, const float4* r, const 
     }
     const float hx = S.h[0], hy = S.h[1], hz = S.h[2];
     const float ix = S.invL[0], iy = S.invL[1], iz = S.invL[2];
-    for (int it = 0; it < nit_w; it += UNROLL) {
+    for (int it = it_begin; it < it_end; it += UNROLL) {
         int j[UNROLL];
         bool ok[UNROLL];
         float4 rj[UNROLL];
 #pragma unroll
         for (int q = 0; q < UNROLL; ++q) {
-            ok[q] = (it + q) < nit;
+            ok[q] = !MASKED || (it + q) < nit;
             j[q] = ok[q] ? load_idx<NC>(base + (size_t)(it + q) * 32) : 0; // masked lanes gather slot 0 (always valid)
         }
 #pragma unroll
@@ -130,11 +137,16 @@ __device__ __forceinline__ void force_group(const Sys& S, const float4* r, const
     const int nit_w = __reduce_max_sync(FULLMASK, nit);
     const int* base = S.nbl + (size_t)vwarp * S.cap_it * 32 + lane;
     fx = fy = fz = u = w = 0.f;
+    // iterations every lane of the warp has (no masks needed), then the ragged tail
+    const int nit_all = __reduce_min_sync(FULLMASK, have_i ? nit : 0) / UNROLL * UNROLL;
     const bool interior = fabsf(ri.x) < S.hin[0] && fabsf(ri.y) < S.hin[1] && fabsf(ri.z) < S.hin[2];
-    if (__any_sync(FULLMASK, have_i && !interior))
-        force_loop<TP, COUL, ONE_TYPE, UNROLL, NC, ENERGY, true>(S, r, s_pp, base, i, nit, nit_w, ri, fx, fy, fz, u, w);
-    else
-        force_loop<TP, COUL, ONE_TYPE, UNROLL, NC, ENERGY, false>(S, r, s_pp, base, i, nit, nit_w, ri, fx, fy, fz, u, w);
+    if (__any_sync(FULLMASK, have_i && !interior)) {
+        force_loop<TP, COUL, ONE_TYPE, UNROLL, NC, ENERGY, true, false>(S, r, s_pp, base, 0, nit, nit_all, ri, fx, fy, fz, u, w);
+        force_loop<TP, COUL, ONE_TYPE, UNROLL, NC, ENERGY, true, true>(S, r, s_pp, base, nit_all, nit, nit_w, ri, fx, fy, fz, u, w);
+    } else {
+        force_loop<TP, COUL, ONE_TYPE, UNROLL, NC, ENERGY, false, false>(S, r, s_pp, base, 0, nit, nit_all, ri, fx, fy, fz, u, w);
+        force_loop<TP, COUL, ONE_TYPE, UNROLL, NC, ENERGY, false, true>(S, r, s_pp, base, nit_all, nit, nit_w, ri, fx, fy, fz, u, w);
+    }
 #pragma unroll
     for (int o = TP / 2; o; o >>= 1) {
         fx += __shfl_xor_sync(FULLMASK, fx, o);
