@@ -362,31 +362,49 @@ __device__ __forceinline__ void ph_build_cell(const Sys& S, const float4* r, con
             w1 = cx + 2 - nx;
         }
         int count = 0;
-        // particle ranges of stencil row q (0..24): main [a.x, a.y) and wrapped [b.x, b.y)
-        auto ranges_of = [&](int q, int2& a, int2& b) {
+        // Minimum image without per-pair rounding work: all candidates of one range lie in cells reached with
+        // the same periodic shift s in {-1, 0, +1} per axis (s != 0 where the stencil row, or the wrapped x
+        // segment, crossed a face), and d = (x_i - s h) - (x_j + s h) is the exact nearest-image displacement
+        // for every pair that can be inside the list cutoff (both brackets are exact, cf. min_image; needs
+        // n >= 5 cells per axis, S18).  sxh: shift of the wrapped x segment; the main segment has none.
+        const float sxh = cx - 2 < 0 ? -S.h[0] : S.h[0];
+        // particle ranges of stencil row q (0..24): main [a.x, a.y) and wrapped [b.x, b.y); its y / z shifts
+        auto ranges_of = [&](int q, int2& a, int2& b, float& syh, float& szh) {
             a = b = make_int2(0, 0);
+            syh = szh = 0.f;
             if (!have_i || q >= 25) return;
             int z = cz + q / 5 - 2, y = cy + q % 5 - 2;
-            z += z < 0 ? nz : 0;
-            z -= z >= nz ? nz : 0;
-            y += y < 0 ? ny : 0;
-            y -= y >= ny ? ny : 0;
+            if (z < 0) {
+                z += nz;
+                szh = -S.h[2];
+            } else if (z >= nz) {
+                z -= nz;
+                szh = S.h[2];
+            }
+            if (y < 0) {
+                y += ny;
+                syh = -S.h[1];
+            } else if (y >= ny) {
+                y -= ny;
+                syh = S.h[1];
+            }
             const int* cs = S.cstart_z + S.rowrank[z * ny + y] * nx;
             a = make_int2(cs[x0], cs[x1 + 1]);
             if (w0 <= w1) b = make_int2(cs[w0], cs[w1 + 1]);
         };
-        // A particle further than the list cutoff from every face has no listed neighbour across a periodic
-        // boundary, and a wrapped candidate's plain difference is ~L, which fails the test anyway: when this
-        // holds for the whole warp the plain difference replaces the minimum image (hin is a little stricter).
-        const bool interior = fabsf(ri.x) < S.hin[0] && fabsf(ri.y) < S.hin[1] && fabsf(ri.z) < S.hin[2];
-        const bool wrap = __any_sync(FULLMASK, have_i && !interior);
+        // this particle's row of the tiled list: entry k at rowbase[(k >> tp_shift) * 32 + (k & (tp - 1))]
+        int* rowbase = S.nbl + ((size_t)(i >> S.ppw_shift) * S.cap_it * 32 + ((i & ((1 << S.ppw_shift) - 1)) << S.tp_shift));
+        const int tmask = (1 << S.tp_shift) - 1;
         int2 na, nb;
-        ranges_of(l, na, nb);
+        float nsy, nsz;
+        ranges_of(l, na, nb, nsy, nsz);
         for (int q0 = 0; q0 < 25; q0 += G) {
             const int2 a = na, b = nb;
-            if (q0 + G < 25) ranges_of(q0 + G + l, na, nb); // one-ahead prefetch of the next round's ranges
+            const float syh = nsy, szh = nsz;
+            if (q0 + G < 25) ranges_of(q0 + G + l, na, nb, nsy, nsz); // one-ahead prefetch of the next round's ranges
             const int n0 = a.y - a.x, n = n0 + (b.y - b.x);
             const int nmax = __reduce_max_sync(FULLMASK, n);
+            const float ay = ri.y - syh, az = ri.z - szh, axw = ri.x - sxh;
             constexpr int U = 4; // candidates in flight per lane
             for (int it0 = 0; it0 < nmax; it0 += U) {
                 float4 rj[U];
@@ -401,18 +419,15 @@ __device__ __forceinline__ void ph_build_cell(const Sys& S, const float4* r, con
                 }
 #pragma unroll
                 for (int q = 0; q < U; ++q) {
-                    float d2;
-                    if (wrap)
-                        d2 = list_dist2(S, ri, rj[q]);
-                    else {
-                        const float dx = ri.x - rj[q].x, dy = ri.y - rj[q].y, dz = ri.z - rj[q].z;
-                        d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, dx * dx));
-                    }
+                    const bool inwrap = it0 + q >= n0;
+                    const float dx = inwrap ? axw - (rj[q].x + sxh) : ri.x - rj[q].x;
+                    const float dy = ay - (rj[q].y + syh), dz = az - (rj[q].z + szh);
+                    const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, dx * dx));
                     const bool acc = have_i && j[q] != i && d2 < s_rcl2[trow + type_of(rj[q])];
                     const unsigned m = __ballot_sync(FULLMASK, acc);
                     if (acc) {
                         const int k = count + __popc(m & lt);
-                        if (k < S.cap) S.nbl[nbl_index(S, i, k)] = j[q];
+                        if (k < S.cap) rowbase[((k >> S.tp_shift) << 5) + (k & tmask)] = j[q];
                     }
                     count += __popc(m & gmask);
                 }
