@@ -147,6 +147,11 @@ def whole_job_rate(units_per_rank: float, seconds_local: float, world: int, devi
 
 # ------------------------------------------------------------------------------------------------ GPU arm
 
+# DRAM bytes (read + write) per MD time step of the dominant kernel, from the committed ncu --set full captures
+# (profiles/r01_persist_c1_ncu.md: 4.68 MB per 200-step k_persist launch at C1; profiles/r01_force_lj1m_ncu.md:
+# 378 MB per k_force launch at C3).  Workloads without a capture report traffic = null.
+NCU_DRAM_BYTES_PER_TIMESTEP = {"ka8000": 4.68e6 / 200, "lj1m": 378e6}
+
 FLOP_PER_LISTED_PAIR_LJ = 42.0       # SURVEY.md 8(d) / DESIGN.md "Roofline": 21 always + 30 x 0.712 inside rc
 FLOP_PER_LISTED_PAIR_COUL = 50.0     # + the Coulomb term
 
@@ -265,7 +270,11 @@ def run_gpu(args, rank, world, local_rank):
             phases = s.profile_persistent(inner)
             roof = {"kernel": "k_persist (one launch = %d time steps: rebuilds + forces + integration)" % inner,
                     "bound": "alu", "achieved": ach, "peak": peak_tf, "unit": "TFLOP/s", "frac": ach / peak_tf,
-                    "traffic": None, "us_per_launch": us_launch, "phases_us_per_timestep": phases}
+                    "traffic": (NCU_DRAM_BYTES_PER_TIMESTEP[args.workload] * inner
+                                if args.workload in NCU_DRAM_BYTES_PER_TIMESTEP else None),
+                    "traffic_source": "ncu dram__bytes_read.sum + dram__bytes_write.sum, profiles/r01_*_ncu.md",
+                    "algorithmic_bytes": alg_bytes * inner,
+                    "us_per_launch": us_launch, "phases_us_per_timestep": phases}
         else:
             roof = {"kernel": "k_force", "bound": "alu", "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s",
                     "frac": ach_tf / peak_tf, "traffic": None, "us_per_launch": us,
