@@ -348,6 +348,62 @@ def test_overflow_is_reported_and_capacity_doubles(rumd):
     s.close()
 
 
+def _gas(N, ntypes, box, seed, pot):
+    r, types = W.random_gas(N, ntypes, box, seed)
+    rng = np.random.default_rng(seed + 1)
+    m = np.ones(N, np.float32)
+    v = (0.5 * rng.standard_normal((N, 3))).astype(np.float32)
+    return r, v, m, types, np.asarray(box, np.float32), pot
+
+
+@pytest.mark.parametrize("N,box,method,tp,persistent", [
+    (1, (12.0, 12.0, 12.0), "n2", 32, 1),        # a single particle: empty list, zero force
+    (5, (30.0, 30.0, 30.0), "cell", 1, 1),       # dilute: almost every cell empty, most rows empty
+    (33, (9.0, 9.0, 9.0), "n2", 4, 0),           # one particle past a warp boundary
+    (33, (9.0, 9.0, 9.0), "cell", 8, 1),
+    (257, (8.0, 11.0, 14.0), "cell", 2, 1),      # orthorhombic, ragged last block, 4 types
+    (257, (8.0, 11.0, 14.0), "n2", 16, 0),
+])
+def test_degenerate_and_ragged_inputs(rumd, N, box, method, tp, persistent):
+    """Edge cases of every kernel path: empty and nearly empty lists, sizes that are not multiples of the warp,
+    block or tile sizes, four particle types with all six pair potentials different, anisotropic boxes."""
+    nt = 4 if N > 33 else 1
+    pot = W.pot_table(nt)
+    for a in range(nt):
+        for b in range(a, nt):
+            W.set_lj(pot, a, b, 1.0 + 0.1 * (a + b), 1.0 - 0.04 * (a + b), 2.5 * (1.0 - 0.04 * (a + b)))
+    r, v, m, types, boxf, pot = _gas(N, nt, box, 77 + N, pot)
+    s = rumd.System(r, v, m, types, boxf, pot)
+    s.set_integrator(rumd.INT_NVE_LEAPFROG, 0.004)
+    s.set_tuning(method=rumd.NB_CELL if method == "cell" else rumd.NB_N2, tp=tp, pb=max(1, 64 // tp), skin=0.3,
+                 persistent=persistent, use_graph=0)
+    s.compute_forces()
+    r64, b64 = r.astype(np.float64), boxf.astype(np.float64)
+    cnt, lst = s.export_nblist()
+    ids = s.d_id.cpu().numpy().astype(np.int64)
+    oc, ol = oracle.nblist(r64, types, b64, pot, 0.3, method="n2")
+    assert np.array_equal(np.sort(pair_keys(cnt, lst, ids)), np.sort(pair_keys(oc, ol)))
+    F, u, w = oracle.forces_allpairs(r64, types, b64, pot)
+    st = s.state()
+    scale = max(1e-3, np.sqrt((F * F).sum(1).mean()))
+    assert np.sqrt(((st["F"] - F) ** 2).sum(1)).max() <= FORCE_TOL * scale
+    assert np.abs(st["u"] - u).max() <= 1e-5 * max(1.0, np.abs(u).max())
+    # 37 steps (odd: ends in the alternate position buffer) against the oracle's trajectory: short, so fp32
+    # and fp64 have not separated yet
+    s.run_steps(37)
+    th = s.get_thermo()
+    assert th["n_steps"] == 37 and np.isfinite(th["H"])
+    o = oracle.run(r64, v.astype(np.float64), m.astype(np.float64), np.zeros((N, 3), np.int32), types, b64, pot, 0.3,
+                   0.004, 37)
+    st = s.state()
+    d = st["r"].astype(np.float64) - o["r"]
+    d -= b64 * np.rint(d / b64)                     # positions compared modulo L (S7)
+    assert np.abs(d).max() < 2e-4
+    assert s.run_steps(0) is None                   # zero steps is a no-op
+    assert s.get_thermo()["n_steps"] == 37
+    s.close()
+
+
 def test_graph_and_plain_launch_agree_bitwise(rumd):
     wl = perturbed(make("ka", N=1000))
     res = []
