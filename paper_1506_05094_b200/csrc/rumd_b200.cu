@@ -163,7 +163,7 @@ static size_t carve(rumd_system* s, char* base, int cap)
     p = take(nc * 4); if (base) S.rowrank = (int*)p;
     p = take((nc / SCAN_CHUNK + 2) * 4); if (base) S.blocksum = (int*)p;
     // (kt, mv2) per block: integrator kernel (N/128 blocks) or persistent kernel (2 sets x <= 4096 blocks)
-    const size_t nblk = std::max<size_t>((N + 31) / 32 + 1, 2 * 4096);
+    const size_t nblk = std::max<size_t>(N + 1, 2 * 4096); // the fused per-step kernel may run N blocks (pb = 1)
     p = take(nblk * 16); if (base) S.partial = (double*)p;
     p = take(8 * 8); if (base) s->prof_buf = (long long*)p;
     return off;
@@ -602,17 +602,20 @@ static int launch_rebuild_chain(rumd_system* s)
     const Sys& S = s->S;
     int n = 0;
     const bool sorting = s->tune.method == RUMD_NB_CELL || s->tune.sort_interval > 0;
+    // Every phase strides over its items, so the grids are capped at a few blocks per SM: on the (many) steps
+    // without a rebuild each kernel only reads the flag and exits, and that costs time per BLOCK.
+    const int cap256 = s->num_sms * 8, cap128 = s->num_sms * 16;
     if (sorting) {
-        const int nbp = (s->N + 255) / 256, nbc = (S.grid.ncell + 255) / 256;
+        const int nbp = std::min((s->N + 255) / 256, cap256), nbc = std::min((S.grid.ncell + 255) / 256, cap256);
         const int nchunks = (S.grid.ncell + SCAN_CHUNK - 1) / SCAN_CHUNK;
         k_cell_assign<<<nbp, 256, 0, s->stream>>>(S);
         if (nchunks <= 8) {
             k_scan_single<<<1, SCAN_THREADS, 0, s->stream>>>(S);
             n += 2;
         } else {
-            k_scan_sums<<<std::min(nchunks, 1024), SCAN_THREADS, 0, s->stream>>>(S);
+            k_scan_sums<<<std::min(nchunks, cap256), SCAN_THREADS, 0, s->stream>>>(S);
             k_scan_blocks<<<1, SCAN_THREADS, 0, s->stream>>>(S);
-            k_scan_apply<<<std::min(nchunks, 1024), SCAN_THREADS, 0, s->stream>>>(S);
+            k_scan_apply<<<std::min(nchunks, cap256), SCAN_THREADS, 0, s->stream>>>(S);
             n += 4;
         }
         k_cell_scatter<<<nbp, 256, 0, s->stream>>>(S);
@@ -623,11 +626,24 @@ static int launch_rebuild_chain(rumd_system* s)
     }
     if (s->tune.method == RUMD_NB_CELL) {
         const long long threads = (long long)s->N << S.build_tp_shift;
-        k_build_cell<<<(unsigned)((threads + 127) / 128), 128, 0, s->stream>>>(S);
+        k_build_cell<<<(unsigned)std::min<long long>((threads + 127) / 128, cap128), 128, 0, s->stream>>>(S);
     } else
-        k_build_n2<<<(s->N + 3) / 4, 128, 0, s->stream>>>(S);
+        k_build_n2<<<std::min((s->N + 3) / 4, cap128), 128, 0, s->stream>>>(S);
     return n + 1;
 }
+
+// fused force + integrate step of the per-step path: positions go from `from_alt ? r_alt : r` to the other buffer
+template <int TP, bool COUL, bool ONE> struct StepLaunch {
+    static int run(rumd_system* s, int nblocks, int nthreads, const Sys* S, int energy)
+    {
+        const int nvt = s->integ == RUMD_INT_NVT_NOSE_HOOVER;
+        if (energy)
+            k_step<TP, COUL, ONE, UnrollOf<TP>::value, true><<<nblocks, nthreads, 0, s->stream>>>(*S, nvt);
+        else
+            k_step<TP, COUL, ONE, UnrollOf<TP>::value, false><<<nblocks, nthreads, 0, s->stream>>>(*S, nvt);
+        return 1;
+    }
+};
 
 static int launch_integrate(rumd_system* s)
 {
@@ -672,6 +688,27 @@ extern "C" rumd_status rumd_compute_forces(rumd_system* s)
 
 // Whole-timestep CUDA graph: `steps` time steps (each the full early-exit chain) captured once and replayed;
 // removes the per-kernel launch cost that dominates at small N.
+// Two fused steps: r -> r_alt -> r.  The second one runs on a copy of the parameter block with the two
+// position buffers exchanged (its rebuild chain sorts and lists the positions where they currently are).
+static int launch_step_pair(rumd_system* s, bool energy_on_second)
+{
+    const int tp = s->tune.tp, nthreads = s->tune.pb * tp;
+    const int nblocks = (int)(((size_t)s->N * tp + nthreads - 1) / nthreads);
+    Sys A = s->S;
+    A.r_out = A.r_alt;
+    Sys B = s->S;
+    B.r = s->S.r_alt;
+    B.r_out = s->S.r;
+    int n = launch_rebuild_chain(s);
+    n += pick_kernel<StepLaunch>(s, nblocks, nthreads, (const Sys*)&A, 0);
+    const Sys keep = s->S;
+    s->S = B; // the chain launchers read s->S
+    n += launch_rebuild_chain(s);
+    s->S = keep;
+    n += pick_kernel<StepLaunch>(s, nblocks, nthreads, (const Sys*)&B, energy_on_second ? 1 : 0);
+    return n;
+}
+
 static rumd_status get_graph(rumd_system* s, GraphCache& gc, int steps, int* kernels_per_graph)
 {
     if (gc.exec && gc.steps == steps) {
@@ -683,7 +720,10 @@ static rumd_status get_graph(rumd_system* s, GraphCache& gc, int steps, int* ker
     cudaGraph_t g = nullptr;
     CUDA_TRY(s, cudaStreamBeginCapture(s->stream, cudaStreamCaptureModeThreadLocal));
     int n = 0;
-    for (int q = 0; q < steps; ++q) n += launch_step(s);
+    if (steps % 2 == 0)
+        for (int q = 0; q < steps; q += 2) n += launch_step_pair(s, q + 2 == steps);
+    else
+        for (int q = 0; q < steps; ++q) n += launch_step(s);
     cudaError_t e = cudaStreamEndCapture(s->stream, &g);
     if (e != cudaSuccess) return fail(s, RUMD_ERR_CUDA, "graph capture failed: %s", cudaGetErrorString(e));
     e = cudaGraphInstantiate(&gc.exec, g, 0);

@@ -347,6 +347,49 @@ __global__ void __launch_bounds__(INT_THREADS) k_integrate(const Sys S, int nvt)
     step_tail<INT_THREADS / 32>(S, nvt != 0, kt, mv2, moved, gridDim.x);
 }
 
+// A5 + A6 fused for the per-step path: forces of r(t) read from S.r, leap-frog update written to S.r_out
+// (the OTHER position buffer: nobody reads a position that was already advanced), then the same block tail as
+// k_integrate.  Saves the integrator's pass over r, v, f (~112 B per particle) and one launch per step.
+// ENERGY: also write f, u, w (the step whose force evaluation is an output of the run).
+template <int TP, bool COUL, bool ONE_TYPE, int UNROLL, bool ENERGY>
+__global__ void __launch_bounds__(1024, 1) k_step(const Sys S, int nvt)
+{
+    __shared__ float4 s_pp[4 * RUMD_MAXT * RUMD_MAXT];
+    load_pair_table(S, s_pp);
+    __syncthreads();
+    if (blockIdx.x == 0 && threadIdx.x == 0) finish_rebuild(S);
+    float a, b;
+    nvt_factors(S, nvt != 0, a, b);
+    const int tid = blockIdx.x * blockDim.x + threadIdx.x;
+    const int i = tid / TP;
+    const int t = tid % TP;
+    const bool have_i = i < S.N;
+    float4 ri = make_float4(0.f, 0.f, 0.f, 0.f);
+    int cnt = 0;
+    if (have_i) {
+        ri = __ldg(&S.r[i]);
+        cnt = S.num_nbrs[i];
+    }
+    float fx, fy, fz, u, w;
+    force_group<TP, COUL, ONE_TYPE, UNROLL, true, ENERGY>(S, S.r, s_pp, tid >> 5, i, t, have_i, ri, cnt, fx, fy, fz, u, w);
+    double kt = 0.0, mv2 = 0.0;
+    bool moved = false;
+    if (have_i && t == 0) {
+        const float4 f = make_float4(fx, fy, fz, 0.5f * u);
+        float4 v = S.v[i];
+        int4 im = S.image[i];
+        integrate_particle(S, a, b, ri, v, f, im, S.r_build[i], moved, kt, mv2);
+        S.r_out[i] = ri;
+        S.v[i] = v;
+        S.image[i] = im;
+        if (ENERGY) {
+            S.f[i] = f;
+            S.w[i] = 0.5f * w;
+        }
+    }
+    step_tail<32>(S, nvt != 0, kt, mv2, moved, gridDim.x);
+}
+
 // ------------------------------------------------------------------------------------------ small kernels
 
 __global__ void k_request_rebuild(const Sys S)
