@@ -424,12 +424,19 @@ __device__ __forceinline__ void ph_build_cell(const Sys& S, const float4* r, con
                     const float dy = ay - (rj[q].y + syh), dz = az - (rj[q].z + szh);
                     const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, dx * dx));
                     const bool acc = have_i && j[q] != i && d2 < s_rcl2[trow + type_of(rj[q])];
-                    const unsigned m = __ballot_sync(FULLMASK, acc);
-                    if (acc) {
-                        const int k = count + __popc(m & lt);
-                        if (k < S.cap) rowbase[((k >> S.tp_shift) << 5) + (k & tmask)] = j[q];
+                    if (G == 1) { // the lane owns the row: no slot negotiation
+                        if (acc) {
+                            if (count < S.cap) rowbase[((count >> S.tp_shift) << 5) + (count & tmask)] = j[q];
+                            ++count;
+                        }
+                    } else {
+                        const unsigned m = __ballot_sync(FULLMASK, acc);
+                        if (acc) {
+                            const int k = count + __popc(m & lt);
+                            if (k < S.cap) rowbase[((k >> S.tp_shift) << 5) + (k & tmask)] = j[q];
+                        }
+                        count += __popc(m & gmask);
                     }
-                    count += __popc(m & gmask);
                 }
             }
         }
