@@ -441,8 +441,8 @@ static rumd_status refresh(rumd_system* s)
     S.sort_interval = t.sort_interval;
     S.method = t.method;
     S.r_out = S.r;
-    {   // lanes per particle of the cell build: a whole warp while the machine is not full, fewer at large N
-        const int btp = t.build_tp > 0 ? t.build_tp : s->N <= 16384 ? 32 : s->N <= 65536 ? 16 : s->N <= 262144 ? 8 : 4;
+    {   // lanes per particle of the cell build: several while the machine is not full, one at large N (measured)
+        const int btp = t.build_tp > 0 ? t.build_tp : s->N <= 32768 ? 8 : 1;
         S.build_tp_shift = ilog2(btp);
     }
     s->any_coul = false;
