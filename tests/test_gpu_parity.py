@@ -129,6 +129,60 @@ def test_one_lane_build_wide_box_matches_oracle(rumd):
     s.close()
 
 
+def _sampled_check(rumd, s, wl, nsample, seed):
+    """List rows, forces and energies of sampled particles against the oracle run on the cluster of all particles
+    within rc_max + skin + 0.2 of the sample (it contains every interaction partner of the sample)."""
+    N = wl.N
+    r64 = wl.r.astype(np.float64)
+    box = wl.box.astype(np.float64)
+    cnt, lst = s.export_nblist()
+    ids = s.d_id.cpu().numpy().astype(np.int64)
+    slot_of = np.empty(N, np.int64)
+    slot_of[ids] = np.arange(N)
+    st = s.state()
+    skin = float(s.get_tuning().skin)
+    rcm = wl.rc_max()
+    rmsF = np.sqrt((st["F"].astype(np.float64) ** 2).sum(1).mean())
+    for i in np.random.default_rng(seed).choice(N, nsample, replace=False):
+        d = r64 - r64[i]
+        d -= box * np.rint(d / box)
+        near = np.flatnonzero((d * d).sum(1) < (rcm + skin + 0.2) ** 2)
+        sub = np.concatenate(([i], near[near != i]))
+        F, u, w = oracle.forces_allpairs(r64[sub], wl.types[sub], box, wl.pot)
+        oc, ol = oracle.nblist(r64[sub], wl.types[sub], box, wl.pot, skin, method="n2")
+        want = set(sub[ol[0, :oc[0]]].tolist())
+        row = slot_of[i]
+        got = set(ids[lst[row, :cnt[row]]].tolist())
+        for j in want ^ got:
+            dj = r64[j] - r64[i]
+            dj -= box * np.rint(dj / box)
+            rcl = max(wl.pot[wl.types[i], wl.types[j], 2], wl.pot[wl.types[i], wl.types[j], 4]) + skin
+            assert abs(np.sqrt((dj * dj).sum()) - rcl) <= BAND
+        assert np.sqrt(((st["F"][i] - F[0]) ** 2).sum()) <= FORCE_TOL * rmsF
+        assert abs(st["u"][i] - u[0]) <= 1e-5 * max(1.0, abs(u[0]))
+        assert abs(st["w"][i] - w[0]) <= 1e-5 * max(1.0, abs(w[0]))
+    return cnt, st
+
+
+@pytest.mark.parametrize("kind,kw", [("ch", dict(n=32)), ("ka", dict(N=131072))])
+def test_full_size_configs_sampled_against_oracle(rumd, kind, kw):
+    """configs[4] (charged, N = 32768, ~170 list entries) and the largest configs[2] entry (KA N = 131072) at full
+    size with the library's default tuning for that N, after 40 time steps from the perturbed lattice (so the
+    list has been rebuilt and the particles re-sorted in flight): sampled rows against the oracle."""
+    wl = perturbed(make(kind, **kw))
+    s = rumd.from_workload(wl)
+    s.run_steps(40)
+    s.build_nblist()                      # list of the CURRENT positions (the one in flight is a few steps old)
+    s.compute_forces()
+    st0 = s.state()
+    wl.r = st0["r"]                       # the oracle sees the positions the GPU now holds (fp32 values)
+    cnt, st = _sampled_check(rumd, s, wl, 48, 11)
+    assert s.get_thermo()["n_rebuilds"] >= 2 and cnt.sum() % 2 == 0
+    Fsum = st["F"].astype(np.float64).sum(0)
+    assert np.abs(Fsum).max() <= 1e-3 * np.abs(st["F"]).sum()
+    s.close()
+
+
 def test_full_size_million_particles_sampled_against_oracle(rumd):
     """configs[3] at full size (N = 1 048 576) in the configuration bench.py times (autotuned defaults): list
     rows and forces of 64 sampled particles against the oracle, each computed on the cluster of all particles
