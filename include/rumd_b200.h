@@ -47,10 +47,15 @@ typedef enum {
 typedef enum { RUMD_POT_LJ_12_6 = 0, RUMD_POT_COULOMB = 1 } rumd_pot_kind;
 typedef enum { RUMD_CUT_SHIFTED_FORCE = 0 } rumd_cutoff; /* P:73-75; the only method on the hot path */
 typedef enum { RUMD_INT_NVE_LEAPFROG = 0, RUMD_INT_NVT_NOSE_HOOVER = 1 } rumd_integrator;
-typedef enum { RUMD_NB_N2 = 0, RUMD_NB_CELL = 1 } rumd_nb_method; /* P:173 "n2", "sort" */
+typedef enum {
+    RUMD_NB_N2 = 0,   /* P:173 "n2": tiled all-pairs list build */
+    RUMD_NB_CELL = 1, /* P:276 "sort": spatial sort + cell-list build */
+    RUMD_NB_NONE = 2  /* P:371 "none": no list at all, every force evaluation loops over all pairs (small N) */
+} rumd_nb_method;
 
 /* Tunable launch parameters (Table 2: NB method, pb, tp, skin; P:379 sort interval).
- *   method        neighbour-list build algorithm.
+ *   method        neighbour-list build algorithm, or RUMD_NB_NONE (no list: all-pairs forces; skin, build_tp,
+ *                 sort_interval are then unused and rumd_export_nblist reports empty rows).
  *   pb            particles per thread block of the force kernel (Table 1 "PPerBlock").
  *   tp            threads per particle of the force kernel, one of 1,2,4,8,16,32 ("TPerPart").
  *                 pb*tp must be a multiple of 32 and <= 1024.

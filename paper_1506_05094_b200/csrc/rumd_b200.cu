@@ -379,7 +379,8 @@ static bool valid_tp(int tp) { return tp == 1 || tp == 2 || tp == 4 || tp == 8 |
 extern "C" rumd_status rumd_set_tuning(rumd_system* s, const rumd_tuning* t)
 {
     if (!s || !t) return RUMD_ERR_INVALID_ARG;
-    if (t->method != RUMD_NB_N2 && t->method != RUMD_NB_CELL) return fail(s, RUMD_ERR_INVALID_ARG, "bad method");
+    if (t->method != RUMD_NB_N2 && t->method != RUMD_NB_CELL && t->method != RUMD_NB_NONE)
+        return fail(s, RUMD_ERR_INVALID_ARG, "bad method");
     if (!valid_tp(t->tp)) return fail(s, RUMD_ERR_INVALID_ARG, "tp must be 1,2,4,8,16 or 32");
     if (t->pb < 1 || (t->pb * t->tp) % 32 || t->pb * t->tp > 1024) return fail(s, RUMD_ERR_INVALID_ARG, "pb*tp must be a multiple of 32 and <= 1024");
     if (!(t->skin > 0.f) || !std::isfinite(t->skin)) return fail(s, RUMD_ERR_INVALID_ARG, "skin must be > 0");
@@ -601,6 +602,7 @@ static int launch_rebuild_chain(rumd_system* s)
 {
     const Sys& S = s->S;
     int n = 0;
+    if (s->tune.method == RUMD_NB_NONE) return 0; // no list to rebuild
     const bool sorting = s->tune.method == RUMD_NB_CELL || s->tune.sort_interval > 0;
     // Every phase strides over its items, so the grids are capped at a few blocks per SM: on the (many) steps
     // without a rebuild each kernel only reads the flag and exits, and that costs time per BLOCK.
@@ -1061,6 +1063,7 @@ extern "C" rumd_status rumd_autotune(rumd_system* s, rumd_tuning* out, int steps
     rumd_tuning best = saved;
     double best_tps = 0.0;
     std::vector<int> methods;
+    if (s->N <= 5000) methods.push_back(RUMD_NB_NONE); // "none" is not tried above 5000 particles
     if (s->N <= 20000) methods.push_back(RUMD_NB_N2); // n2 is not tried for large systems
     methods.push_back(RUMD_NB_CELL);
     for (int method : methods) {

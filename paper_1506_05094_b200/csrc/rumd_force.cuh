@@ -159,6 +159,73 @@ __device__ __forceinline__ void force_group(const Sys& S, const float4* r, const
     }
 }
 
+// P:371 "none" method: no neighbour list, lane t of the particle's TP lanes takes particles j = t, t + TP, ...
+// of the WHOLE system (coalesced position loads), exact minimum image for every pair, self pair masked.  O(N^2)
+// pair evaluations per step, but no list, no rebuilds and no index stream: wins for the smallest systems.
+template <int TP, bool COUL, bool ONE_TYPE, bool NC, bool ENERGY>
+__device__ __forceinline__ void force_group_all(const Sys& S, const float4* r, const float4* s_pp, int i, int t,
+                                                bool have_i, const float4 ri, float& fx, float& fy, float& fz,
+                                                float& u, float& w)
+{
+    const int trow = ONE_TYPE ? 0 : 4 * type_of(ri) * S.ntypes;
+    float4 pf, pc, pe;
+    pc = pe = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (ONE_TYPE) {
+        pf = s_pp[0];
+        if (COUL) pc = s_pp[1];
+        if (ENERGY) pe = s_pp[2];
+    }
+    fx = fy = fz = u = w = 0.f;
+    const float hx = S.h[0], hy = S.h[1], hz = S.h[2];
+    const float ix = S.invL[0], iy = S.invL[1], iz = S.invL[2];
+    constexpr int U = 4;
+    for (int j0 = t; j0 < S.N; j0 += U * TP) {
+        float4 rj[U];
+        bool ok[U];
+#pragma unroll
+        for (int q = 0; q < U; ++q) {
+            const int j = j0 + q * TP;
+            ok[q] = have_i && j < S.N && j != i;
+            rj[q] = load_pos<NC>(&r[j < S.N ? j : 0]);
+        }
+#pragma unroll
+        for (int q = 0; q < U; ++q) {
+            const float dx = min_image(ri.x, rj[q].x, hx, ix);
+            const float dy = min_image(ri.y, rj[q].y, hy, iy);
+            const float dz = min_image(ri.z, rj[q].z, hz, iz);
+            if (!ONE_TYPE) {
+                const int o = trow + 4 * type_of(rj[q]);
+                pf = s_pp[o];
+                if (COUL) pc = s_pp[o + 1];
+                if (ENERGY) pe = s_pp[o + 2];
+            }
+            pair_accumulate<COUL, ENERGY>(pf, pc, pe, ok[q], dx, dy, dz, fx, fy, fz, u, w);
+        }
+    }
+#pragma unroll
+    for (int o = TP / 2; o; o >>= 1) {
+        fx += __shfl_xor_sync(FULLMASK, fx, o);
+        fy += __shfl_xor_sync(FULLMASK, fy, o);
+        fz += __shfl_xor_sync(FULLMASK, fz, o);
+        if (ENERGY) {
+            u += __shfl_xor_sync(FULLMASK, u, o);
+            w += __shfl_xor_sync(FULLMASK, w, o);
+        }
+    }
+}
+
+// forces of one particle by whichever method is configured (warp-uniform choice)
+template <int TP, bool COUL, bool ONE_TYPE, int UNROLL, bool NC, bool ENERGY>
+__device__ __forceinline__ void force_any(const Sys& S, const float4* r, const float4* s_pp, int vwarp, int i, int t,
+                                          bool have_i, const float4 ri, int cnt, float& fx, float& fy, float& fz,
+                                          float& u, float& w)
+{
+    if (S.method == 2)
+        force_group_all<TP, COUL, ONE_TYPE, NC, ENERGY>(S, r, s_pp, i, t, have_i, ri, fx, fy, fz, u, w);
+    else
+        force_group<TP, COUL, ONE_TYPE, UNROLL, NC, ENERGY>(S, r, s_pp, vwarp, i, t, have_i, ri, cnt, fx, fy, fz, u, w);
+}
+
 // the pair table in shared memory: record of the ordered pair (a, b) at 4*(a*ntypes + b) (four float4)
 __device__ __forceinline__ void load_pair_table(const Sys& S, float4* s_pp)
 {
@@ -171,8 +238,10 @@ __device__ __forceinline__ void load_pair_table(const Sys& S, float4* s_pp)
 __device__ __forceinline__ void finish_rebuild(const Sys& S)
 {
     if (S.sc->flag != 0u) {
-        S.sc->n_rebuilds += 1;
-        S.sc->max_nbrs[S.sc->n_rebuilds & 1] = 0;
+        if (S.method != 2) { // (the "none" method has no list: nothing was built)
+            S.sc->n_rebuilds += 1;
+            S.sc->max_nbrs[S.sc->n_rebuilds & 1] = 0;
+        }
         S.sc->flag = 0u;
     }
 }
@@ -192,10 +261,10 @@ __global__ void __launch_bounds__(1024, 1) k_force(const Sys S)
     int cnt = 0;
     if (have_i) {
         ri = __ldg(&S.r[i]);
-        cnt = S.num_nbrs[i];
+        cnt = S.method == 2 ? 0 : S.num_nbrs[i];
     }
     float fx, fy, fz, u, w;
-    force_group<TP, COUL, ONE_TYPE, UNROLL, true, true>(S, S.r, s_pp, tid >> 5, i, t, have_i, ri, cnt, fx, fy, fz, u, w);
+    force_any<TP, COUL, ONE_TYPE, UNROLL, true, true>(S, S.r, s_pp, tid >> 5, i, t, have_i, ri, cnt, fx, fy, fz, u, w);
     if (have_i && t == 0) {
         S.f[i] = make_float4(fx, fy, fz, 0.5f * u); // P:160 "compensate for double counting"
         S.w[i] = 0.5f * w;
@@ -368,10 +437,10 @@ __global__ void __launch_bounds__(1024, 1) k_step(const Sys S, int nvt)
     int cnt = 0;
     if (have_i) {
         ri = __ldg(&S.r[i]);
-        cnt = S.num_nbrs[i];
+        cnt = S.method == 2 ? 0 : S.num_nbrs[i];
     }
     float fx, fy, fz, u, w;
-    force_group<TP, COUL, ONE_TYPE, UNROLL, true, ENERGY>(S, S.r, s_pp, tid >> 5, i, t, have_i, ri, cnt, fx, fy, fz, u, w);
+    force_any<TP, COUL, ONE_TYPE, UNROLL, true, ENERGY>(S, S.r, s_pp, tid >> 5, i, t, have_i, ri, cnt, fx, fy, fz, u, w);
     double kt = 0.0, mv2 = 0.0;
     bool moved = false;
     if (have_i && t == 0) {
@@ -441,7 +510,7 @@ __global__ void __launch_bounds__(1024) k_thermo(const Sys S)
 __global__ void k_export_nbl(const Sys S, int* count, int* list, int rowcap)
 {
     const int i = blockIdx.x;
-    const int c = S.num_nbrs[i];
+    const int c = S.method == 2 ? 0 : S.num_nbrs[i]; // the "none" method keeps no list
     if (threadIdx.x == 0) count[i] = c;
     for (int k = threadIdx.x; k < rowcap; k += blockDim.x)
         list[(size_t)i * rowcap + k] = k < c ? S.nbl[nbl_index(S, i, k)] : -1;

@@ -49,13 +49,13 @@ __device__ __forceinline__ double warp_sum(double x)
 
 // true iff this launch has rebuild work to do (the build kernel is "called at every timestep and
 // checks ... whether there is anything to be done").
-__device__ __forceinline__ bool rebuild_requested(const Sys& S) { return S.sc->flag != 0u; }
+__device__ __forceinline__ bool rebuild_requested(const Sys& S) { return S.sc->flag != 0u && S.method != 2; }
 
 // sort on this rebuild?  cell method: always; n2 method: every sort_interval-th rebuild.
 __device__ __forceinline__ bool sort_on_rebuild(const Sys& S, long long n_rebuilds)
 {
     if (S.method == 1) return true;
-    return S.sort_interval > 0 && (n_rebuilds % S.sort_interval) == 0;
+    return S.method == 0 && S.sort_interval > 0 && (n_rebuilds % S.sort_interval) == 0;
 }
 __device__ __forceinline__ bool sort_requested(const Sys& S)
 {

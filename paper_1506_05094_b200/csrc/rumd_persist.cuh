@@ -139,7 +139,7 @@ __global__ void __launch_bounds__(PERSIST_THREADS, PERSIST_MINB) k_persist(const
     for (int k = 0; k < nsteps; ++k) {
         if (prof) s_prof[4] = clock64();
         // ---------------------------------------------------------------- (rebuild if flag) A2 / A3 / A4
-        if (flag) {
+        if (flag && S.method != 2) { // (the "none" method keeps no list)
             int* max_slot = &sc->max_nbrs[n_rebuilds & 1];
             if (blockIdx.x == 0 && threadIdx.x == 0) sc->max_nbrs[(n_rebuilds + 1) & 1] = 0;
             if (sort_on_rebuild(S, n_rebuilds)) {
@@ -213,13 +213,13 @@ __global__ void __launch_bounds__(PERSIST_THREADS, PERSIST_MINB) k_persist(const
             int cnt = 0;
             if (have_i) {
                 ri = rc[i];
-                cnt = S.num_nbrs[i];
+                cnt = S.method == 2 ? 0 : S.num_nbrs[i];
             }
             float fx, fy, fz, u, w;
             if (last) // energies and virials are outputs of the LAST force evaluation only
-                force_group<TP, COUL, ONE_TYPE, UNROLL, false, true>(S, rc, s_pp, (int)vw, i, t, have_i, ri, cnt, fx, fy, fz, u, w);
+                force_any<TP, COUL, ONE_TYPE, UNROLL, false, true>(S, rc, s_pp, (int)vw, i, t, have_i, ri, cnt, fx, fy, fz, u, w);
             else
-                force_group<TP, COUL, ONE_TYPE, UNROLL, false, false>(S, rc, s_pp, (int)vw, i, t, have_i, ri, cnt, fx, fy, fz, u, w);
+                force_any<TP, COUL, ONE_TYPE, UNROLL, false, false>(S, rc, s_pp, (int)vw, i, t, have_i, ri, cnt, fx, fy, fz, u, w);
             if (have_i && t == 0) {
                 while (*((volatile int*)&s_ab_step) <= k) {} // factors of step k published? (warp 0, above)
                 __threadfence_block();

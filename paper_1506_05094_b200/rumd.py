@@ -20,7 +20,7 @@ OK, ERR_INVALID_ARG, ERR_NOT_READY, ERR_CUDA, ERR_NBL_OVERFLOW, ERR_BOX_TOO_SMAL
 POT_LJ_12_6, POT_COULOMB = 0, 1
 CUT_SHIFTED_FORCE = 0
 INT_NVE_LEAPFROG, INT_NVT_NOSE_HOOVER = 0, 1
-NB_N2, NB_CELL = 0, 1
+NB_N2, NB_CELL, NB_NONE = 0, 1, 2
 
 EXPORTS = [
     "rumd_create", "rumd_destroy", "rumd_bind_state", "rumd_workspace_bytes", "rumd_bind_workspace",

@@ -402,6 +402,34 @@ def test_overflow_is_reported_and_capacity_doubles(rumd):
     s.close()
 
 
+@pytest.mark.parametrize("kind,kw,tp,persistent", [("lj", dict(ncell=4), 32, 1), ("ka", dict(N=512), 16, 1),
+                                                   ("ch", dict(n=8), 8, 0), ("ka", dict(N=1000), 4, 1)])
+def test_none_method_all_pairs_forces(rumd, kind, kw, tp, persistent):
+    """P:371 "none": no neighbour list, every force evaluation visits all pairs.  Forces / energies / virials
+    against the oracle's brute force, and the same trajectory as the list-based path (to fp32 summation order)."""
+    wl = perturbed(make(kind, **kw))
+    s = rumd.from_workload(wl)
+    s.set_tuning(method=rumd.NB_NONE, tp=tp, pb=max(1, 128 // tp), persistent=persistent, use_graph=0)
+    s.compute_forces()
+    check_forces(s, wl.r.astype(np.float64), wl.types, wl.box.astype(np.float64), wl.pot)
+    cnt, _ = s.export_nblist()
+    assert cnt.sum() == 0
+    s.run_steps(25)
+    a = s.state()
+    th = s.get_thermo()
+    assert th["n_steps"] == 25 and th["n_rebuilds"] == 0
+    s.close()
+    s2 = rumd.from_workload(wl)
+    s2.set_tuning(method=rumd.NB_N2, tp=tp, pb=max(1, 128 // tp), persistent=persistent, use_graph=0)
+    s2.run_steps(25)
+    b = s2.state()
+    s2.close()
+    d = a["r"].astype(np.float64) - b["r"]
+    box = wl.box.astype(np.float64)
+    d -= box * np.rint(d / box)
+    assert np.abs(d).max() < 1e-4 and np.abs(a["v"] - b["v"]).max() < 2e-3
+
+
 def _gas(N, ntypes, box, seed, pot):
     r, types = W.random_gas(N, ntypes, box, seed)
     rng = np.random.default_rng(seed + 1)
