@@ -56,7 +56,7 @@ typedef enum {
 /* Tunable launch parameters (Table 2: NB method, pb, tp, skin; P:379 sort interval).
  *   method        neighbour-list build algorithm, or RUMD_NB_NONE (no list: all-pairs forces; skin, build_tp,
  *                 sort_interval are then unused and rumd_export_nblist reports empty rows).
- *   pb            particles per thread block of the force kernel (Table 1 "PPerBlock").
+ *   pb            particles per thread block of the per-step force kernel (Table 1 "PPerBlock").
  *   tp            threads per particle of the force kernel, one of 1,2,4,8,16,32 ("TPerPart").
  *                 pb*tp must be a multiple of 32 and <= 1024.
  *   skin          Verlet skin; list cutoff of a type pair = rc_ab + skin (S4).
@@ -66,9 +66,9 @@ typedef enum {
  *                 graphs (steps_per_graph steps each).
  *   steps_per_graph  time steps unrolled into one graph launch (>= 1; 0 = library default).
  *   persistent    1: rumd_run_steps(n) is ONE cooperative kernel that runs all n steps (fused force +
- *                 integrate, double-buffered positions, grid barrier per step, in-kernel rebuilds);
- *                 0: per-step kernels (early-exit rebuild chain, force, integrate).  pb*tp (rounded to
- *                 256..1024) is the block size of the persistent kernel.
+ *                 integrate, double-buffered positions, grid barrier per step, in-kernel rebuilds; blocks of
+ *                 256 threads, pb is not used); 0: per-step kernels (early-exit rebuild chain, then force +
+ *                 integrate, fused into one kernel per step inside CUDA graphs).
  *   build_tp      lanes per particle of the cell-list build, one of 1,2,4,8,16,32 ("not been tried
  *                 yet"); 0 = library default for this N. */
 typedef struct {

@@ -44,8 +44,7 @@ struct rumd_system {
     int4* snap_image = nullptr;
     int* snap_id = nullptr;
     DevScalars* snap_sc = nullptr;
-    std::vector<int> zrank_host; // for the current grid
-    int grid_for[3] = {0, 0, 0};
+    int grid_for[3] = {0, 0, 0}; // cell grid the device rowrank table was built for
     GraphCache graph_multi, graph_one;
     rumd_thermo* h_thermo = nullptr; // pinned
     DevScalars* h_sc = nullptr;      // pinned
