@@ -45,7 +45,11 @@ typedef enum {
 } rumd_status;
 
 typedef enum { RUMD_POT_LJ_12_6 = 0, RUMD_POT_COULOMB = 1 } rumd_pot_kind;
-typedef enum { RUMD_CUT_SHIFTED_FORCE = 0 } rumd_cutoff; /* P:73-75; the only method on the hot path */
+typedef enum { /* P:73-75 "the cutoff methods: no shift, shifted potential and shifted force" */
+    RUMD_CUT_SHIFTED_FORCE = 0,     /* f = f(r) - f(rc), u = u(r) - u(rc) + (r - rc) f(rc): the hot-path default */
+    RUMD_CUT_SHIFTED_POTENTIAL = 1, /* f = f(r),         u = u(r) - u(rc) */
+    RUMD_CUT_NONE = 2               /* f = f(r),         u = u(r)  (plain truncation) */
+} rumd_cutoff;
 typedef enum { RUMD_INT_NVE_LEAPFROG = 0, RUMD_INT_NVT_NOSE_HOOVER = 1 } rumd_integrator;
 typedef enum {
     RUMD_NB_N2 = 0,   /* P:173 "n2": tiled all-pairs list build */
@@ -128,9 +132,9 @@ rumd_status rumd_bind_workspace(rumd_system* s, void* d_ws, size_t bytes, int nb
 /* P:49-50 `pot.SetParams(i, j, Sigma, Epsilon, Rcut)`; symmetric in (type_i, type_j).  params: host.
  *   RUMD_POT_LJ_12_6 : {epsilon, sigma, rcut}   u = 4 eps [(s/r)^12 - (s/r)^6]           (O3)
  *   RUMD_POT_COULOMB : {k*q_i*q_j, rcut}        u = k q_i q_j / r, no self term          (O4, S6)
- * rcut is an ABSOLUTE distance (S2).  Shifted-force cutoff: f_SF = f(r) - f(rc),
- * u_SF = u(r) - u(rc) + (r - rc) f(rc) for r < rc, else 0.  One slot per kind per type pair: the same
- * kind again overwrites, different kinds add, each with its own rc (S5).  rcut <= 0 removes the term. */
+ * rcut is an ABSOLUTE distance (S2).  cutoff: one of rumd_cutoff, applied for r < rcut, zero beyond (S3).
+ * One slot per kind per type pair: the same kind again overwrites, different kinds add, each with its own
+ * rc and cutoff method (S5).  rcut <= 0 removes the term. */
 rumd_status rumd_set_pair_potential(rumd_system* s, int type_i, int type_j, rumd_pot_kind kind,
                                     rumd_cutoff cutoff, const float* params, int n_params);
 

@@ -9,7 +9,8 @@ arrays.  See the header of ``rumd_oracle.c`` for the list of pins.
 
 Array conventions: positions / velocities / forces are float64 ``(N, 3)``; types int32 ``(N,)``;
 box float64 ``(3,)``; potentials float64 ``(ntypes, ntypes, 5)`` with records
-``(epsilon, sigma, rc_LJ, k*qa*qb, rc_Coulomb)`` (an rc <= 0 disables that term).
+``(epsilon, sigma, rc_LJ, k*qa*qb, rc_Coulomb, cut_LJ, cut_Coulomb)`` (an rc <= 0 disables that term;
+cut = 0 shifted force, 1 shifted potential, 2 no shift).
 """
 from __future__ import annotations
 
@@ -24,7 +25,7 @@ _SRC = os.path.join(_HERE, "rumd_oracle.c")
 _LIB = os.path.join(_HERE, "librumd_oracle.so")
 
 NVE, NVT = 0, 1
-POT_STRIDE = 5
+POT_STRIDE = 7
 
 
 def build(force: bool = False) -> str:
@@ -52,6 +53,8 @@ def lib():
         L.orc_lj_raw.argtypes = [C.c_double] * 3 + [_dp, _dp]
         L.orc_lj_sf.argtypes = [C.c_double] * 4 + [_dp, _dp]
         L.orc_coulomb_sf.argtypes = [C.c_double] * 3 + [_dp, _dp]
+        L.orc_lj_cut.argtypes = [C.c_double] * 4 + [C.c_int, _dp, _dp]
+        L.orc_coulomb_cut.argtypes = [C.c_double] * 3 + [C.c_int, _dp, _dp]
         L.orc_pair_sf.argtypes = [_dp, C.c_double, _dp, _dp]
         L.orc_pair_rc.argtypes = [_dp]
         L.orc_pair_rc.restype = C.c_double
@@ -116,6 +119,15 @@ def lj_sf(r, eps, sig, rc):
 
 def coulomb_sf(r, qq, rc):
     return _pair(lib().orc_coulomb_sf, float(r), float(qq), float(rc))
+
+
+def lj_cut(r, eps, sig, rc, method):
+    """(u, f) of LJ 12-6 with cutoff method 0 = shifted force, 1 = shifted potential, 2 = no shift."""
+    return _pair(lib().orc_lj_cut, float(r), float(eps), float(sig), float(rc), int(method))
+
+
+def coulomb_cut(r, qq, rc, method):
+    return _pair(lib().orc_coulomb_cut, float(r), float(qq), float(rc), int(method))
 
 
 def pair_sf(rec, r):

@@ -29,6 +29,8 @@
  * orthorhombic, origin-centred, coordinates in [-L/2, L/2] (S7).  Potentials are one record of
  * ORC_POT_STRIDE doubles per ORDERED type pair (a*ntypes+b):
  *     pot[0]=epsilon pot[1]=sigma pot[2]=rc_LJ (<=0: no LJ term) pot[3]=k*qa*qb pot[4]=rc_Coulomb (<=0: none)
+ *     pot[5]=cutoff method of the LJ term, pot[6]=cutoff method of the Coulomb term:
+ *            0 = shifted force, 1 = shifted potential, 2 = no shift (plain truncation)
  * rc values are ABSOLUTE distances (S2).
  */
 #include <math.h>
@@ -38,7 +40,7 @@
 #include <omp.h>
 #endif
 
-#define ORC_POT_STRIDE 5
+#define ORC_POT_STRIDE 7
 
 int orc_num_threads(void)
 {
@@ -104,17 +106,54 @@ void orc_coulomb_sf(double r, double qq, double rc, double *u, double *f)
     }
 }
 
-/* S5: terms of different kinds on one type pair add; each applies its own rc. */
+/* P:73-75 "the cutoff methods: no shift, shifted potential and shifted force" applied to a raw pair
+ * function value (ur, fr) at r given its value (uc, fc) at the cutoff; zero at and beyond rc (S3):
+ *   shifted force     : u = ur - uc + (r - rc) fc,  f = fr - fc   (continuous force, linear term in u)
+ *   shifted potential : u = ur - uc,                f = fr        (continuous energy, force jumps by fc at rc)
+ *   no shift          : u = ur,                     f = fr        (both jump at rc)                      */
+void orc_apply_cutoff(int method, double r, double rc, double ur, double fr, double uc, double fc, double *u,
+                      double *f)
+{
+    if (!(r < rc)) {
+        *u = 0.0;
+        *f = 0.0;
+    } else if (method == 0) {
+        *u = ur - uc + (r - rc) * fc;
+        *f = fr - fc;
+    } else if (method == 1) {
+        *u = ur - uc;
+        *f = fr;
+    } else {
+        *u = ur;
+        *f = fr;
+    }
+}
+
+/* LJ 12-6 / Coulomb with any of the three cutoff methods */
+void orc_lj_cut(double r, double eps, double sig, double rc, int method, double *u, double *f)
+{
+    double ur, fr, uc, fc;
+    orc_lj_raw(r, eps, sig, &ur, &fr);
+    orc_lj_raw(rc, eps, sig, &uc, &fc);
+    orc_apply_cutoff(method, r, rc, ur, fr, uc, fc, u, f);
+}
+
+void orc_coulomb_cut(double r, double qq, double rc, int method, double *u, double *f)
+{
+    orc_apply_cutoff(method, r, rc, qq / r, qq / (r * r), qq / rc, qq / (rc * rc), u, f);
+}
+
+/* S5: terms of different kinds on one type pair add; each applies its own rc and its own cutoff method. */
 void orc_pair_sf(const double *p, double r, double *u, double *f)
 {
     double ut = 0.0, ft = 0.0, uu, ff;
     if (p[2] > 0.0) {
-        orc_lj_sf(r, p[0], p[1], p[2], &uu, &ff);
+        orc_lj_cut(r, p[0], p[1], p[2], (int)p[5], &uu, &ff);
         ut += uu;
         ft += ff;
     }
     if (p[4] > 0.0) {
-        orc_coulomb_sf(r, p[3], p[4], &uu, &ff);
+        orc_coulomb_cut(r, p[3], p[4], (int)p[6], &uu, &ff);
         ut += uu;
         ft += ff;
     }

@@ -14,6 +14,7 @@
 struct PotSlot {
     bool lj = false, coul = false;
     double eps = 0, sig = 0, rc_lj = 0, qq = 0, rc_c = 0;
+    int cut_lj = 0, cut_c = 0; // rumd_cutoff of each term
 };
 
 struct GraphCache {
@@ -316,7 +317,8 @@ extern "C" rumd_status rumd_set_pair_potential(rumd_system* s, int ti, int tj, r
 {
     if (!s || !params) return RUMD_ERR_INVALID_ARG;
     if (ti < 0 || tj < 0 || ti >= s->ntypes || tj >= s->ntypes) return fail(s, RUMD_ERR_INVALID_ARG, "type out of range");
-    if (cutoff != RUMD_CUT_SHIFTED_FORCE) return fail(s, RUMD_ERR_INVALID_ARG, "only the shifted-force cutoff is implemented");
+    if (cutoff != RUMD_CUT_SHIFTED_FORCE && cutoff != RUMD_CUT_SHIFTED_POTENTIAL && cutoff != RUMD_CUT_NONE)
+        return fail(s, RUMD_ERR_INVALID_ARG, "unknown cutoff method");
     for (int q = 0; q < n_params; ++q)
         if (!std::isfinite(params[q])) return fail(s, RUMD_ERR_INVALID_ARG, "non-finite parameter");
     for (int pass = 0; pass < 2; ++pass) {
@@ -327,12 +329,14 @@ extern "C" rumd_status rumd_set_pair_potential(rumd_system* s, int ti, int tj, r
             p.eps = params[0];
             p.sig = params[1];
             p.rc_lj = params[2];
+            p.cut_lj = (int)cutoff;
             if (p.lj && !(p.sig > 0)) return fail(s, RUMD_ERR_INVALID_ARG, "sigma must be > 0");
         } else if (kind == RUMD_POT_COULOMB) {
             if (n_params != 2) return fail(s, RUMD_ERR_INVALID_ARG, "Coulomb takes {k*qi*qj, rcut}");
             p.coul = params[1] > 0.f;
             p.qq = params[0];
             p.rc_c = params[1];
+            p.cut_c = (int)cutoff;
         } else
             return fail(s, RUMD_ERR_INVALID_ARG, "unknown potential kind");
     }
@@ -455,8 +459,10 @@ static rumd_status refresh(rumd_system* s)
             if (p.lj) {
                 const double s6 = std::pow(p.sig, 6), c6 = 4 * p.eps * s6, c12 = c6 * s6;
                 const double ri6 = std::pow(p.rc_lj, -6);
-                const double uc = c12 * ri6 * ri6 - c6 * ri6;
-                const double fc = (12 * c12 * ri6 * ri6 - 6 * c6 * ri6) / p.rc_lj;
+                // the kernel evaluates u = u(r) + fc r - k0 and f = f(r) - fc: shifted force fc = f(rc),
+                // k0 = u(rc) + rc fc; shifted potential fc = 0, k0 = u(rc); no shift fc = k0 = 0
+                const double uc = p.cut_lj == RUMD_CUT_NONE ? 0.0 : c12 * ri6 * ri6 - c6 * ri6;
+                const double fc = p.cut_lj == RUMD_CUT_SHIFTED_FORCE ? (12 * c12 * ri6 * ri6 - 6 * c6 * ri6) / p.rc_lj : 0.0;
                 q.c12 = (float)c12;
                 q.c6 = (float)c6;
                 q.c12x12 = (float)(12.0 * c12);
@@ -469,8 +475,10 @@ static rumd_status refresh(rumd_system* s)
             if (p.coul) {
                 q.qq = (float)p.qq;
                 q.rc2_c = (float)(p.rc_c * p.rc_c);
-                q.fc_c = (float)(p.qq / (p.rc_c * p.rc_c));
-                q.k0_c = (float)(2.0 * p.qq / p.rc_c);
+                const double ucc = p.cut_c == RUMD_CUT_NONE ? 0.0 : p.qq / p.rc_c;
+                const double fcc = p.cut_c == RUMD_CUT_SHIFTED_FORCE ? p.qq / (p.rc_c * p.rc_c) : 0.0;
+                q.fc_c = (float)fcc;
+                q.k0_c = (float)(ucc + p.rc_c * fcc);
                 rc = std::max(rc, p.rc_c);
                 s->any_coul = true;
             }

@@ -18,7 +18,7 @@ _LIBPATH = os.environ.get("RUMD_B200_LIB") or os.path.join(_HERE, "librumd_b200.
 
 OK, ERR_INVALID_ARG, ERR_NOT_READY, ERR_CUDA, ERR_NBL_OVERFLOW, ERR_BOX_TOO_SMALL, ERR_NONFINITE = range(7)
 POT_LJ_12_6, POT_COULOMB = 0, 1
-CUT_SHIFTED_FORCE = 0
+CUT_SHIFTED_FORCE, CUT_SHIFTED_POTENTIAL, CUT_NONE = 0, 1, 2
 INT_NVE_LEAPFROG, INT_NVT_NOSE_HOOVER = 0, 1
 NB_N2, NB_CELL, NB_NONE = 0, 1, 2
 
@@ -150,15 +150,16 @@ class System:
         self._check(self.L.rumd_bind_state(self.h, *[C.c_void_p(t.data_ptr()) for t in
                                                     (self.d_r, self.d_v, self.d_f, self.d_w, self.d_image,
                                                      self.d_id)]))
-        # potentials (P:49-50 SetParams); pot records are (eps, sigma, rc_LJ, k qa qb, rc_Coulomb)
+        # potentials (P:49-50 SetParams); pot records are (eps, sigma, rc_LJ, k qa qb, rc_Coulomb, cut_LJ, cut_C)
         pot = np.asarray(pot, dtype=np.float64)
         for a in range(self.ntypes):
             for b in range(a, self.ntypes):
-                e, sg, rcl, qq, rcc = pot[a, b]
+                e, sg, rcl, qq, rcc = pot[a, b, :5]
+                cut_lj, cut_c = (int(pot[a, b, 5]), int(pot[a, b, 6])) if pot.shape[-1] >= 7 else (0, 0)
                 if rcl > 0:
-                    self.set_pair_potential(a, b, POT_LJ_12_6, [e, sg, rcl])
+                    self.set_pair_potential(a, b, POT_LJ_12_6, [e, sg, rcl], cut_lj)
                 if rcc > 0:
-                    self.set_pair_potential(a, b, POT_COULOMB, [qq, rcc])
+                    self.set_pair_potential(a, b, POT_COULOMB, [qq, rcc], cut_c)
         self.rc_max = float(max(pot[..., 2].max(), pot[..., 4].max()))
         self.density = N / float(np.prod(self.box.astype(np.float64)))
         if capacity is None:
@@ -193,9 +194,9 @@ class System:
         self.d_ws = ws  # keep the new one alive, drop the old one only now
         self.capacity = capacity
 
-    def set_pair_potential(self, ti, tj, kind, params):
+    def set_pair_potential(self, ti, tj, kind, params, cutoff=CUT_SHIFTED_FORCE):
         arr = (C.c_float * len(params))(*[float(x) for x in params])
-        self._check(self.L.rumd_set_pair_potential(self.h, ti, tj, kind, CUT_SHIFTED_FORCE, arr, len(params)))
+        self._check(self.L.rumd_set_pair_potential(self.h, ti, tj, kind, int(cutoff), arr, len(params)))
 
     def set_integrator(self, kind, dt, T0=1.0, tau=0.2):
         self._check(self.L.rumd_set_integrator(self.h, int(kind), float(dt), float(T0), float(tau)))

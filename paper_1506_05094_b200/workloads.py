@@ -19,7 +19,8 @@ import numpy as np
 SEED0 = 150605094  # + 1000*config + index-in-sweep
 
 NVE, NVT = 0, 1
-POT_STRIDE = 5  # (epsilon, sigma, rc_LJ, k*qa*qb, rc_Coulomb); rc <= 0 disables the term
+POT_STRIDE = 7  # (epsilon, sigma, rc_LJ, k*qa*qb, rc_Coulomb, cut_LJ, cut_Coulomb); rc <= 0 disables the term
+CUT_SHIFTED_FORCE, CUT_SHIFTED_POTENTIAL, CUT_NONE = 0, 1, 2
 
 
 @dataclass
@@ -117,14 +118,14 @@ def pot_table(ntypes: int) -> np.ndarray:
     return np.zeros((ntypes, ntypes, POT_STRIDE), dtype=np.float64)
 
 
-def set_lj(pot, a, b, eps, sig, rc):
+def set_lj(pot, a, b, eps, sig, rc, cut=CUT_SHIFTED_FORCE):
     for i, j in ((a, b), (b, a)):
-        pot[i, j, 0], pot[i, j, 1], pot[i, j, 2] = f32(eps), f32(sig), f32(rc)
+        pot[i, j, 0], pot[i, j, 1], pot[i, j, 2], pot[i, j, 5] = f32(eps), f32(sig), f32(rc), float(cut)
 
 
-def set_coulomb(pot, a, b, qq, rc):
+def set_coulomb(pot, a, b, qq, rc, cut=CUT_SHIFTED_FORCE):
     for i, j in ((a, b), (b, a)):
-        pot[i, j, 3], pot[i, j, 4] = f32(qq), f32(rc)
+        pot[i, j, 3], pot[i, j, 4], pot[i, j, 6] = f32(qq), f32(rc), float(cut)
 
 
 def lj_single() -> np.ndarray:

@@ -430,6 +430,61 @@ def test_none_method_all_pairs_forces(rumd, kind, kw, tp, persistent):
     assert np.abs(d).max() < 1e-4 and np.abs(a["v"] - b["v"]).max() < 2e-3
 
 
+def _with_cutoffs(pot, cut_lj, cut_c):
+    pot = pot.copy()
+    pot[..., 5] = cut_lj
+    pot[..., 6] = cut_c
+    return pot
+
+
+@pytest.mark.parametrize("kind,kw,cut_lj,cut_c,method,tp", [
+    ("ka", dict(N=1000), W.CUT_SHIFTED_POTENTIAL, 0, "n2", 16),
+    ("ka", dict(N=2048), W.CUT_NONE, 0, "cell", 4),
+    ("ch", dict(n=10), W.CUT_SHIFTED_POTENTIAL, W.CUT_NONE, "cell", 8),
+    ("ch", dict(n=12), W.CUT_NONE, W.CUT_SHIFTED_POTENTIAL, "cell", 1),
+    ("lj", dict(ncell=6), W.CUT_SHIFTED_POTENTIAL, 0, "none", 32),
+])
+def test_other_cutoff_methods_match_oracle(rumd, kind, kw, cut_lj, cut_c, method, tp):
+    """shifted potential and plain truncation (next to the hot path's shifted force) on the same
+    kernels.  With these methods the pair force JUMPS at rc (by f(rc) ~ 0.04), so a pair within fp32 rounding
+    of a cutoff may be counted on one side only: particles owning a pair within 1e-6 of one of its cutoffs are
+    left out of the force comparison (S30) -- the analogue of the 1e-6 band of the list."""
+    wl = perturbed(make(kind, **kw))
+    wl.pot = _with_cutoffs(wl.pot, cut_lj, cut_c)
+    s = rumd.from_workload(wl)
+    m = {"n2": rumd.NB_N2, "cell": rumd.NB_CELL, "none": rumd.NB_NONE}[method]
+    s.set_tuning(method=m, tp=tp, pb=max(1, 128 // tp))
+    s.compute_forces()
+    r64, box = wl.r.astype(np.float64), wl.box.astype(np.float64)
+    F, u, w = oracle.forces_allpairs(r64, wl.types, box, wl.pot)
+    d = r64[:, None, :] - r64[None, :, :]
+    d -= box * np.rint(d / box)
+    dist = np.sqrt((d * d).sum(-1))
+    ti, tj = wl.types[:, None], wl.types[None, :]
+    near = np.zeros(dist.shape, bool)
+    for col in (2, 4):
+        rc = wl.pot[ti, tj, col]
+        near |= (rc > 0) & (np.abs(dist - rc) <= BAND)
+    keep = ~near.any(1)
+    assert keep.sum() >= 0.99 * wl.N
+    st = s.state()
+    rms = np.sqrt((F * F).sum(1).mean())
+    err = np.sqrt(((st["F"].astype(np.float64) - F) ** 2).sum(1))
+    assert err[keep].max() <= FORCE_TOL * rms
+    assert np.abs(st["u"] - u)[keep].max() <= 1e-5 * max(1.0, np.abs(u).max())
+    assert np.abs(st["w"] - w)[keep].max() <= 1e-5 * max(1.0, np.abs(w).max())
+    if keep.all():
+        th = s.get_thermo()
+        assert abs(th["U"] - u.sum()) <= ENERGY_TOL * np.abs(u).sum()
+        assert abs(th["W"] - w.sum()) <= ENERGY_TOL * np.abs(w).sum()
+    # the three methods really differ: the energy is not the shifted-force one
+    F0, u0, w0 = oracle.forces_allpairs(r64, wl.types, box, _with_cutoffs(wl.pot, 0, 0))
+    assert abs(u.sum() - u0.sum()) > 1e-3 * np.abs(u0).sum()
+    s.run_steps(20)
+    assert np.isfinite(s.get_thermo()["H"])
+    s.close()
+
+
 def _gas(N, ntypes, box, seed, pot):
     r, types = W.random_gas(N, ntypes, box, seed)
     rng = np.random.default_rng(seed + 1)

@@ -516,3 +516,87 @@ def test_run_is_independent_of_the_search_method_and_skin():
     b = oracle.run(wl.r, wl.v, wl.m, img0, wl.types, wl.box, wl.pot, 0.6, wl.dt, 50, **kw)
     assert np.abs(a["r"] - b["r"]).max() < 1e-9 and a["n_builds"] >= b["n_builds"]
     assert np.abs(a["log"][:, 0] - b["log"][:, 0]).max() < 1e-8 * np.abs(a["log"][:, 0]).max()
+
+
+# ------------------------------------------------------------------ the three cutoff methods
+
+
+def test_cutoff_methods_closed_forms():
+    """shifted force / shifted potential / no shift against the raw pair function they are built from."""
+    eps, sig, rc = 1.5, 0.8, 2.0
+    uc, fc = oracle.lj_raw(rc, eps, sig)
+    for r in (0.75, 0.9, 1.3, 1.99):
+        ur, fr = oracle.lj_raw(r, eps, sig)
+        assert oracle.lj_cut(r, eps, sig, rc, 0) == pytest.approx((ur - uc + (r - rc) * fc, fr - fc), rel=1e-13)
+        assert oracle.lj_cut(r, eps, sig, rc, 0) == pytest.approx(oracle.lj_sf(r, eps, sig, rc), rel=1e-15)
+        assert oracle.lj_cut(r, eps, sig, rc, 1) == pytest.approx((ur - uc, fr), rel=1e-13)
+        assert oracle.lj_cut(r, eps, sig, rc, 2) == pytest.approx((ur, fr), rel=1e-15)
+        qq, rcc = -1.0, 4.0
+        assert oracle.coulomb_cut(r, qq, rcc, 0) == pytest.approx(oracle.coulomb_sf(r, qq, rcc), rel=1e-15)
+        assert oracle.coulomb_cut(r, qq, rcc, 1) == pytest.approx((qq / r - qq / rcc, qq / r ** 2), rel=1e-13)
+        assert oracle.coulomb_cut(r, qq, rcc, 2) == pytest.approx((qq / r, qq / r ** 2), rel=1e-15)
+    for m in (0, 1, 2):
+        assert oracle.lj_cut(rc, eps, sig, rc, m) == (0.0, 0.0) and oracle.lj_cut(rc + 0.3, eps, sig, rc, m) == (0.0, 0.0)
+    # what is continuous at the cutoff: SF both, SP the energy only (the force jumps by f(rc)), none neither
+    below = rc * (1 - 1e-12)
+    assert oracle.lj_cut(below, eps, sig, rc, 0) == pytest.approx((0.0, 0.0), abs=1e-10)
+    u1, f1 = oracle.lj_cut(below, eps, sig, rc, 1)
+    assert abs(u1) < 1e-10 and f1 == pytest.approx(fc, rel=1e-9)
+    assert oracle.lj_cut(below, eps, sig, rc, 2) == pytest.approx((uc, fc), rel=1e-9)
+
+
+@pytest.mark.parametrize("method", [0, 1, 2])
+def test_cutoff_methods_force_is_minus_gradient(method):
+    rec = np.array([1.5, 0.8, 2.0, -1.0, 3.0, method, method])
+    h = 1e-6
+    for r in (0.8, 1.1, 1.7, 1.95, 2.5, 2.9):
+        up, _ = oracle.pair_sf(rec, r + h)
+        um, _ = oracle.pair_sf(rec, r - h)
+        _, f = oracle.pair_sf(rec, r)
+        assert f == pytest.approx(-(up - um) / (2 * h), rel=2e-7)
+
+
+def test_cutoff_methods_fcc_lattice_sums():
+    """Static fcc lattice energies for plain truncation and the shifted potential, by the
+    integer-shell lattice sum and by the particle code; and the exact relations between the three methods:
+    U_SP = U_none - (54/2) u(rc),  U_SF = U_SP + 1/2 sum (r - rc) f(rc)."""
+    a = (4.0 / 0.8442) ** (1.0 / 3.0)
+    r, box = W.fcc_lattice(6, 6, 6, 0.8442)
+    t = np.zeros(len(r), np.int32)
+    res = {}
+    for method, key in ((2, "fcc_u_per_n_noshift"), (1, "fcc_u_per_n_shiftedpot"), (0, "fcc_u_per_n")):
+        pot = W.pot_table(1)
+        W.set_lj(pot, 0, 0, 1.0, 1.0, 2.5, cut=method)
+
+        def vecs():
+            for i, j, k in itertools.product(range(-8, 9), repeat=3):
+                if (i + j + k) % 2 == 0 and (i, j, k) != (0, 0, 0):
+                    yield (i * i + j * j + k * k) / 4.0, pot[0, 0]
+        U, WW, _ = _shell_sum(vecs(), a, [2.5], oracle.pair_sf)
+        assert 0.5 * U == pytest.approx(GOLD[key], rel=2e-10)
+        F, u, w = oracle.forces_allpairs(r, t, box, pot)
+        assert u.sum() / len(r) == pytest.approx(GOLD[key], rel=2e-10)
+        assert np.abs(F).max() < 1e-10
+        res[method] = (u.sum() / len(r), w.sum() / len(r))
+    uc, fc = oracle.lj_raw(2.5, 1.0, 1.0)
+    assert res[1][0] == pytest.approx(res[2][0] - 27 * uc, rel=1e-12)          # 54 neighbours inside rc
+    assert res[1][1] == pytest.approx(res[2][1], rel=1e-12)                    # same forces -> same virial
+    # SF adds (r - rc) f(rc) per pair to u and subtracts r f(rc) from r f
+    shells = [(math.sqrt(0.5) * a, 12), (a, 6), (math.sqrt(1.5) * a, 24), (math.sqrt(2.0) * a, 12)]
+    assert res[0][0] == pytest.approx(res[1][0] + 0.5 * sum(n * (d - 2.5) * fc for d, n in shells), rel=1e-12)
+    assert res[0][1] == pytest.approx(res[1][1] - 0.5 * sum(n * d * fc for d, n in shells), rel=1e-12)
+
+
+def test_cutoff_methods_list_forces_equal_brute_force():
+    pot = W.pot_table(2)
+    W.set_lj(pot, 0, 0, 1.0, 1.0, 2.5, cut=1)
+    W.set_lj(pot, 0, 1, 1.5, 0.8, 2.0, cut=2)
+    W.set_lj(pot, 1, 1, 0.5, 0.88, 2.2, cut=0)
+    W.set_coulomb(pot, 0, 1, -1.0, 3.0, cut=1)
+    r, t = W.random_gas(200, 2, (8.0, 9.0, 10.0), 5)
+    box = np.array([8.0, 9.0, 10.0])
+    F, u, w = oracle.forces_allpairs(r.astype(np.float64), t, box, pot)
+    cnt, lst = oracle.nblist(r.astype(np.float64), t, box, pot, 0.4)
+    F2, u2, w2 = oracle.forces_list(r.astype(np.float64), t, box, pot, cnt, lst)
+    assert np.allclose(F, F2, rtol=1e-12, atol=1e-12) and np.allclose(u, u2, rtol=1e-12) and np.allclose(w, w2, rtol=1e-12)
+    assert np.abs(F.sum(0)).max() < 1e-10 * np.abs(F).sum()
