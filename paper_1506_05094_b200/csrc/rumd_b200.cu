@@ -530,7 +530,9 @@ static rumd_status refresh(rumd_system* s)
 // ---------------------------------------------------------------------------------------------- launch chains
 
 // Kernel selection over (TP, COUL, ONE_TYPE); UNROLL follows TP (wide groups have few iterations per lane).
-template <int TP> struct UnrollOf { static constexpr int value = TP >= 8 ? 2 : 4; };
+// Listed pairs in flight per lane (the paper's one-ahead prefetch, P:108 item 4, generalised).  Measured on
+// B200 (2 / 4 / 8 / 16 per lane): 8 is best while a lane has >= ~10 entries, 4 for the wide groups.
+template <int TP> struct UnrollOf { static constexpr int value = TP >= 16 ? 4 : 8; };
 
 template <template <int, bool, bool> class F, int TP, typename... A>
 static auto pick_flags(rumd_system* s, A... a)
