@@ -215,6 +215,16 @@ __global__ void __launch_bounds__(PERSIST_THREADS, PERSIST_MINB) k_persist(const
                 ri = rc[i];
                 cnt = S.method == 2 ? 0 : S.num_nbrs[i];
             }
+            // Small systems (wide lane groups): the integrator's inputs are fetched BEFORE the force loop so that
+            // their latency hides behind it; at tp < 8 the twelve registers cost more than the latency (measured).
+            constexpr bool EARLY = TP >= 8;
+            float4 v = make_float4(0.f, 0.f, 0.f, 1.f), rb = v;
+            int4 im = make_int4(0, 0, 0, 0);
+            if (EARLY && have_i && t == 0) {
+                v = S.v[i];
+                im = S.image[i];
+                rb = S.r_build[i];
+            }
             float fx, fy, fz, u, w;
             if (last) // energies and virials are outputs of the LAST force evaluation only
                 force_any<TP, COUL, ONE_TYPE, UNROLL, false, true>(S, rc, s_pp, (int)vw, i, t, have_i, ri, cnt, fx, fy, fz, u, w);
@@ -225,11 +235,14 @@ __global__ void __launch_bounds__(PERSIST_THREADS, PERSIST_MINB) k_persist(const
                 __threadfence_block();
                 const float a = ((volatile float*)s_ab)[0], b = ((volatile float*)s_ab)[1];
                 const float4 f = make_float4(fx, fy, fz, 0.5f * u);
-                float4 v = S.v[i];
-                int4 im = S.image[i];
+                if (!EARLY) {
+                    v = S.v[i];
+                    im = S.image[i];
+                    rb = S.r_build[i];
+                }
                 bool mv;
                 double kti, mv2i;
-                integrate_particle(S, a, b, ri, v, f, im, S.r_build[i], mv, kti, mv2i);
+                integrate_particle(S, a, b, ri, v, f, im, rb, mv, kti, mv2i);
                 rn[i] = ri;
                 S.v[i] = v;
                 S.image[i] = im;
