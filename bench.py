@@ -148,12 +148,29 @@ def whole_job_rate(units_per_rank: float, seconds_local: float, world: int, devi
 # ------------------------------------------------------------------------------------------------ GPU arm
 
 # DRAM bytes (read + write) per MD time step of the dominant kernel, from the committed ncu --set full captures
-# (profiles/r01_persist_c1_ncu.md: 4.68 MB per 200-step k_persist launch at C1; profiles/r01_force_lj1m_ncu.md:
-# 378 MB per k_force launch at C3).  Workloads without a capture report traffic = null.
-NCU_DRAM_BYTES_PER_TIMESTEP = {"ka8000": 4.68e6 / 200, "lj1m": 378e6}
+# (profiles/r01_persist_c1_ncu.md: 4.87 MB per 200-step k_persist launch at C1; profiles/r01_force_lj1m_ncu.md:
+# 376.8 MB per k_force launch at C3).  Workloads without a capture report traffic = null.
+NCU_DRAM_BYTES_PER_TIMESTEP = {"ka8000": 4.87e6 / 200, "lj1m": 376.8e6}
 
 FLOP_PER_LISTED_PAIR_LJ = 42.0       # SURVEY.md 8(d) / DESIGN.md "Roofline": 21 always + 30 x 0.712 inside rc
 FLOP_PER_LISTED_PAIR_COUL = 50.0     # + the Coulomb term
+
+
+def count_listed(s):
+    """Listed pairs of the current state (the unit of the flop convention).  With the "none" method there is no
+    list: the count is taken from a list built once with the N^2 method at the same skin."""
+    from paper_1506_05094_b200 import rumd
+
+    t = s.get_tuning()
+    none = t.method == rumd.NB_NONE
+    if none:
+        s.set_tuning(method=rumd.NB_N2)
+    s.compute_forces()
+    cnt, _ = s.export_nblist()
+    if none:
+        s.set_tuning(method=rumd.NB_NONE)
+        s.compute_forces()
+    return int(cnt.sum())
 
 
 def equilibrate(s, wl, steps):
@@ -246,9 +263,7 @@ def run_gpu(args, rank, world, local_rank):
     out = None
     if rank == 0:
         # ---- roofline of the dominant kernel (pair force), timed live with CUDA events on the library's stream
-        s.compute_forces()
-        cnt, _ = s.export_nblist()
-        listed = int(cnt.sum())
+        listed = count_listed(s)
         us = s.time_force(reps=200)
         coul = bool((wl.pot[..., 4] > 0).any())
         flop = (FLOP_PER_LISTED_PAIR_COUL if coul else FLOP_PER_LISTED_PAIR_LJ) * listed
@@ -257,6 +272,7 @@ def run_gpu(args, rank, world, local_rank):
         peak_tf = fp32_peak_tflops(peaks["sm_max_mhz"])
         ach_tf = flop / (us * 1e-6) / 1e12
         alg_bytes = 4.0 * listed + (16 + 4 + 20) * N
+        s.profile_step()          # first call pays CUDA's lazy loading of the un-fused kernels
         prof = s.profile_step()
         flop_pp = flop / listed
         force_kernel = {"kernel": "k_force (stand-alone, current tuning)", "us_per_launch": us, "achieved": ach_tf,
@@ -343,9 +359,7 @@ def run_sweep(args, names):
         ms = sum(a.elapsed_time(b) for a, b in ev)
         th1 = s.get_thermo()
         tps = 5 * inner / (ms * 1e-3)
-        s.compute_forces()
-        cnt, _ = s.export_nblist()
-        listed = int(cnt.sum())
+        listed = count_listed(s)
         us = s.time_force(reps=50)
         coul = bool((wl.pot[..., 4] > 0).any())
         flop = (FLOP_PER_LISTED_PAIR_COUL if coul else FLOP_PER_LISTED_PAIR_LJ) * listed
