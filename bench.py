@@ -376,6 +376,49 @@ def run_sweep(args, names):
     return out
 
 
+# ------------------------------------------------------------------------------------------------ ensembles
+
+ENSEMBLES = [("ka512", 444), ("ka1000", 444), ("ka2048", 444)]
+
+
+def run_ensembles(args, specs):
+    """SURVEY 8(f)-2 / P:63: R independent replicas of a small system advanced by one launch (one thread block per
+    replica).  Reports replica-time-steps per second (R x steps / time) and particle-steps per second."""
+    import torch
+
+    from paper_1506_05094_b200 import rumd
+
+    out = []
+    for name, R in specs:
+        wl, desc = make_workload(name)
+        v = np.stack([W.maxwell_boltzmann(np.random.default_rng(W.SEED0 + 7000 + q), wl.m.astype(np.float64),
+                                          float(wl.T0)).astype(np.float32) for q in range(R)])
+        best = None
+        for tp in (2, 4, 8):
+            s = rumd.System(np.stack([wl.r] * R), v, wl.m, wl.types, wl.box, wl.pot, skin_for_capacity=0.6)
+            s.set_integrator(wl.integrator, wl.dt, wl.T0, wl.tau)
+            s.set_tuning(method=rumd.NB_N2, tp=tp, pb=256 // tp, skin=0.45)
+            s.run_steps(args.equil)
+            s.get_thermo_replicas()
+            n = max(200, min(2000, int(4e8 / (R * wl.N))))
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(s.stream)
+            s.run_steps(n)
+            b.record(s.stream)
+            torch.cuda.synchronize()
+            ms = a.elapsed_time(b)
+            s.get_thermo_replicas()
+            rate = R * n / (ms * 1e-3)
+            if best is None or rate > best["replica_timesteps_per_s"]:
+                best = {"workload": name, "N": wl.N, "replicas": R, "tp": tp, "replica_timesteps_per_s": rate,
+                        "particle_steps_per_s": rate * wl.N, "us_per_batch_step": 1e3 * ms / n}
+            s.close()
+        out.append(best)
+        print("ensemble %s x%d: %.0f replica-timesteps/s" % (name, R, best["replica_timesteps_per_s"]), file=sys.stderr,
+              flush=True)
+    return out
+
+
 # ------------------------------------------------------------------------------------------------ oracle arm
 
 
@@ -477,6 +520,8 @@ def main():
             out["cpu_baseline"] = None
         if args.sweep is not None and world == 1:
             out["sweep"] = run_sweep(args, args.sweep or SWEEP)
+            if not args.sweep:
+                out["ensembles"] = run_ensembles(args, ENSEMBLES)
         print(json.dumps(out), flush=True)
     if world > 1:
         torch.distributed.barrier()

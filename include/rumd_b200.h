@@ -111,6 +111,20 @@ rumd_status rumd_create(rumd_system** out, int n_particles, int n_types, const f
                         void* cuda_stream);
 rumd_status rumd_destroy(rumd_system* s);
 
+/* Batched ensemble ("large ensembles of MD simulations of small systems"): the handle describes ONE
+ * system of n_particles; after rumd_set_replicas(s, R), R >= 1, the state arrays of rumd_bind_state hold R such
+ * systems back to back (replica q owns elements [q n, (q+1) n)), all with the same box, potentials, integrator
+ * and tuning, each with its own list, thermostat and counters, and rumd_run_steps(n) advances all of them by
+ * n steps in ONE kernel launch (one thread block per replica, no inter-block synchronisation).  Must be called
+ * before rumd_bind_state / rumd_bind_workspace (the workspace grows with R).  Needs method RUMD_NB_N2 or
+ * RUMD_NB_NONE.  With R > 1 the single-system calls (rumd_build_nblist, rumd_compute_forces,
+ * rumd_export_nblist, rumd_get_thermo, rumd_snapshot / restore, rumd_autotune, the profiling calls) return
+ * RUMD_ERR_INVALID_ARG; use rumd_get_thermo_replicas.  d_f / d_w hold the forces of the last step of a run. */
+rumd_status rumd_set_replicas(rumd_system* s, int n_replicas);
+/* out: HOST array of n_out >= R records, one per replica (U, W, K of the last step of the last run; xi, eta, H,
+ * counters).  Synchronizes; reports sticky errors of any replica. */
+rumd_status rumd_get_thermo_replicas(rumd_system* s, rumd_thermo* out, int n_out);
+
 /* State arrays, DEVICE pointers, caller-owned, n_particles elements each, 16-byte aligned:
  *   d_r     float4 : x, y, z, particle type as int bits in .w             (Fig. 3)
  *   d_v     float4 : leap-frog velocity v(t - dt/2) x, y, z; mass in .w   (S8)

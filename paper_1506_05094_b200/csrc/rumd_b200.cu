@@ -2,6 +2,7 @@
 // chains, whole-timestep CUDA graphs and the Blackwell autotuner.  Product code: shares nothing with oracle/.
 #include "../../include/rumd_b200.h"
 #include "rumd_persist.cuh"
+#include "rumd_ensemble.cuh"
 
 #include <algorithm>
 #include <cmath>
@@ -24,7 +25,10 @@ struct GraphCache {
 };
 
 struct rumd_system {
-    int N = 0, ntypes = 0;
+    int N = 0, ntypes = 0;  // N: particles of ONE system
+    int nrep = 1;           // replicas (batched ensemble); the state arrays hold nrep * N particles
+    Sys* d_systems = nullptr;     // ensemble: per-replica parameter blocks (in the workspace)
+    DevScalars* ens_sc = nullptr; // ensemble: per-replica scalars (in the workspace)
     float box[3] = {0, 0, 0};
     cudaStream_t stream = nullptr;
     bool own_stream = false;
@@ -131,7 +135,9 @@ static uint32_t part1by1(uint32_t x) // spread the low 16 bits to the even bit p
 // Carve the workspace.  Returns bytes needed; if base != nullptr also fills the pointers.
 static size_t carve(rumd_system* s, char* base, int cap)
 {
-    const size_t N = (size_t)s->N, Npad = align_up(N, 32);
+    // ensemble: every replica owns a slice of each particle array; list rows are padded per replica
+    const size_t R = (size_t)s->nrep;
+    const size_t N = (size_t)s->N * R, Npad = align_up((size_t)s->N, 32) * R;
     const size_t nc = max_cells(s);
     size_t off = 0;
     auto take = [&](size_t bytes) {
@@ -166,6 +172,10 @@ static size_t carve(rumd_system* s, char* base, int cap)
     const size_t nblk = std::max<size_t>(N + 1, 2 * 4096); // the fused per-step kernel may run N blocks (pb = 1)
     p = take(nblk * 16); if (base) S.partial = (double*)p;
     p = take(8 * 8); if (base) s->prof_buf = (long long*)p;
+    if (R > 1) {
+        p = take(R * sizeof(Sys)); if (base) s->d_systems = (Sys*)p;
+        p = take(R * sizeof(DevScalars)); if (base) s->ens_sc = (DevScalars*)p;
+    }
     return off;
 }
 
@@ -240,6 +250,26 @@ extern "C" rumd_status rumd_destroy(rumd_system* s)
 
 // ---------------------------------------------------------------------------------------------- setters
 
+static void ens_reset(rumd_system* s)
+{
+    if (s->nrep > 1 && s->ens_sc) {
+        k_ens_reset<<<(s->nrep + 127) / 128, 128, 0, s->stream>>>(s->ens_sc, s->nrep);
+        s->launches++;
+    }
+}
+
+// Batched ensemble: the handle describes ONE system of n_particles; with n_replicas > 1 the state arrays
+// hold n_replicas such systems back to back and rumd_run_steps advances all of them in one launch.
+extern "C" rumd_status rumd_set_replicas(rumd_system* s, int n_replicas)
+{
+    if (!s) return RUMD_ERR_INVALID_ARG;
+    if (n_replicas < 1 || (long long)n_replicas * s->N > (1LL << 30)) return fail(s, RUMD_ERR_INVALID_ARG, "bad replica count");
+    if (s->state_bound || s->ws_bound) return fail(s, RUMD_ERR_NOT_READY, "set the replica count before binding state and workspace");
+    s->nrep = n_replicas;
+    s->params_dirty = true;
+    return RUMD_OK;
+}
+
 extern "C" rumd_status rumd_bind_state(rumd_system* s, void* d_r, void* d_v, void* d_f, void* d_w, void* d_image,
                                        void* d_id)
 {
@@ -259,6 +289,7 @@ extern "C" rumd_status rumd_bind_state(rumd_system* s, void* d_r, void* d_v, voi
     if (s->ws_bound) {
         k_reset_scalars<<<1, 1, 0, s->stream>>>(s->S);
         s->launches++;
+        ens_reset(s);
         CUDA_TRY(s, cudaGetLastError());
     }
     return RUMD_OK;
@@ -294,7 +325,7 @@ extern "C" rumd_status rumd_bind_workspace(rumd_system* s, void* d_ws, size_t by
     s->grid_for[0] = s->grid_for[1] = s->grid_for[2] = 0;
     drop_graphs(s);
     CUDA_TRY(s, cudaMemsetAsync(s->S.ccount, 0, max_cells(s) * 4, s->stream));
-    CUDA_TRY(s, cudaMemsetAsync(s->S.num_nbrs, 0, align_up((size_t)s->N, 32) * 4, s->stream));
+    CUDA_TRY(s, cudaMemsetAsync(s->S.num_nbrs, 0, align_up((size_t)s->N, 32) * (size_t)s->nrep * 4, s->stream));
     if (had) {
         keep.flag = 1u;
         keep.pending = 0u;
@@ -307,6 +338,7 @@ extern "C" rumd_status rumd_bind_workspace(rumd_system* s, void* d_ws, size_t by
     } else {
         k_reset_scalars<<<1, 1, 0, s->stream>>>(s->S);
         s->launches++;
+        ens_reset(s);
         CUDA_TRY(s, cudaGetLastError());
     }
     return RUMD_OK;
@@ -518,11 +550,40 @@ static rumd_status refresh(rumd_system* s)
     }
     s->int_blocks = (s->N + INT_THREADS - 1) / INT_THREADS;
     s->persist_grid_for = -1;
+    if (s->nrep > 1) {
+        if (t.method == RUMD_NB_CELL) return fail(s, RUMD_ERR_INVALID_ARG, "replicas use the n2 or the none method (one block per replica)");
+        // per-replica parameter blocks: the same constants, pointers moved to the replica's slices
+        std::vector<Sys> sys((size_t)s->nrep, S);
+        const size_t n = (size_t)s->N, npad = (size_t)S.Npad;
+        for (int q = 0; q < s->nrep; ++q) {
+            Sys& Q = sys[(size_t)q];
+            Q.r = S.r + q * n;
+            Q.v = S.v + q * n;
+            Q.f = S.f + q * n;
+            Q.w = S.w + q * n;
+            Q.image = S.image + q * n;
+            Q.id = S.id + q * n;
+            Q.r_out = Q.r;
+            Q.r_alt = S.r_alt + q * n;
+            Q.r_build = S.r_build + q * n;
+            Q.nbl = S.nbl + q * npad * (size_t)S.cap;
+            Q.num_nbrs = S.num_nbrs + q * npad;
+            Q.sc = s->ens_sc + q;
+            Q.prof = nullptr;
+        }
+        CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+        CUDA_TRY(s, cudaMemcpyAsync(s->d_systems, sys.data(), sys.size() * sizeof(Sys), cudaMemcpyHostToDevice, s->stream));
+        CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+    }
     s->params_dirty = false;
     drop_graphs(s);
     // a list built with other parameters (skin, tp layout, method) is void
     k_request_rebuild<<<1, 1, 0, s->stream>>>(S);
     s->launches++;
+    if (s->nrep > 1) {
+        k_ens_request_rebuild<<<(s->nrep + 127) / 128, 128, 0, s->stream>>>(s->ens_sc, s->nrep);
+        s->launches++;
+    }
     CUDA_TRY(s, cudaGetLastError());
     return RUMD_OK;
 }
@@ -576,6 +637,10 @@ template <int TP, bool COUL, bool ONE> struct PersistKernel {
 };
 
 static int persist_threads_of(const rumd_tuning&) { return PERSIST_THREADS; }
+
+template <int TP, bool COUL, bool ONE> struct EnsembleKernel {
+    static const void* run(rumd_system*) { return (const void*)&k_ensemble<TP, COUL, ONE, UnrollOf<TP>::value>; }
+};
 
 // n steps in ONE cooperative launch.  The grid is sized to cover N*tp virtual threads when it can be
 // co-resident, else to the co-residency limit (the kernel strides).
@@ -670,6 +735,13 @@ static int launch_step(rumd_system* s)
     return n;
 }
 
+// entry points that only make sense for a single system
+#define SINGLE_ONLY(s)                                                                                   \
+    do {                                                                                                 \
+        if ((s) && (s)->nrep > 1)                                                                        \
+            return fail((s), RUMD_ERR_INVALID_ARG, "not available for a batched ensemble (replicas > 1)"); \
+    } while (0)
+
 static rumd_status ready(rumd_system* s, bool need_integ)
 {
     if (!s) return RUMD_ERR_INVALID_ARG;
@@ -679,6 +751,7 @@ static rumd_status ready(rumd_system* s, bool need_integ)
 
 extern "C" rumd_status rumd_build_nblist(rumd_system* s)
 {
+    SINGLE_ONLY(s);
     rumd_status st = ready(s, false);
     if (st != RUMD_OK) return st;
     k_request_rebuild<<<1, 1, 0, s->stream>>>(s->S);
@@ -689,6 +762,7 @@ extern "C" rumd_status rumd_build_nblist(rumd_system* s)
 
 extern "C" rumd_status rumd_compute_forces(rumd_system* s)
 {
+    SINGLE_ONLY(s);
     rumd_status st = ready(s, false);
     if (st != RUMD_OK) return st;
     s->launches += launch_rebuild_chain(s);
@@ -752,6 +826,17 @@ extern "C" rumd_status rumd_run_steps(rumd_system* s, long n)
     if (st != RUMD_OK) return st;
     if (n < 0) return fail(s, RUMD_ERR_INVALID_ARG, "negative step count");
     if (n == 0) return RUMD_OK;
+    if (s->nrep > 1) { // batched ensemble: one block per replica runs the whole call
+        for (long left = n; left > 0;) {
+            int chunk = (int)std::min<long>(left, 1L << 20);
+            int nvt = s->integ == RUMD_INT_NVT_NOSE_HOOVER;
+            void* args[] = {(void*)&s->d_systems, (void*)&chunk, (void*)&nvt};
+            CUDA_TRY(s, cudaLaunchKernel(pick_kernel<EnsembleKernel>(s), dim3(s->nrep), dim3(ENS_THREADS), args, 0, s->stream));
+            s->launches += 1;
+            left -= chunk;
+        }
+        return RUMD_OK;
+    }
     if (s->tune.persistent) {
         // one cooperative launch per <= 2^16 steps (keeps the 32-bit arrival count of the grid barrier in range)
         for (long left = n; left > 0;) {
@@ -795,6 +880,7 @@ extern "C" rumd_status rumd_run_steps(rumd_system* s, long n)
 
 extern "C" rumd_status rumd_export_nblist(rumd_system* s, void* d_count, void* d_list, int row_capacity)
 {
+    SINGLE_ONLY(s);
     rumd_status st = ready(s, false);
     if (st != RUMD_OK) return st;
     if (!d_count || !d_list || row_capacity < 1) return fail(s, RUMD_ERR_INVALID_ARG, "bad export arguments");
@@ -806,6 +892,7 @@ extern "C" rumd_status rumd_export_nblist(rumd_system* s, void* d_count, void* d
 
 extern "C" rumd_status rumd_get_thermo(rumd_system* s, rumd_thermo* out)
 {
+    SINGLE_ONLY(s);
     rumd_status st = ready(s, false);
     if (st != RUMD_OK) return st;
     if (!out) return fail(s, RUMD_ERR_INVALID_ARG, "null output");
@@ -843,8 +930,47 @@ extern "C" rumd_status rumd_get_thermo(rumd_system* s, rumd_thermo* out)
     return RUMD_OK;
 }
 
+// Per-replica thermodynamic scalars of a batched ensemble; U, W, K refer to the last step of the last run.
+extern "C" rumd_status rumd_get_thermo_replicas(rumd_system* s, rumd_thermo* out, int n_out)
+{
+    rumd_status st = ready(s, false);
+    if (st != RUMD_OK) return st;
+    if (s->nrep < 2) return fail(s, RUMD_ERR_INVALID_ARG, "no replicas: use rumd_get_thermo");
+    if (!out || n_out < s->nrep) return fail(s, RUMD_ERR_INVALID_ARG, "output array too small");
+    std::vector<DevScalars> h((size_t)s->nrep);
+    CUDA_TRY(s, cudaMemcpyAsync(h.data(), s->ens_sc, h.size() * sizeof(DevScalars), cudaMemcpyDeviceToHost, s->stream));
+    CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+    CUDA_TRY(s, cudaGetLastError());
+    rumd_status worst = RUMD_OK;
+    for (int q = 0; q < s->nrep; ++q) {
+        const DevScalars& d = h[(size_t)q];
+        rumd_thermo& o = out[q];
+        o.U = d.U;
+        o.W = d.W;
+        o.K = d.K;
+        o.mv2 = d.mv2;
+        o.xi = d.xi;
+        o.eta = d.eta;
+        o.H = d.K + d.U;
+        if (s->integ == RUMD_INT_NVT_NOSE_HOOVER) {
+            o.H += s->S.g * s->S.T0 * d.eta_t;
+            if (s->S.omega2 > 0) o.H += 0.5 * s->S.g * s->S.T0 * d.xi_t * d.xi_t / s->S.omega2;
+        }
+        o.n_steps = d.n_steps;
+        o.n_rebuilds = d.n_rebuilds;
+        o.max_nbrs = d.max_nbrs[0];
+        o.nbl_capacity = s->cap;
+        o.overflow = (int)d.overflow;
+        o.pad_ = 0;
+        if (d.overflow) worst = fail(s, RUMD_ERR_NBL_OVERFLOW, "neighbour list overflow in replica %d: %d neighbours > capacity %d", q, d.max_nbrs[0], s->cap);
+        else if (d.nonfinite && worst == RUMD_OK) worst = fail(s, RUMD_ERR_NONFINITE, "non-finite energy in replica %d", q);
+    }
+    return worst;
+}
+
 extern "C" rumd_status rumd_snapshot(rumd_system* s)
 {
+    SINGLE_ONLY(s);
     rumd_status st = ready(s, false);
     if (st != RUMD_OK) return st;
     const Sys& S = s->S;
@@ -858,6 +984,7 @@ extern "C" rumd_status rumd_snapshot(rumd_system* s)
 
 extern "C" rumd_status rumd_restore(rumd_system* s)
 {
+    SINGLE_ONLY(s);
     rumd_status st = ready(s, false);
     if (st != RUMD_OK) return st;
     const Sys& S = s->S;
@@ -875,13 +1002,14 @@ extern "C" rumd_status rumd_upload_state(rumd_system* s, const void* h_r, const 
 {
     rumd_status st = ready(s, false);
     if (st != RUMD_OK) return st;
-    const size_t N = (size_t)s->N;
+    const size_t N = (size_t)s->N * (size_t)s->nrep;
     if (h_r) CUDA_TRY(s, cudaMemcpyAsync(s->S.r, h_r, N * 16, cudaMemcpyHostToDevice, s->stream));
     if (h_v) CUDA_TRY(s, cudaMemcpyAsync(s->S.v, h_v, N * 16, cudaMemcpyHostToDevice, s->stream));
     if (h_image) CUDA_TRY(s, cudaMemcpyAsync(s->S.image, h_image, N * 16, cudaMemcpyHostToDevice, s->stream));
     if (h_id) CUDA_TRY(s, cudaMemcpyAsync(s->S.id, h_id, N * 4, cudaMemcpyHostToDevice, s->stream));
     k_reset_scalars<<<1, 1, 0, s->stream>>>(s->S);
     s->launches++;
+    ens_reset(s);
     CUDA_TRY(s, cudaGetLastError());
     return RUMD_OK;
 }
@@ -891,7 +1019,7 @@ extern "C" rumd_status rumd_download_state(rumd_system* s, void* h_r, void* h_v,
 {
     rumd_status st = ready(s, false);
     if (st != RUMD_OK) return st;
-    const size_t N = (size_t)s->N;
+    const size_t N = (size_t)s->N * (size_t)s->nrep;
     if (h_r) CUDA_TRY(s, cudaMemcpyAsync(h_r, s->S.r, N * 16, cudaMemcpyDeviceToHost, s->stream));
     if (h_v) CUDA_TRY(s, cudaMemcpyAsync(h_v, s->S.v, N * 16, cudaMemcpyDeviceToHost, s->stream));
     if (h_f) CUDA_TRY(s, cudaMemcpyAsync(h_f, s->S.f, N * 16, cudaMemcpyDeviceToHost, s->stream));
@@ -905,6 +1033,7 @@ extern "C" rumd_status rumd_download_state(rumd_system* s, void* h_r, void* h_v,
 // One un-graphed step with events around each kernel class (launch-gap / share analysis at small N).
 extern "C" rumd_status rumd_profile_step(rumd_system* s, float* ms_out, int* did_rebuild_out)
 {
+    SINGLE_ONLY(s);
     rumd_status st = ready(s, true);
     if (st != RUMD_OK) return st;
     if (!ms_out) return fail(s, RUMD_ERR_INVALID_ARG, "null output");
@@ -933,6 +1062,7 @@ extern "C" rumd_status rumd_profile_step(rumd_system* s, float* ms_out, int* did
 // a graph (no host launch gaps), bracketed by CUDA events on the library's stream.  The list must exist.
 extern "C" rumd_status rumd_time_force(rumd_system* s, int reps, float* us_per_launch)
 {
+    SINGLE_ONLY(s);
     rumd_status st = ready(s, false);
     if (st != RUMD_OK) return st;
     if (reps < 1 || !us_per_launch) return fail(s, RUMD_ERR_INVALID_ARG, "bad arguments");
@@ -967,6 +1097,7 @@ extern "C" rumd_status rumd_time_force(rumd_system* s, int reps, float* us_per_l
 // Where the time of the persistent kernel goes: runs n steps with the cycle counters of block 0 switched on.
 extern "C" rumd_status rumd_profile_persistent(rumd_system* s, int nsteps, double* out8)
 {
+    SINGLE_ONLY(s);
     rumd_status st = ready(s, true);
     if (st != RUMD_OK) return st;
     if (nsteps < 1 || !out8) return fail(s, RUMD_ERR_INVALID_ARG, "bad arguments");
@@ -1060,6 +1191,7 @@ struct Tuner {
 
 extern "C" rumd_status rumd_autotune(rumd_system* s, rumd_tuning* out, int steps_per_trial, double* tps_out)
 {
+    SINGLE_ONLY(s);
     rumd_status st = ready(s, true);
     if (st != RUMD_OK) return st;
     if (steps_per_trial < 8) steps_per_trial = 8;

@@ -27,7 +27,7 @@ EXPORTS = [
     "rumd_set_pair_potential", "rumd_set_integrator", "rumd_default_tuning", "rumd_set_tuning",
     "rumd_get_tuning", "rumd_autotune", "rumd_build_nblist", "rumd_compute_forces", "rumd_run_steps",
     "rumd_export_nblist", "rumd_get_thermo", "rumd_snapshot", "rumd_restore", "rumd_upload_state",
-    "rumd_download_state", "rumd_launch_count", "rumd_profile_step", "rumd_time_force", "rumd_profile_persistent", "rumd_last_error", "rumd_version",
+    "rumd_download_state", "rumd_launch_count", "rumd_profile_step", "rumd_time_force", "rumd_profile_persistent", "rumd_set_replicas", "rumd_get_thermo_replicas", "rumd_last_error", "rumd_version",
 ]
 
 
@@ -94,6 +94,8 @@ def lib():
         L.rumd_profile_step.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(ip)]
         L.rumd_time_force.argtypes = [vp, ip, C.POINTER(C.c_float)]
         L.rumd_profile_persistent.argtypes = [vp, ip, C.POINTER(C.c_double)]
+        L.rumd_set_replicas.argtypes = [vp, ip]
+        L.rumd_get_thermo_replicas.argtypes = [vp, C.POINTER(Thermo), ip]
         L.rumd_last_error.argtypes = [vp]
         L.rumd_last_error.restype = C.c_char_p
         L.rumd_version.restype = C.c_char_p
@@ -108,8 +110,9 @@ def estimate_capacity(density: float, rc_max: float, skin: float) -> int:
 
 
 class System:
-    """One simulation (Fig. 1).  Owns torch tensors for the state and the workspace and hands their
-    device pointers to the library.  ``wl`` is a ``workloads.Workload``-like object."""
+    """One simulation (Fig. 1), or a batched ensemble of R independent replicas of it when ``r`` and
+    ``v`` have shape (R, N, 3) (``rumd_set_replicas``): ``types`` and ``m`` may then be (N,) (shared) or
+    (R, N).  Owns torch tensors for the state and the workspace and hands their device pointers to the library."""
 
     def __init__(self, r, v, m, types, box, pot, device="cuda:0", skin_for_capacity=0.5, capacity=None,
                  stream=None):
@@ -119,23 +122,32 @@ class System:
         self.device = torch.device(device)
         torch.cuda.set_device(self.device)
         r = np.ascontiguousarray(r, dtype=np.float32)
-        N = r.shape[0]
-        self.N = N
+        self.replicas = int(r.shape[0]) if r.ndim == 3 else 1
+        R = self.replicas
+        self.N = int(r.shape[-2])       # particles of ONE system
+        if r.ndim == 3:
+            v = np.ascontiguousarray(v, dtype=np.float32).reshape(R * self.N, 3)
+            types = np.broadcast_to(np.asarray(types, dtype=np.int32), (R, self.N)).reshape(-1).copy()
+            m = np.broadcast_to(np.asarray(m, dtype=np.float32), (R, self.N)).reshape(-1).copy()
+            r = r.reshape(R * self.N, 3)
+        N = r.shape[0]                  # elements of the state arrays
         self.ntypes = int(pot.shape[0])
         self.box = np.ascontiguousarray(box, dtype=np.float32)
         # a dedicated side stream (the legacy default stream cannot be captured into CUDA graphs)
         self.stream = stream if stream is not None else torch.cuda.Stream(self.device)
         h = C.c_void_p()
-        st = self.L.rumd_create(C.byref(h), N, self.ntypes, self.box.ctypes.data_as(C.POINTER(C.c_float)),
+        st = self.L.rumd_create(C.byref(h), self.N, self.ntypes, self.box.ctypes.data_as(C.POINTER(C.c_float)),
                                 C.c_void_p(self.stream.cuda_stream))
         if st != OK:
             raise RumdError(st, "rumd_create failed")
         self.h = h
+        if R > 1:
+            self._check(self.L.rumd_set_replicas(self.h, R))
         # host staging (pinned) in the ABI layouts
         self.h_r = torch.zeros((N, 4), dtype=torch.float32).pin_memory()
         self.h_v = torch.zeros((N, 4), dtype=torch.float32).pin_memory()
         self.h_image = torch.zeros((N, 4), dtype=torch.int32).pin_memory()
-        self.h_id = torch.arange(N, dtype=torch.int32).pin_memory()
+        self.h_id = (torch.arange(N, dtype=torch.int32) % self.N).contiguous().pin_memory()
         self.h_r[:, :3] = torch.from_numpy(r)
         self.h_r[:, 3] = torch.from_numpy(np.ascontiguousarray(types, dtype=np.int32)).view(torch.float32)
         self.h_v[:, :3] = torch.from_numpy(np.ascontiguousarray(v, dtype=np.float32))
@@ -161,7 +173,7 @@ class System:
                 if rcc > 0:
                     self.set_pair_potential(a, b, POT_COULOMB, [qq, rcc], cut_c)
         self.rc_max = float(max(pot[..., 2].max(), pot[..., 4].max()))
-        self.density = N / float(np.prod(self.box.astype(np.float64)))
+        self.density = self.N / float(np.prod(self.box.astype(np.float64)))
         if capacity is None:
             capacity = estimate_capacity(self.density, self.rc_max, skin_for_capacity)
         self.d_ws = None
@@ -244,6 +256,11 @@ class System:
         self._check(st)
         return th.as_dict()
 
+    def get_thermo_replicas(self) -> list:
+        arr = (Thermo * self.replicas)()
+        self._check(self.L.rumd_get_thermo_replicas(self.h, arr, self.replicas))
+        return [t.as_dict() for t in arr]
+
     def snapshot(self):
         self._check(self.L.rumd_snapshot(self.h))
 
@@ -296,6 +313,14 @@ class System:
     # ---- convenience read-back (numpy, ORIGINAL particle numbering via d_id)
     def state(self) -> dict:
         self.stream.synchronize()
+        if self.replicas > 1:   # no sorting in ensembles: slots are original indices
+            R, n = self.replicas, self.N
+            r = self.d_r.cpu().numpy().reshape(R, n, 4)
+            v = self.d_v.cpu().numpy().reshape(R, n, 4)
+            f = self.d_f.cpu().numpy().reshape(R, n, 4)
+            return dict(r=r[..., :3].copy(), types=r[..., 3].copy().view(np.int32), v=v[..., :3].copy(),
+                        m=v[..., 3].copy(), F=f[..., :3].copy(), u=f[..., 3].copy(),
+                        w=self.d_w.cpu().numpy().reshape(R, n), image=self.d_image.cpu().numpy().reshape(R, n, 4)[..., :3].copy())
         ids = self.d_id.cpu().numpy().astype(np.int64)
         inv = np.empty_like(ids)
         inv[ids] = np.arange(self.N)

@@ -672,3 +672,86 @@ def test_invalid_arguments_are_rejected(rumd):
         s.compute_forces()
     assert e.value.status == rumd.ERR_BOX_TOO_SMALL
     s.close()
+
+
+# ------------------------------------------------------------------ batched ensembles
+
+
+def _ensemble_inputs(kind, kw, R, seed0=100):
+    wls = []
+    for q in range(R):
+        wl = perturbed(make(kind, **kw), seed=seed0 + q)
+        rng = np.random.default_rng(seed0 + 50 + q)
+        wl.v = W.maxwell_boltzmann(rng, wl.m.astype(np.float64), float(wl.T0)).astype(np.float32)
+        wls.append(wl)
+    return wls
+
+
+@pytest.mark.parametrize("kind,kw,tp,method,nvt", [("lj", dict(ncell=4), 16, "n2", False), ("ka", dict(N=512), 32, "n2", True),
+                                                   ("ka", dict(N=1000), 8, "n2", True), ("lj", dict(ncell=4), 32, "none", False)])
+def test_batched_ensemble_replicas_match_oracle_and_single_runs(rumd, kind, kw, tp, method, nvt):
+    """R independent replicas (different positions and velocities) advanced by ONE launch, one block each:
+    every replica's forces / energy against the oracle, its trajectory against the oracle's and -- in NVE --
+    bit for bit against the same system run alone through the single-system path."""
+    R, nsteps = 5, 31
+    wls = _ensemble_inputs(kind, kw, R)
+    wl0 = wls[0]
+    integ = W.NVT if nvt else W.NVE
+    s = rumd.System(np.stack([w.r for w in wls]), np.stack([w.v for w in wls]), wl0.m, wl0.types if kind != "ka" else
+                    np.stack([w.types for w in wls]), wl0.box, wl0.pot)
+    assert s.replicas == R
+    s.set_integrator(integ, wl0.dt, wl0.T0, wl0.tau)
+    m = rumd.NB_N2 if method == "n2" else rumd.NB_NONE
+    s.set_tuning(method=m, tp=tp, pb=256 // tp, skin=0.3)
+    s.run_steps(1)
+    th = s.get_thermo_replicas()
+    box = wl0.box.astype(np.float64)
+    for q, wl in enumerate(wls):
+        F, u, w = oracle.forces_allpairs(wl.r.astype(np.float64), wl.types, box, wl.pot)
+        assert abs(th[q]["U"] - u.sum()) <= ENERGY_TOL * np.abs(u).sum()
+        assert abs(th[q]["W"] - w.sum()) <= ENERGY_TOL * np.abs(w).sum()
+        assert th[q]["n_steps"] == 1 and (th[q]["n_rebuilds"] == (1 if method == "n2" else 0))
+    st1 = s.state()
+    for q, wl in enumerate(wls):
+        F, u, w = oracle.forces_allpairs(wl.r.astype(np.float64), wl.types, box, wl.pot)
+        rms = np.sqrt((F * F).sum(1).mean())
+        assert np.sqrt(((st1["F"][q] - F) ** 2).sum(1)).max() <= FORCE_TOL * rms
+    s.run_steps(nsteps - 1)
+    st = s.state()
+    th = s.get_thermo_replicas()
+    for q, wl in enumerate(wls):
+        o = oracle.run(wl.r.astype(np.float64), wl.v.astype(np.float64), wl.m.astype(np.float64), np.zeros((wl.N, 3), np.int32),
+                       wl.types, box, wl.pot, 0.3, float(wl.dt), nsteps, mode=integ, T0=wl.T0, tau=wl.tau)
+        d = st["r"][q].astype(np.float64) - o["r"]
+        d -= box * np.rint(d / box)
+        assert np.abs(d).max() < 2e-4
+        assert th[q]["n_steps"] == nsteps
+        assert th[q]["U"] == pytest.approx(o["log"][-1, 0], rel=1e-4, abs=1e-3)
+        if nvt:
+            assert th[q]["xi"] == pytest.approx(o["xi"], rel=1e-3, abs=1e-6)
+    s.close()
+    if not nvt:   # the same replica alone, single-system persistent path: bit-identical
+        for q in (0, R - 1):
+            wl = wls[q]
+            s1 = rumd.System(wl.r, wl.v, wl.m, wl.types, wl.box, wl.pot)
+            s1.set_integrator(integ, wl.dt, wl.T0, wl.tau)
+            s1.set_tuning(method=m, tp=tp, pb=256 // tp, skin=0.3, persistent=1)
+            s1.run_steps(1)
+            s1.run_steps(nsteps - 1)
+            a = s1.state()
+            assert np.array_equal(a["r"], st["r"][q]) and np.array_equal(a["v"], st["v"][q])
+            assert np.array_equal(a["F"], st["F"][q])
+            s1.close()
+
+
+def test_batched_ensemble_rejects_single_system_calls(rumd):
+    wls = _ensemble_inputs("lj", dict(ncell=4), 3)
+    s = rumd.System(np.stack([w.r for w in wls]), np.stack([w.v for w in wls]), wls[0].m, wls[0].types, wls[0].box, wls[0].pot)
+    s.set_integrator(W.NVE, 0.005)
+    for call in (s.compute_forces, s.build_nblist, s.get_thermo, s.snapshot):
+        with pytest.raises(rumd.RumdError):
+            call()
+    s.set_tuning(method=rumd.NB_CELL)
+    with pytest.raises(rumd.RumdError):
+        s.run_steps(1)
+    s.close()
