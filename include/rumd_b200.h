@@ -44,7 +44,14 @@ typedef enum {
     RUMD_ERR_NONFINITE = 6      /* energy is NaN/Inf */
 } rumd_status;
 
-typedef enum { RUMD_POT_LJ_12_6 = 0, RUMD_POT_COULOMB = 1 } rumd_pot_kind;
+typedef enum { /* P:73 pair potentials; the first is the LJ slot of a type pair, all the others share its second slot */
+    RUMD_POT_LJ_12_6 = 0,       /* {epsilon, sigma, rcut}   u = 4 eps [(s/r)^12 - (s/r)^6] */
+    RUMD_POT_COULOMB = 1,       /* {k qi qj, rcut}          u = a / r */
+    RUMD_POT_IPL = 2,           /* {a, n, rcut}             u = a r^-n   (inverse power law) */
+    RUMD_POT_YUKAWA = 3,        /* {a, b, rcut}             u = a exp(-r / b) / r */
+    RUMD_POT_GAUSSIAN_CORE = 4, /* {a, b, rcut}             u = a exp(-(r / b)^2) */
+    RUMD_POT_BUCKINGHAM = 5     /* {a, b, c, rcut}          u = a exp(-r / b) - c / r^6 */
+} rumd_pot_kind;
 typedef enum { /* P:73-75 "the cutoff methods: no shift, shifted potential and shifted force" */
     RUMD_CUT_SHIFTED_FORCE = 0,     /* f = f(r) - f(rc), u = u(r) - u(rc) + (r - rc) f(rc): the hot-path default */
     RUMD_CUT_SHIFTED_POTENTIAL = 1, /* f = f(r),         u = u(r) - u(rc) */
@@ -146,6 +153,8 @@ rumd_status rumd_bind_workspace(rumd_system* s, void* d_ws, size_t bytes, int nb
 /* P:49-50 `pot.SetParams(i, j, Sigma, Epsilon, Rcut)`; symmetric in (type_i, type_j).  params: host.
  *   RUMD_POT_LJ_12_6 : {epsilon, sigma, rcut}   u = 4 eps [(s/r)^12 - (s/r)^6]           (O3)
  *   RUMD_POT_COULOMB : {k*q_i*q_j, rcut}        u = k q_i q_j / r, no self term          (O4, S6)
+ *   RUMD_POT_IPL / YUKAWA / GAUSSIAN_CORE / BUCKINGHAM : see rumd_pot_kind; they occupy the same slot as
+ *   Coulomb (a type pair has the LJ term plus at most ONE of these; setting one replaces the other).
  * rcut is an ABSOLUTE distance (S2).  cutoff: one of rumd_cutoff, applied for r < rcut, zero beyond (S3).
  * One slot per kind per type pair: the same kind again overwrites, different kinds add, each with its own
  * rc and cutoff method (S5).  rcut <= 0 removes the term. */

@@ -9,8 +9,9 @@ arrays.  See the header of ``rumd_oracle.c`` for the list of pins.
 
 Array conventions: positions / velocities / forces are float64 ``(N, 3)``; types int32 ``(N,)``;
 box float64 ``(3,)``; potentials float64 ``(ntypes, ntypes, 5)`` with records
-``(epsilon, sigma, rc_LJ, k*qa*qb, rc_Coulomb, cut_LJ, cut_Coulomb)`` (an rc <= 0 disables that term;
-cut = 0 shifted force, 1 shifted potential, 2 no shift).
+``(epsilon, sigma, rc_LJ, a, rc_2, cut_LJ, cut_2, kind_2, b, c)`` (an rc <= 0 disables that term;
+cut = 0 shifted force, 1 shifted potential, 2 no shift; kind_2 = 0 Coulomb a/r, 1 IPL a r^-b,
+2 Yukawa a exp(-r/b)/r, 3 Gaussian core a exp(-(r/b)^2), 4 Buckingham a exp(-r/b) - c/r^6).
 """
 from __future__ import annotations
 
@@ -25,7 +26,7 @@ _SRC = os.path.join(_HERE, "rumd_oracle.c")
 _LIB = os.path.join(_HERE, "librumd_oracle.so")
 
 NVE, NVT = 0, 1
-POT_STRIDE = 7
+POT_STRIDE = 10
 
 
 def build(force: bool = False) -> str:
@@ -55,6 +56,8 @@ def lib():
         L.orc_coulomb_sf.argtypes = [C.c_double] * 3 + [_dp, _dp]
         L.orc_lj_cut.argtypes = [C.c_double] * 4 + [C.c_int, _dp, _dp]
         L.orc_coulomb_cut.argtypes = [C.c_double] * 3 + [C.c_int, _dp, _dp]
+        L.orc_extra_raw.argtypes = [C.c_int] + [C.c_double] * 4 + [_dp, _dp]
+        L.orc_extra_cut.argtypes = [C.c_int] + [C.c_double] * 5 + [C.c_int, _dp, _dp]
         L.orc_pair_sf.argtypes = [_dp, C.c_double, _dp, _dp]
         L.orc_pair_rc.argtypes = [_dp]
         L.orc_pair_rc.restype = C.c_double
@@ -128,6 +131,15 @@ def lj_cut(r, eps, sig, rc, method):
 
 def coulomb_cut(r, qq, rc, method):
     return _pair(lib().orc_coulomb_cut, float(r), float(qq), float(rc), int(method))
+
+
+def extra_raw(kind, r, a, b=0.0, c=0.0):
+    """(u, f) of the unshifted second-term potentials: 0 Coulomb, 1 IPL, 2 Yukawa, 3 Gaussian core, 4 Buckingham."""
+    return _pair(lib().orc_extra_raw, int(kind), float(r), float(a), float(b), float(c))
+
+
+def extra_cut(kind, r, a, b, c, rc, method):
+    return _pair(lib().orc_extra_cut, int(kind), float(r), float(a), float(b), float(c), float(rc), int(method))
 
 
 def pair_sf(rec, r):

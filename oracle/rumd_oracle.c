@@ -31,6 +31,12 @@
  *     pot[0]=epsilon pot[1]=sigma pot[2]=rc_LJ (<=0: no LJ term) pot[3]=k*qa*qb pot[4]=rc_Coulomb (<=0: none)
  *     pot[5]=cutoff method of the LJ term, pot[6]=cutoff method of the Coulomb term:
  *            0 = shifted force, 1 = shifted potential, 2 = no shift (plain truncation)
+ *     pot[7]=kind of the second term (P:73 list of pair potentials), with pot[3]=a, pot[8]=b, pot[9]=c:
+ *            0 Coulomb        u = a / r                      (a = k q_i q_j)
+ *            1 inverse power  u = a r^-b                     (IPL)
+ *            2 Yukawa         u = a exp(-r / b) / r
+ *            3 Gaussian core  u = a exp(-(r / b)^2)
+ *            4 Buckingham     u = a exp(-r / b) - c / r^6
  * rc values are ABSOLUTE distances (S2).
  */
 #include <math.h>
@@ -40,7 +46,7 @@
 #include <omp.h>
 #endif
 
-#define ORC_POT_STRIDE 7
+#define ORC_POT_STRIDE 10
 
 int orc_num_threads(void)
 {
@@ -143,6 +149,35 @@ void orc_coulomb_cut(double r, double qq, double rc, int method, double *u, doub
     orc_apply_cutoff(method, r, rc, qq / r, qq / (r * r), qq / rc, qq / (rc * rc), u, f);
 }
 
+/* The other pair potentials of P:73 ("IPL, Gaussian core, Buckingham, ..., Yukawa"), unshifted: (u, f = -du/dr). */
+void orc_extra_raw(int kind, double r, double a, double b, double c, double *u, double *f)
+{
+    if (kind == 1) {          /* inverse power law: u = a r^-b, f = b a r^-(b+1) */
+        *u = a * pow(r, -b);
+        *f = b * a * pow(r, -b - 1.0);
+    } else if (kind == 2) {   /* Yukawa: u = a e^(-r/b) / r, f = u (1/r + 1/b) */
+        *u = a * exp(-r / b) / r;
+        *f = *u * (1.0 / r + 1.0 / b);
+    } else if (kind == 3) {   /* Gaussian core: u = a e^(-(r/b)^2), f = 2 r u / b^2 */
+        *u = a * exp(-(r / b) * (r / b));
+        *f = 2.0 * r * (*u) / (b * b);
+    } else if (kind == 4) {   /* Buckingham: u = a e^(-r/b) - c r^-6, f = (a/b) e^(-r/b) - 6 c r^-7 */
+        *u = a * exp(-r / b) - c * pow(r, -6.0);
+        *f = a / b * exp(-r / b) - 6.0 * c * pow(r, -7.0);
+    } else {                  /* Coulomb */
+        *u = a / r;
+        *f = a / (r * r);
+    }
+}
+
+void orc_extra_cut(int kind, double r, double a, double b, double c, double rc, int method, double *u, double *f)
+{
+    double ur, fr, uc, fc;
+    orc_extra_raw(kind, r, a, b, c, &ur, &fr);
+    orc_extra_raw(kind, rc, a, b, c, &uc, &fc);
+    orc_apply_cutoff(method, r, rc, ur, fr, uc, fc, u, f);
+}
+
 /* S5: terms of different kinds on one type pair add; each applies its own rc and its own cutoff method. */
 void orc_pair_sf(const double *p, double r, double *u, double *f)
 {
@@ -153,7 +188,7 @@ void orc_pair_sf(const double *p, double r, double *u, double *f)
         ft += ff;
     }
     if (p[4] > 0.0) {
-        orc_coulomb_cut(r, p[3], p[4], (int)p[6], &uu, &ff);
+        orc_extra_cut((int)p[7], r, p[3], p[8], p[9], p[4], (int)p[6], &uu, &ff);
         ut += uu;
         ft += ff;
     }

@@ -14,8 +14,10 @@
 
 struct PotSlot {
     bool lj = false, coul = false;
-    double eps = 0, sig = 0, rc_lj = 0, qq = 0, rc_c = 0;
+    double eps = 0, sig = 0, rc_lj = 0, qq = 0, rc_c = 0; // qq: prefactor a of the second term
     int cut_lj = 0, cut_c = 0; // rumd_cutoff of each term
+    int kind2 = 0;             // second term: 0 Coulomb, 1 IPL, 2 Yukawa, 3 Gaussian core, 4 Buckingham
+    double b2 = 0, c2 = 0;     // its further parameters
 };
 
 struct GraphCache {
@@ -363,12 +365,20 @@ extern "C" rumd_status rumd_set_pair_potential(rumd_system* s, int ti, int tj, r
             p.rc_lj = params[2];
             p.cut_lj = (int)cutoff;
             if (p.lj && !(p.sig > 0)) return fail(s, RUMD_ERR_INVALID_ARG, "sigma must be > 0");
-        } else if (kind == RUMD_POT_COULOMB) {
-            if (n_params != 2) return fail(s, RUMD_ERR_INVALID_ARG, "Coulomb takes {k*qi*qj, rcut}");
-            p.coul = params[1] > 0.f;
+        } else if (kind == RUMD_POT_COULOMB || kind == RUMD_POT_IPL || kind == RUMD_POT_YUKAWA ||
+                   kind == RUMD_POT_GAUSSIAN_CORE || kind == RUMD_POT_BUCKINGHAM) {
+            const int want = kind == RUMD_POT_COULOMB ? 2 : kind == RUMD_POT_BUCKINGHAM ? 4 : 3;
+            if (n_params != want) return fail(s, RUMD_ERR_INVALID_ARG, "this potential takes %d parameters (see rumd_pot_kind)", want);
+            const float rc = params[want - 1];
+            p.coul = rc > 0.f;
             p.qq = params[0];
-            p.rc_c = params[1];
+            p.rc_c = rc;
             p.cut_c = (int)cutoff;
+            p.kind2 = (int)kind - 1;
+            p.b2 = want >= 3 ? params[1] : 0.0;
+            p.c2 = want >= 4 ? params[2] : 0.0;
+            if (p.coul && (kind == RUMD_POT_YUKAWA || kind == RUMD_POT_GAUSSIAN_CORE || kind == RUMD_POT_BUCKINGHAM) && !(p.b2 > 0))
+                return fail(s, RUMD_ERR_INVALID_ARG, "the length parameter b must be > 0");
         } else
             return fail(s, RUMD_ERR_INVALID_ARG, "unknown potential kind");
     }
@@ -505,12 +515,31 @@ static rumd_status refresh(rumd_system* s)
                 rc = std::max(rc, p.rc_lj);
             }
             if (p.coul) {
-                q.qq = (float)p.qq;
-                q.rc2_c = (float)(p.rc_c * p.rc_c);
-                const double ucc = p.cut_c == RUMD_CUT_NONE ? 0.0 : p.qq / p.rc_c;
-                const double fcc = p.cut_c == RUMD_CUT_SHIFTED_FORCE ? p.qq / (p.rc_c * p.rc_c) : 0.0;
+                // second term at the cutoff, in double: u(rc), f(rc) of the raw potential
+                const double a = p.qq, b = p.b2, c = p.c2, rcc = p.rc_c;
+                double uraw, fraw, p1 = 0.0, p2 = 0.0;
+                switch (p.kind2) {
+                case 1: uraw = a * std::pow(rcc, -b); fraw = b * a * std::pow(rcc, -b - 1.0); p1 = b; break;
+                case 2: uraw = a * std::exp(-rcc / b) / rcc; fraw = uraw * (1.0 / rcc + 1.0 / b); p1 = 1.0 / b; break;
+                case 3: uraw = a * std::exp(-(rcc / b) * (rcc / b)); fraw = 2.0 * rcc * uraw / (b * b); p1 = 1.0 / (b * b); break;
+                case 4:
+                    uraw = a * std::exp(-rcc / b) - c * std::pow(rcc, -6.0);
+                    fraw = a / b * std::exp(-rcc / b) - 6.0 * c * std::pow(rcc, -7.0);
+                    p1 = 1.0 / b;
+                    p2 = c;
+                    break;
+                default: uraw = a / rcc; fraw = a / (rcc * rcc); break;
+                }
+                q.qq = (float)a;
+                q.rc2_c = (float)(rcc * rcc);
+                const double ucc = p.cut_c == RUMD_CUT_NONE ? 0.0 : uraw;
+                const double fcc = p.cut_c == RUMD_CUT_SHIFTED_FORCE ? fraw : 0.0;
                 q.fc_c = (float)fcc;
-                q.k0_c = (float)(ucc + p.rc_c * fcc);
+                q.k0_c = (float)(ucc + rcc * fcc);
+                const int kbits = p.kind2;
+                memcpy(&q.kind2, &kbits, sizeof(int));
+                q.p1 = (float)p1;
+                q.p2 = (float)p2;
                 rc = std::max(rc, p.rc_c);
                 s->any_coul = true;
             }

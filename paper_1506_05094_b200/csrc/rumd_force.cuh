@@ -11,7 +11,11 @@
 // computed for every pair and selected.  1/r^2 = MUFU.RCP(r^2) (1 ulp; the r^-14 force term amplifies it 7-fold
 // to < 1e-6 relative per pair, two orders inside the 1e-4 rms|F| bar) and 1/r = MUFU.RSQ(r^2) (2 ulp; used
 // only in the small shifted-force terms and the Coulomb term): no Newton steps.
-//   pf = (12 c12, 6 c6, rc_lj^2, fc_lj)   pc = (qq, rc_c^2, fc_c, -)   pe = (c12, c6, k0_lj, k0_c)
+//   pf = (12 c12, 6 c6, rc_lj^2, fc_lj)   pc = (a, rc_2^2, fc_2, -)   pe = (c12, c6, k0_lj, k0_2)
+//   px = (-, kind of the second term, p1, p2)
+// The second term (COUL instantiations) is Coulomb a/r or one of the other pair potentials of P:73: IPL
+// a r^-n, Yukawa a exp(-r/b)/r, Gaussian core a exp(-(r/b)^2), Buckingham a exp(-r/b) - c/r^6; the kind is the
+// same for all pairs of one type pair, so the switch diverges only between type pairs.
 __device__ __forceinline__ float __frcp_approx(float x)
 {
     float y;
@@ -20,7 +24,7 @@ __device__ __forceinline__ float __frcp_approx(float x)
 }
 
 template <bool COUL, bool ENERGY>
-__device__ __forceinline__ void pair_accumulate(const float4 pf, const float4 pc, const float4 pe, bool ok,
+__device__ __forceinline__ void pair_accumulate(const float4 pf, const float4 pc, const float4 pe, const float4 px, bool ok,
                                                 float dx, float dy, float dz, float& fx, float& fy, float& fz,
                                                 float& u, float& w)
 {
@@ -40,12 +44,33 @@ __device__ __forceinline__ void pair_accumulate(const float4 pf, const float4 pc
     }
     if (COUL) {
         const bool in_c = ok && r2 < pc.y;
-        const float fc = __fmaf_rn(pc.x * y, rinv2, -pc.z * y); // qq r^-3 - fc / r
-        fr += in_c ? fc : 0.f;
-        if (ENERGY) {
-            const float uc = __fmaf_rn(pc.x, y, __fmaf_rn(pc.z, r, -pe.w)); // qq / r + fc r - k0
-            uu += in_c ? uc : 0.f;
+        float ux, fx_r; // raw u and f / r of the second term
+        switch (__float_as_int(px.y)) {
+        default: // Coulomb: u = a / r
+            ux = pc.x * y;
+            fx_r = ux * rinv2;
+            break;
+        case 1: // inverse power law: u = a r^-n, n = p1
+            ux = pc.x * exp2f(-0.5f * px.z * __log2f(r2));
+            fx_r = px.z * ux * rinv2;
+            break;
+        case 2: // Yukawa: u = a exp(-r / b) / r, p1 = 1 / b;  f = u (1/r + 1/b)
+            ux = pc.x * __expf(-r * px.z) * y;
+            fx_r = ux * (y + px.z) * y;
+            break;
+        case 3: // Gaussian core: u = a exp(-(r/b)^2), p1 = 1 / b^2;  f = 2 r u / b^2
+            ux = pc.x * __expf(-r2 * px.z);
+            fx_r = 2.0f * px.z * ux;
+            break;
+        case 4: { // Buckingham: u = a exp(-r / b) - c r^-6, p1 = 1 / b, p2 = c;  f = (a/b) e^(-r/b) - 6 c r^-7
+            const float e = pc.x * __expf(-r * px.z), c6 = px.w * rinv6;
+            ux = e - c6;
+            fx_r = __fmaf_rn(e * px.z, r, -6.0f * c6) * rinv2;
+            break;
         }
+        }
+        fr += in_c ? __fmaf_rn(-pc.z, y, fx_r) : 0.f;                     // f / r - fc / r
+        if (ENERGY) uu += in_c ? ux + __fmaf_rn(pc.z, r, -pe.w) : 0.f; // u + fc r - k0
     }
     fx = __fmaf_rn(fr, dx, fx);
     fy = __fmaf_rn(fr, dy, fy);
@@ -83,12 +108,13 @@ __device__ __forceinline__ void force_loop(const Sys& S, const float4* r, const 
                                            float& fz, float& u, float& w)
 {
     const int trow = ONE_TYPE ? 0 : 4 * type_of(ri) * S.ntypes;
-    float4 pf, pc, pe;
-    pc = pe = make_float4(0.f, 0.f, 0.f, 0.f);
+    float4 pf, pc, pe, px;
+    pc = pe = px = make_float4(0.f, 0.f, 0.f, 0.f);
     if (ONE_TYPE) {
         pf = s_pp[0];
         if (COUL) pc = s_pp[1];
         if (ENERGY) pe = s_pp[2];
+        if (COUL) px = s_pp[3];
     }
     const float hx = S.h[0], hy = S.h[1], hz = S.h[2];
     const float ix = S.invL[0], iy = S.invL[1], iz = S.invL[2];
@@ -120,8 +146,9 @@ __device__ __forceinline__ void force_loop(const Sys& S, const float4* r, const 
                 pf = s_pp[o];
                 if (COUL) pc = s_pp[o + 1];
                 if (ENERGY) pe = s_pp[o + 2];
+                if (COUL) px = s_pp[o + 3];
             }
-            pair_accumulate<COUL, ENERGY>(pf, pc, pe, ok[q], dx, dy, dz, fx, fy, fz, u, w);
+            pair_accumulate<COUL, ENERGY>(pf, pc, pe, px, ok[q], dx, dy, dz, fx, fy, fz, u, w);
         }
     }
 }
@@ -168,12 +195,13 @@ __device__ __forceinline__ void force_group_all(const Sys& S, const float4* r, c
                                                 float& u, float& w)
 {
     const int trow = ONE_TYPE ? 0 : 4 * type_of(ri) * S.ntypes;
-    float4 pf, pc, pe;
-    pc = pe = make_float4(0.f, 0.f, 0.f, 0.f);
+    float4 pf, pc, pe, px;
+    pc = pe = px = make_float4(0.f, 0.f, 0.f, 0.f);
     if (ONE_TYPE) {
         pf = s_pp[0];
         if (COUL) pc = s_pp[1];
         if (ENERGY) pe = s_pp[2];
+        if (COUL) px = s_pp[3];
     }
     fx = fy = fz = u = w = 0.f;
     const float hx = S.h[0], hy = S.h[1], hz = S.h[2];
@@ -198,8 +226,9 @@ __device__ __forceinline__ void force_group_all(const Sys& S, const float4* r, c
                 pf = s_pp[o];
                 if (COUL) pc = s_pp[o + 1];
                 if (ENERGY) pe = s_pp[o + 2];
+                if (COUL) px = s_pp[o + 3];
             }
-            pair_accumulate<COUL, ENERGY>(pf, pc, pe, ok[q], dx, dy, dz, fx, fy, fz, u, w);
+            pair_accumulate<COUL, ENERGY>(pf, pc, pe, px, ok[q], dx, dy, dz, fx, fy, fz, u, w);
         }
     }
 #pragma unroll

@@ -13,9 +13,10 @@
 //   Coulomb (O4):  u = qq/r, same shift with fc = qq/rc^2, k0 = 2 qq/rc
 struct __align__(16) PairParams {
     float c12x12, c6x6, rc2_lj, fc_lj; // float4 #0: force, LJ term
-    float qq, rc2_c, fc_c, rc2_max;    // float4 #1: force, Coulomb term; rc2_max = max rc^2 of the pair's terms
+    float qq, rc2_c, fc_c, rc2_max;    // float4 #1: force, second term (qq = its prefactor a); rc2_max = max rc^2
     float c12, c6, k0_lj, k0_c;        // float4 #2: energies
-    float rcl2, pad0, pad1, pad2;      // float4 #3: rcl2 = (rc_ab + skin)^2 list cutoff (S4)
+    float rcl2, kind2, p1, p2;         // float4 #3: rcl2 = (rc_ab + skin)^2 list cutoff (S4); second term: kind
+                                       // as int bits (0 Coulomb 1 IPL 2 Yukawa 3 Gaussian core 4 Buckingham), parameters
 };
 
 // Device scalars living in the workspace.

@@ -17,7 +17,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIBPATH = os.environ.get("RUMD_B200_LIB") or os.path.join(_HERE, "librumd_b200.so")  # override: A/B builds
 
 OK, ERR_INVALID_ARG, ERR_NOT_READY, ERR_CUDA, ERR_NBL_OVERFLOW, ERR_BOX_TOO_SMALL, ERR_NONFINITE = range(7)
-POT_LJ_12_6, POT_COULOMB = 0, 1
+POT_LJ_12_6, POT_COULOMB, POT_IPL, POT_YUKAWA, POT_GAUSSIAN_CORE, POT_BUCKINGHAM = range(6)
 CUT_SHIFTED_FORCE, CUT_SHIFTED_POTENTIAL, CUT_NONE = 0, 1, 2
 INT_NVE_LEAPFROG, INT_NVT_NOSE_HOOVER = 0, 1
 NB_N2, NB_CELL, NB_NONE = 0, 1, 2
@@ -171,7 +171,10 @@ class System:
                 if rcl > 0:
                     self.set_pair_potential(a, b, POT_LJ_12_6, [e, sg, rcl], cut_lj)
                 if rcc > 0:
-                    self.set_pair_potential(a, b, POT_COULOMB, [qq, rcc], cut_c)
+                    kind2 = int(pot[a, b, 7]) if pot.shape[-1] >= 10 else 0
+                    pb, pc = (pot[a, b, 8], pot[a, b, 9]) if pot.shape[-1] >= 10 else (0.0, 0.0)
+                    params = {0: [qq, rcc], 4: [qq, pb, pc, rcc]}.get(kind2, [qq, pb, rcc])
+                    self.set_pair_potential(a, b, POT_COULOMB + kind2, params, cut_c)
         self.rc_max = float(max(pot[..., 2].max(), pot[..., 4].max()))
         self.density = self.N / float(np.prod(self.box.astype(np.float64)))
         if capacity is None:

@@ -19,7 +19,8 @@ import numpy as np
 SEED0 = 150605094  # + 1000*config + index-in-sweep
 
 NVE, NVT = 0, 1
-POT_STRIDE = 7  # (epsilon, sigma, rc_LJ, k*qa*qb, rc_Coulomb, cut_LJ, cut_Coulomb); rc <= 0 disables the term
+POT_STRIDE = 10  # (epsilon, sigma, rc_LJ, a, rc_2, cut_LJ, cut_2, kind_2, b, c); rc <= 0 disables the term
+KIND_COULOMB, KIND_IPL, KIND_YUKAWA, KIND_GAUSSIAN_CORE, KIND_BUCKINGHAM = 0, 1, 2, 3, 4  # second term
 CUT_SHIFTED_FORCE, CUT_SHIFTED_POTENTIAL, CUT_NONE = 0, 1, 2
 
 
@@ -124,8 +125,15 @@ def set_lj(pot, a, b, eps, sig, rc, cut=CUT_SHIFTED_FORCE):
 
 
 def set_coulomb(pot, a, b, qq, rc, cut=CUT_SHIFTED_FORCE):
+    set_second_term(pot, a, b, KIND_COULOMB, qq, 0.0, 0.0, rc, cut)
+
+
+def set_second_term(pot, a, b, kind, pa, pb, pc, rc, cut=CUT_SHIFTED_FORCE):
+    """The pair's second term: Coulomb pa/r, IPL pa r^-pb, Yukawa pa exp(-r/pb)/r, Gaussian core pa exp(-(r/pb)^2),
+    Buckingham pa exp(-r/pb) - pc/r^6."""
     for i, j in ((a, b), (b, a)):
-        pot[i, j, 3], pot[i, j, 4], pot[i, j, 6] = f32(qq), f32(rc), float(cut)
+        pot[i, j, 3], pot[i, j, 4], pot[i, j, 6] = f32(pa), f32(rc), float(cut)
+        pot[i, j, 7], pot[i, j, 8], pot[i, j, 9] = float(kind), f32(pb), f32(pc)
 
 
 def lj_single() -> np.ndarray:

@@ -485,6 +485,58 @@ def test_other_cutoff_methods_match_oracle(rumd, kind, kw, cut_lj, cut_c, method
     s.close()
 
 
+def _extra_pot(which):
+    pot = W.pot_table(2)
+    if which == "ipl":          # purely repulsive IPL-12 mixture (no LJ term at all)
+        for (a, b), (amp, rc) in {(0, 0): (1.0, 2.0), (0, 1): (1.3, 1.8), (1, 1): (0.7, 1.9)}.items():
+            W.set_second_term(pot, a, b, W.KIND_IPL, amp, 12.0, 0.0, rc)
+    elif which == "yukawa":     # LJ + screened charges
+        pot = W.kob_andersen()
+        for (a, b), q in {(0, 0): 1.0, (0, 1): -1.0, (1, 1): 1.0}.items():
+            W.set_second_term(pot, a, b, W.KIND_YUKAWA, q, 1.2, 0.0, 3.2)
+    elif which == "gauss":      # Gaussian core, shifted potential
+        for (a, b) in ((0, 0), (0, 1), (1, 1)):
+            W.set_second_term(pot, a, b, W.KIND_GAUSSIAN_CORE, 3.0 + a + b, 0.9, 0.0, 2.6, cut=W.CUT_SHIFTED_POTENTIAL)
+    elif which == "buck":       # Buckingham on unlike pairs, LJ on like pairs
+        W.set_lj(pot, 0, 0, 1.0, 1.0, 2.5)
+        W.set_lj(pot, 1, 1, 0.5, 0.88, 2.2)
+        W.set_second_term(pot, 0, 1, W.KIND_BUCKINGHAM, 2500.0, 0.2, 1.6, 2.4)
+    return pot
+
+
+@pytest.mark.parametrize("which,method,tp,persistent", [("ipl", "cell", 8, 1), ("yukawa", "cell", 4, 1), ("gauss", "n2", 16, 0),
+                                                        ("buck", "cell", 2, 1), ("yukawa", "none", 32, 1)])
+def test_other_pair_potentials_match_oracle(rumd, which, method, tp, persistent):
+    """inverse power law, Yukawa, Gaussian core and Buckingham as the second term of a type pair, on the
+    same kernels: list, forces, energies and virials against the oracle, then a short trajectory."""
+    wl = perturbed(make("ka", N=4096 if method != "none" else 512))
+    wl.pot = _extra_pot(which)
+    s = rumd.from_workload(wl)
+    m = {"n2": rumd.NB_N2, "cell": rumd.NB_CELL, "none": rumd.NB_NONE}[method]
+    s.set_tuning(method=m, tp=tp, pb=max(1, 128 // tp), persistent=persistent, use_graph=0)
+    s.compute_forces()
+    r64, box = wl.r.astype(np.float64), wl.box.astype(np.float64)
+    if method != "none":
+        check_nblist(s, r64, wl.types, box, wl.pot, float(wl.skin))
+    if which == "gauss":        # shifted potential: discontinuous force at rc (S30)
+        F, u, w = oracle.forces_allpairs(r64, wl.types, box, wl.pot)
+        st = s.state()
+        rms = np.sqrt((F * F).sum(1).mean())
+        err = np.sqrt(((st["F"].astype(np.float64) - F) ** 2).sum(1))
+        assert np.sort(err)[-8] <= FORCE_TOL * rms and np.median(err) <= 0.1 * FORCE_TOL * rms
+    else:
+        check_forces(s, r64, wl.types, box, wl.pot)
+    s.run_steps(25)
+    th = s.get_thermo()
+    o = oracle.run(r64, wl.v.astype(np.float64), wl.m.astype(np.float64), np.zeros((wl.N, 3), np.int32), wl.types, box,
+                   wl.pot, float(wl.skin), float(wl.dt), 25, mode=wl.integrator, T0=wl.T0, tau=wl.tau)
+    st = s.state()
+    d = st["r"].astype(np.float64) - o["r"]
+    d -= box * np.rint(d / box)
+    assert np.abs(d).max() < 3e-4 and np.isfinite(th["H"])
+    s.close()
+
+
 def _gas(N, ntypes, box, seed, pot):
     r, types = W.random_gas(N, ntypes, box, seed)
     rng = np.random.default_rng(seed + 1)

@@ -547,7 +547,7 @@ def test_cutoff_methods_closed_forms():
 
 @pytest.mark.parametrize("method", [0, 1, 2])
 def test_cutoff_methods_force_is_minus_gradient(method):
-    rec = np.array([1.5, 0.8, 2.0, -1.0, 3.0, method, method])
+    rec = np.array([1.5, 0.8, 2.0, -1.0, 3.0, method, method, 0, 0, 0])
     h = 1e-6
     for r in (0.8, 1.1, 1.7, 1.95, 2.5, 2.9):
         up, _ = oracle.pair_sf(rec, r + h)
@@ -600,3 +600,72 @@ def test_cutoff_methods_list_forces_equal_brute_force():
     F2, u2, w2 = oracle.forces_list(r.astype(np.float64), t, box, pot, cnt, lst)
     assert np.allclose(F, F2, rtol=1e-12, atol=1e-12) and np.allclose(u, u2, rtol=1e-12) and np.allclose(w, w2, rtol=1e-12)
     assert np.abs(F.sum(0)).max() < 1e-10 * np.abs(F).sum()
+
+
+# ------------------------------------------------------------------ the other pair potentials
+
+
+def test_extra_potentials_closed_forms():
+    """IPL, Yukawa, Gaussian core, Buckingham at points where the value is known in closed form."""
+    # IPL a r^-n: r = 2, n = 12 -> a / 4096; f = n u / r
+    u, f = oracle.extra_raw(1, 2.0, 3.0, 12.0)
+    assert u == pytest.approx(3.0 / 4096.0, rel=1e-14) and f == pytest.approx(12.0 * u / 2.0, rel=1e-14)
+    # IPL with n = 1 is Coulomb
+    assert oracle.extra_raw(1, 1.7, -2.0, 1.0) == pytest.approx(oracle.extra_raw(0, 1.7, -2.0), rel=1e-14)
+    # LJ 12-6 = IPL(4 eps s^12, 12) - IPL(4 eps s^6, 6)
+    eps, sig, r = 1.5, 0.8, 1.1
+    u12, f12 = oracle.extra_raw(1, r, 4 * eps * sig ** 12, 12.0)
+    u6, f6 = oracle.extra_raw(1, r, 4 * eps * sig ** 6, 6.0)
+    assert (u12 - u6, f12 - f6) == pytest.approx(oracle.lj_raw(r, eps, sig), rel=1e-12)
+    # Yukawa at r = b: u = a / (e b), f = 2 u / b; b -> infinity is Coulomb
+    u, f = oracle.extra_raw(2, 0.7, 2.0, 0.7)
+    assert u == pytest.approx(2.0 / (math.e * 0.7), rel=1e-14) and f == pytest.approx(2.0 * u / 0.7, rel=1e-14)
+    assert oracle.extra_raw(2, 1.3, 2.0, 1e12) == pytest.approx(oracle.extra_raw(0, 1.3, 2.0), rel=1e-10)
+    # Gaussian core at r = b: u = a / e, f = 2 u / b; at r = 0+ the force vanishes
+    u, f = oracle.extra_raw(3, 1.5, 4.0, 1.5)
+    assert u == pytest.approx(4.0 / math.e, rel=1e-14) and f == pytest.approx(2.0 * u / 1.5, rel=1e-14)
+    assert oracle.extra_raw(3, 1e-9, 4.0, 1.5)[1] == pytest.approx(0.0, abs=1e-7)
+    # Buckingham = exponential repulsion - dispersion: with a = 0 it is -c r^-6 (an IPL), with c = 0 a pure exponential
+    assert oracle.extra_raw(4, 1.4, 0.0, 0.3, 2.0) == pytest.approx(tuple(-x for x in oracle.extra_raw(1, 1.4, 2.0, 6.0)), rel=1e-13)
+    u, f = oracle.extra_raw(4, 0.6, 50.0, 0.3, 0.0)
+    assert u == pytest.approx(50.0 * math.exp(-2.0), rel=1e-14) and f == pytest.approx(u / 0.3, rel=1e-14)
+
+
+@pytest.mark.parametrize("kind,a,b,c", [(1, 1.3, 9.0, 0.0), (1, 2.0, 18.0, 0.0), (2, -1.5, 0.9, 0.0), (3, 3.0, 1.2, 0.0),
+                                        (4, 800.0, 0.27, 1.9)])
+@pytest.mark.parametrize("method", [0, 1, 2])
+def test_extra_potentials_force_is_minus_gradient_and_cutoffs(kind, a, b, c, method):
+    rc, h = 2.4, 1e-6
+    rec = np.array([0.0, 0.0, 0.0, a, rc, 0, method, kind, b, c])
+    for r in (0.85, 1.2, 1.9, 2.39):
+        up, _ = oracle.pair_sf(rec, r + h)
+        um, _ = oracle.pair_sf(rec, r - h)
+        _, f = oracle.pair_sf(rec, r)
+        assert f == pytest.approx(-(up - um) / (2 * h), rel=3e-7, abs=1e-9)
+    assert oracle.pair_sf(rec, rc) == (0.0, 0.0) and oracle.pair_sf(rec, 3.0) == (0.0, 0.0)
+    ur, fr = oracle.extra_raw(kind, 1.3, a, b, c)
+    uc, fc = oracle.extra_raw(kind, rc, a, b, c)
+    want = {0: (ur - uc + (1.3 - rc) * fc, fr - fc), 1: (ur - uc, fr), 2: (ur, fr)}[method]
+    assert oracle.pair_sf(rec, 1.3) == pytest.approx(want, rel=1e-13)
+
+
+def test_extra_potentials_list_forces_equal_brute_force_and_newton():
+    pot = W.pot_table(2)
+    W.set_lj(pot, 0, 0, 1.0, 1.0, 2.5)
+    W.set_second_term(pot, 0, 0, W.KIND_YUKAWA, 1.2, 0.8, 0.0, 3.0)
+    W.set_second_term(pot, 0, 1, W.KIND_BUCKINGHAM, 900.0, 0.28, 1.5, 2.6, cut=W.CUT_SHIFTED_POTENTIAL)
+    W.set_second_term(pot, 1, 1, W.KIND_IPL, 1.0, 12.0, 0.0, 2.0)
+    r, t = W.random_gas(216, 2, (8.5, 8.5, 9.5), 3)
+    box = np.array([8.5, 8.5, 9.5])
+    r64 = r.astype(np.float64)
+    F, u, w = oracle.forces_allpairs(r64, t, box, pot)
+    cnt, lst = oracle.nblist(r64, t, box, pot, 0.35)
+    F2, u2, w2 = oracle.forces_list(r64, t, box, pot, cnt, lst)
+    assert np.allclose(F, F2, rtol=1e-12, atol=1e-12) and np.allclose(u, u2, rtol=1e-12) and np.allclose(w, w2, rtol=1e-12)
+    assert np.abs(F.sum(0)).max() < 1e-10 * np.abs(F).sum()
+    # virial = -dU/d(ln scale): uniform dilation (as in P5)
+    lam = 1e-6
+    Up = oracle.forces_allpairs(r64 * (1 + lam), t, box * (1 + lam), pot)[1].sum()
+    Um = oracle.forces_allpairs(r64 * (1 - lam), t, box * (1 - lam), pot)[1].sum()
+    # only valid for continuous energies: the shifted-potential AB term is continuous in u, fine
+    assert (Up - Um) / (2 * lam) == pytest.approx(-w.sum(), rel=2e-5)
