@@ -1,20 +1,25 @@
 """Build librumd_b200.so in-tree with nvcc for sm_100a (cross-compiles without a GPU).
 
-    python -m paper_1506_05094_b200.build [--force]
+    python -m paper_1506_05094_b200.build [--force] [-v]
+
+The kernels templated on threads-per-particle live in one translation unit per tp (csrc/rumd_inst_tp*.cu); the
+seven translation units are compiled in parallel and linked into one shared library.
 """
 from __future__ import annotations
 
 import os
 import subprocess
 import sys
+from concurrent.futures import ThreadPoolExecutor
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
+OBJDIR = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "librumd_b200.so")
-SOURCES = ["rumd_b200.cu"]
-HEADERS = ["rumd_types.cuh", "rumd_kernels.cuh", "rumd_force.cuh", "rumd_persist.cuh", "../../include/rumd_b200.h"]
-NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-              "-Xcompiler", "-fPIC", "-shared"]
+SOURCES = ["rumd_b200.cu"] + ["rumd_inst_tp%d.cu" % tp for tp in (1, 2, 4, 8, 16, 32)]
+HEADERS = ["rumd_types.cuh", "rumd_kernels.cuh", "rumd_force.cuh", "rumd_persist.cuh", "rumd_ensemble.cuh",
+           "rumd_dispatch.cuh", "rumd_inst.cuh", "../../include/rumd_b200.h"]
+NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC"]
 
 
 def _nvcc() -> str:
@@ -32,14 +37,24 @@ def up_to_date() -> bool:
     return all(os.path.getmtime(d) <= t for d in deps)
 
 
+def _compile(src: str, verbose: bool) -> str:
+    obj = os.path.join(OBJDIR, os.path.splitext(src)[0] + ".%d.o" % os.getpid())
+    cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", "-o", obj, os.path.join(CSRC, src)]
+    subprocess.check_call(cmd)
+    return obj
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and up_to_date():
         return LIB
+    os.makedirs(OBJDIR, exist_ok=True)
+    with ThreadPoolExecutor(max_workers=len(SOURCES)) as pool:
+        objs = list(pool.map(lambda src: _compile(src, verbose), SOURCES))
     tmp = LIB + ".tmp%d" % os.getpid()
-    cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + \
-          [os.path.join(CSRC, f) for f in SOURCES]
-    subprocess.check_call(cmd)
+    subprocess.check_call([_nvcc(), "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", tmp] + objs)
     os.replace(tmp, LIB)
+    for o in objs:
+        os.remove(o)
     return LIB
 
 

@@ -1,6 +1,7 @@
 // rumd_b200.cu -- host side of librumd_b200.so: C ABI (include/rumd_b200.h), workspace carving, launch
 // chains, whole-timestep CUDA graphs and the Blackwell autotuner.  Product code: shares nothing with oracle/.
 #include "../../include/rumd_b200.h"
+#include "rumd_dispatch.cuh"
 #include "rumd_persist.cuh"
 #include "rumd_ensemble.cuh"
 
@@ -38,7 +39,7 @@ struct rumd_system {
     bool state_bound = false, ws_bound = false, integ_set = false;
     bool params_dirty = true;
     PotSlot pot[RUMD_MAXT][RUMD_MAXT];
-    bool any_coul = false;
+    bool any_coul = false, any_generic = false; // a second term is set / one of them is not Coulomb
     int integ = 0;
     float dt = 0, T0 = 0, tau = 0;
     rumd_tuning tune;
@@ -492,6 +493,7 @@ static rumd_status refresh(rumd_system* s)
         S.build_tp_shift = ilog2(btp);
     }
     s->any_coul = false;
+    s->any_generic = false;
     memset(S.pp, 0, sizeof S.pp);
     for (int a = 0; a < s->ntypes; ++a)
         for (int b = 0; b < s->ntypes; ++b) {
@@ -542,6 +544,7 @@ static rumd_status refresh(rumd_system* s)
                 q.p2 = (float)p2;
                 rc = std::max(rc, p.rc_c);
                 s->any_coul = true;
+                if (p.kind2 != 0) s->any_generic = true;
             }
             q.rcl2 = (float)((rc + skin) * (rc + skin));
             q.rc2_max = (float)(rc * rc);
@@ -619,65 +622,41 @@ static rumd_status refresh(rumd_system* s)
 
 // ---------------------------------------------------------------------------------------------- launch chains
 
-// Kernel selection over (TP, COUL, ONE_TYPE); UNROLL follows TP (wide groups have few iterations per lane).
-// Listed pairs in flight per lane (the paper's one-ahead prefetch, P:108 item 4, generalised).  Measured on
-// B200 (2 / 4 / 8 / 16 per lane): 8 is best while a lane has >= ~10 entries, 4 for the wide groups.
-template <int TP> struct UnrollOf { static constexpr int value = TP >= 16 ? 4 : 8; };
-
-template <template <int, bool, bool> class F, int TP, typename... A>
-static auto pick_flags(rumd_system* s, A... a)
-{
-    const bool one = s->ntypes == 1;
-    if (s->any_coul) return one ? F<TP, true, true>::run(s, a...) : F<TP, true, false>::run(s, a...);
-    return one ? F<TP, false, true>::run(s, a...) : F<TP, false, false>::run(s, a...);
-}
-
-template <template <int, bool, bool> class F, typename... A>
-static auto pick_kernel(rumd_system* s, A... a)
+// Kernel selection over (tp, second-term kind, one type): the instantiations live in one translation unit per tp
+// (rumd_inst_tp*.cu, built in parallel) and are reached through their KernelSet.
+static const KernelSet* kernels_of(const rumd_system* s)
 {
     switch (s->tune.tp) {
-    case 1: return pick_flags<F, 1>(s, a...);
-    case 2: return pick_flags<F, 2>(s, a...);
-    case 4: return pick_flags<F, 4>(s, a...);
-    case 8: return pick_flags<F, 8>(s, a...);
-    case 16: return pick_flags<F, 16>(s, a...);
-    default: return pick_flags<F, 32>(s, a...);
+    case 1: return rumd_kernels_tp1();
+    case 2: return rumd_kernels_tp2();
+    case 4: return rumd_kernels_tp4();
+    case 8: return rumd_kernels_tp8();
+    case 16: return rumd_kernels_tp16();
+    default: return rumd_kernels_tp32();
     }
 }
-
-template <int TP, bool COUL, bool ONE> struct ForceLaunch {
-    static int run(rumd_system* s, int nblocks, int nthreads)
-    {
-        k_force<TP, COUL, ONE, UnrollOf<TP>::value><<<nblocks, nthreads, 0, s->stream>>>(s->S);
-        return 1;
-    }
-};
+// second term of the pair potentials: 0 none, 1 Coulomb only (the hot path of configs[4]), 2 any kind of P:73
+static int coul_of(const rumd_system* s) { return s->any_coul ? (s->any_generic ? 2 : 1) : 0; }
+static bool one_of(const rumd_system* s) { return s->ntypes == 1; }
 
 static int launch_force(rumd_system* s)
 {
     const int tp = s->tune.tp, nthreads = s->tune.pb * tp;
     const int nblocks = (int)(((size_t)s->N * tp + nthreads - 1) / nthreads);
-    return pick_kernel<ForceLaunch>(s, nblocks, nthreads);
+    kernels_of(s)->force(coul_of(s), one_of(s), s->S, nblocks, nthreads, s->stream);
+    return 1;
 }
 
-// A7, persistent form: the address of the k_persist instantiation for the current tuning.
-template <int TP, bool COUL, bool ONE> struct PersistKernel {
-    static const void* run(rumd_system*) { return (const void*)&k_persist<TP, COUL, ONE, UnrollOf<TP>::value>; }
-};
-
 static int persist_threads_of(const rumd_tuning&) { return PERSIST_THREADS; }
-
-template <int TP, bool COUL, bool ONE> struct EnsembleKernel {
-    static const void* run(rumd_system*) { return (const void*)&k_ensemble<TP, COUL, ONE, UnrollOf<TP>::value>; }
-};
 
 // n steps in ONE cooperative launch.  The grid is sized to cover N*tp virtual threads when it can be
 // co-resident, else to the co-residency limit (the kernel strides).
 static rumd_status launch_persistent(rumd_system* s, int nsteps)
 {
-    const void* fn = pick_kernel<PersistKernel>(s);
+    const void* fn = kernels_of(s)->persist[coul_of(s)][one_of(s) ? 1 : 0];
     const int threads = persist_threads_of(s->tune);
-    const int sig = s->tune.tp * 4096 + threads + (s->any_coul ? 1 << 20 : 0) + (s->ntypes == 1 ? 1 << 21 : 0);
+    const int sig = s->tune.tp * 4096 + threads + (s->any_coul ? 1 << 20 : 0) + (s->ntypes == 1 ? 1 << 21 : 0) +
+                    (s->any_generic ? 1 << 22 : 0);
     if (sig != s->persist_grid_for) {
         int per_sm = 0;
         CUDA_TRY(s, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, threads, 0));
@@ -736,19 +715,6 @@ static int launch_rebuild_chain(rumd_system* s)
         k_build_n2<<<std::min((s->N + 3) / 4, cap128), 128, 0, s->stream>>>(S);
     return n + 1;
 }
-
-// fused force + integrate step of the per-step path: positions go from `from_alt ? r_alt : r` to the other buffer
-template <int TP, bool COUL, bool ONE> struct StepLaunch {
-    static int run(rumd_system* s, int nblocks, int nthreads, const Sys* S, int energy)
-    {
-        const int nvt = s->integ == RUMD_INT_NVT_NOSE_HOOVER;
-        if (energy)
-            k_step<TP, COUL, ONE, UnrollOf<TP>::value, true><<<nblocks, nthreads, 0, s->stream>>>(*S, nvt);
-        else
-            k_step<TP, COUL, ONE, UnrollOf<TP>::value, false><<<nblocks, nthreads, 0, s->stream>>>(*S, nvt);
-        return 1;
-    }
-};
 
 static int launch_integrate(rumd_system* s)
 {
@@ -814,12 +780,15 @@ static int launch_step_pair(rumd_system* s, bool energy_on_second)
     B.r = s->S.r_alt;
     B.r_out = s->S.r;
     int n = launch_rebuild_chain(s);
-    n += pick_kernel<StepLaunch>(s, nblocks, nthreads, (const Sys*)&A, 0);
+    const int nvt = s->integ == RUMD_INT_NVT_NOSE_HOOVER;
+    kernels_of(s)->step(coul_of(s), one_of(s), false, nvt, A, nblocks, nthreads, s->stream);
+    n += 1;
     const Sys keep = s->S;
     s->S = B; // the chain launchers read s->S
     n += launch_rebuild_chain(s);
     s->S = keep;
-    n += pick_kernel<StepLaunch>(s, nblocks, nthreads, (const Sys*)&B, energy_on_second ? 1 : 0);
+    kernels_of(s)->step(coul_of(s), one_of(s), energy_on_second, nvt, B, nblocks, nthreads, s->stream);
+    n += 1;
     return n;
 }
 
@@ -860,7 +829,8 @@ extern "C" rumd_status rumd_run_steps(rumd_system* s, long n)
             int chunk = (int)std::min<long>(left, 1L << 20);
             int nvt = s->integ == RUMD_INT_NVT_NOSE_HOOVER;
             void* args[] = {(void*)&s->d_systems, (void*)&chunk, (void*)&nvt};
-            CUDA_TRY(s, cudaLaunchKernel(pick_kernel<EnsembleKernel>(s), dim3(s->nrep), dim3(ENS_THREADS), args, 0, s->stream));
+            CUDA_TRY(s, cudaLaunchKernel(kernels_of(s)->ensemble[coul_of(s)][one_of(s) ? 1 : 0], dim3(s->nrep), dim3(ENS_THREADS), args, 0,
+                                         s->stream));
             s->launches += 1;
             left -= chunk;
         }

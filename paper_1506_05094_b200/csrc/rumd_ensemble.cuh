@@ -18,7 +18,7 @@
 
 #define ENS_THREADS 256
 
-__global__ void k_ens_reset(DevScalars* sc, int nrep)
+static __global__ void k_ens_reset(DevScalars* sc, int nrep)
 {
     const int q = blockIdx.x * blockDim.x + threadIdx.x;
     if (q >= nrep) return;
@@ -28,7 +28,7 @@ __global__ void k_ens_reset(DevScalars* sc, int nrep)
     sc[q] = z;
 }
 
-__global__ void k_ens_request_rebuild(DevScalars* sc, int nrep)
+static __global__ void k_ens_request_rebuild(DevScalars* sc, int nrep)
 {
     const int q = blockIdx.x * blockDim.x + threadIdx.x;
     if (q < nrep) sc[q].flag = 1u;
@@ -48,7 +48,7 @@ __device__ __forceinline__ double ens_block_sum(double x, double* s)
     return a;
 }
 
-template <int TP, bool COUL, bool ONE_TYPE, int UNROLL>
+template <int TP, int COUL, bool ONE_TYPE, int UNROLL>
 __global__ void __launch_bounds__(ENS_THREADS, 3) k_ensemble(const Sys* __restrict__ systems, const int nsteps, const int nvt)
 {
     __shared__ Sys R; // this replica's parameter block

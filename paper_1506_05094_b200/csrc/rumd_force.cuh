@@ -23,7 +23,7 @@ __device__ __forceinline__ float __frcp_approx(float x)
     return y;
 }
 
-template <bool COUL, bool ENERGY>
+template <int COUL, bool ENERGY>
 __device__ __forceinline__ void pair_accumulate(const float4 pf, const float4 pc, const float4 pe, const float4 px, bool ok,
                                                 float dx, float dy, float dz, float& fx, float& fy, float& fz,
                                                 float& u, float& w)
@@ -45,7 +45,7 @@ __device__ __forceinline__ void pair_accumulate(const float4 pf, const float4 pc
     if (COUL) {
         const bool in_c = ok && r2 < pc.y;
         float ux, fx_r; // raw u and f / r of the second term
-        switch (__float_as_int(px.y)) {
+        switch (COUL == 1 ? 0 : __float_as_int(px.y)) { // COUL == 1: every second term is Coulomb, no switch
         default: // Coulomb: u = a / r
             ux = pc.x * y;
             fx_r = ux * rinv2;
@@ -102,7 +102,7 @@ __device__ __forceinline__ void pair_accumulate(const float4 pf, const float4 pc
 template <bool NC> __device__ __forceinline__ int load_idx(const int* p) { return NC ? __ldg(p) : __ldcs(p); }
 template <bool NC> __device__ __forceinline__ float4 load_pos(const float4* p) { return NC ? __ldg(p) : *p; }
 
-template <int TP, bool COUL, bool ONE_TYPE, int UNROLL, bool NC, bool ENERGY, bool WRAP, bool MASKED>
+template <int TP, int COUL, bool ONE_TYPE, int UNROLL, bool NC, bool ENERGY, bool WRAP, bool MASKED>
 __device__ __forceinline__ void force_loop(const Sys& S, const float4* r, const float4* s_pp, const int* base,
                                            int it_begin, int nit, int it_end, const float4 ri, float& fx, float& fy,
                                            float& fz, float& u, float& w)
@@ -114,7 +114,7 @@ __device__ __forceinline__ void force_loop(const Sys& S, const float4* r, const 
         pf = s_pp[0];
         if (COUL) pc = s_pp[1];
         if (ENERGY) pe = s_pp[2];
-        if (COUL) px = s_pp[3];
+        if (COUL == 2) px = s_pp[3];
     }
     const float hx = S.h[0], hy = S.h[1], hz = S.h[2];
     const float ix = S.invL[0], iy = S.invL[1], iz = S.invL[2];
@@ -146,14 +146,14 @@ __device__ __forceinline__ void force_loop(const Sys& S, const float4* r, const 
                 pf = s_pp[o];
                 if (COUL) pc = s_pp[o + 1];
                 if (ENERGY) pe = s_pp[o + 2];
-                if (COUL) px = s_pp[o + 3];
+                if (COUL == 2) px = s_pp[o + 3];
             }
             pair_accumulate<COUL, ENERGY>(pf, pc, pe, px, ok[q], dx, dy, dz, fx, fy, fz, u, w);
         }
     }
 }
 
-template <int TP, bool COUL, bool ONE_TYPE, int UNROLL, bool NC, bool ENERGY>
+template <int TP, int COUL, bool ONE_TYPE, int UNROLL, bool NC, bool ENERGY>
 __device__ __forceinline__ void force_group(const Sys& S, const float4* r, const float4* s_pp, int vwarp, int i,
                                             int t, bool have_i, const float4 ri, int cnt, float& fx, float& fy,
                                             float& fz, float& u, float& w)
@@ -189,7 +189,7 @@ __device__ __forceinline__ void force_group(const Sys& S, const float4* r, const
 // P:371 "none" method: no neighbour list, lane t of the particle's TP lanes takes particles j = t, t + TP, ...
 // of the WHOLE system (coalesced position loads), exact minimum image for every pair, self pair masked.  O(N^2)
 // pair evaluations per step, but no list, no rebuilds and no index stream: wins for the smallest systems.
-template <int TP, bool COUL, bool ONE_TYPE, bool NC, bool ENERGY>
+template <int TP, int COUL, bool ONE_TYPE, bool NC, bool ENERGY>
 __device__ __forceinline__ void force_group_all(const Sys& S, const float4* r, const float4* s_pp, int i, int t,
                                                 bool have_i, const float4 ri, float& fx, float& fy, float& fz,
                                                 float& u, float& w)
@@ -201,7 +201,7 @@ __device__ __forceinline__ void force_group_all(const Sys& S, const float4* r, c
         pf = s_pp[0];
         if (COUL) pc = s_pp[1];
         if (ENERGY) pe = s_pp[2];
-        if (COUL) px = s_pp[3];
+        if (COUL == 2) px = s_pp[3];
     }
     fx = fy = fz = u = w = 0.f;
     const float hx = S.h[0], hy = S.h[1], hz = S.h[2];
@@ -226,7 +226,7 @@ __device__ __forceinline__ void force_group_all(const Sys& S, const float4* r, c
                 pf = s_pp[o];
                 if (COUL) pc = s_pp[o + 1];
                 if (ENERGY) pe = s_pp[o + 2];
-                if (COUL) px = s_pp[o + 3];
+                if (COUL == 2) px = s_pp[o + 3];
             }
             pair_accumulate<COUL, ENERGY>(pf, pc, pe, px, ok[q], dx, dy, dz, fx, fy, fz, u, w);
         }
@@ -244,7 +244,7 @@ __device__ __forceinline__ void force_group_all(const Sys& S, const float4* r, c
 }
 
 // forces of one particle by whichever method is configured (warp-uniform choice)
-template <int TP, bool COUL, bool ONE_TYPE, int UNROLL, bool NC, bool ENERGY>
+template <int TP, int COUL, bool ONE_TYPE, int UNROLL, bool NC, bool ENERGY>
 __device__ __forceinline__ void force_any(const Sys& S, const float4* r, const float4* s_pp, int vwarp, int i, int t,
                                           bool have_i, const float4 ri, int cnt, float& fx, float& fy, float& fz,
                                           float& u, float& w)
@@ -275,7 +275,7 @@ __device__ __forceinline__ void finish_rebuild(const Sys& S)
     }
 }
 
-template <int TP, bool COUL, bool ONE_TYPE, int UNROLL>
+template <int TP, int COUL, bool ONE_TYPE, int UNROLL>
 __global__ void __launch_bounds__(1024, 1) k_force(const Sys S)
 {
     __shared__ float4 s_pp[4 * RUMD_MAXT * RUMD_MAXT];
@@ -427,7 +427,7 @@ __device__ __forceinline__ void step_tail(const Sys& S, bool nvt, double kt, dou
 }
 
 #define INT_THREADS 128
-__global__ void __launch_bounds__(INT_THREADS) k_integrate(const Sys S, int nvt)
+static __global__ void __launch_bounds__(INT_THREADS) k_integrate(const Sys S, int nvt)
 {
     float a, b;
     nvt_factors(S, nvt != 0, a, b);
@@ -449,7 +449,7 @@ __global__ void __launch_bounds__(INT_THREADS) k_integrate(const Sys S, int nvt)
 // (the OTHER position buffer: nobody reads a position that was already advanced), then the same block tail as
 // k_integrate.  Saves the integrator's pass over r, v, f (~112 B per particle) and one launch per step.
 // ENERGY: also write f, u, w (the step whose force evaluation is an output of the run).
-template <int TP, bool COUL, bool ONE_TYPE, int UNROLL, bool ENERGY>
+template <int TP, int COUL, bool ONE_TYPE, int UNROLL, bool ENERGY>
 __global__ void __launch_bounds__(1024, 1) k_step(const Sys S, int nvt)
 {
     __shared__ float4 s_pp[4 * RUMD_MAXT * RUMD_MAXT];
@@ -490,7 +490,7 @@ __global__ void __launch_bounds__(1024, 1) k_step(const Sys S, int nvt)
 
 // ------------------------------------------------------------------------------------------ small kernels
 
-__global__ void k_request_rebuild(const Sys S)
+static __global__ void k_request_rebuild(const Sys S)
 {
     S.sc->flag = 1u;
     S.sc->pending = 0u;
@@ -498,7 +498,7 @@ __global__ void k_request_rebuild(const Sys S)
     S.sc->overflow = 0u;
 }
 
-__global__ void k_reset_scalars(const Sys S)
+static __global__ void k_reset_scalars(const Sys S)
 {
     DevScalars z;
     memset(&z, 0, sizeof(z));
@@ -507,7 +507,7 @@ __global__ void k_reset_scalars(const Sys S)
 }
 
 // U = sum u_i, W = sum w_i in fp64, fixed order (single block).
-__global__ void __launch_bounds__(1024) k_thermo(const Sys S)
+static __global__ void __launch_bounds__(1024) k_thermo(const Sys S)
 {
     __shared__ double s_u[32], s_w[32];
     double u = 0.0, w = 0.0;
@@ -536,7 +536,7 @@ __global__ void __launch_bounds__(1024) k_thermo(const Sys S)
 }
 
 // Row-major export of the tiled list (inspection / parity tests).
-__global__ void k_export_nbl(const Sys S, int* count, int* list, int rowcap)
+static __global__ void k_export_nbl(const Sys S, int* count, int* list, int rowcap)
 {
     const int i = blockIdx.x;
     const int c = S.method == 2 ? 0 : S.num_nbrs[i]; // the "none" method keeps no list
@@ -546,7 +546,7 @@ __global__ void k_export_nbl(const Sys S, int* count, int* list, int rowcap)
 }
 
 // snapshot / restore of (r, v, image, id)
-__global__ void k_copy_state(int N, const float4* r, const float4* v, const int4* im, const int* id, float4* r2,
+static __global__ void k_copy_state(int N, const float4* r, const float4* v, const int4* im, const int* id, float4* r2,
                              float4* v2, int4* im2, int* id2)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;

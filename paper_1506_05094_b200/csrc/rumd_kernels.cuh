@@ -471,7 +471,7 @@ __device__ __forceinline__ void build_cell_dispatch(const Sys& S, const float4* 
 
 __device__ __forceinline__ int* max_slot_of(const Sys& S) { return &S.sc->max_nbrs[S.sc->n_rebuilds & 1]; }
 
-__global__ void __launch_bounds__(128) k_build_n2(const Sys S)
+static __global__ void __launch_bounds__(128) k_build_n2(const Sys S)
 {
     if (!rebuild_requested(S)) return;
     __shared__ float4 tile[N2_TILE];
@@ -481,7 +481,7 @@ __global__ void __launch_bounds__(128) k_build_n2(const Sys S)
     ph_build_n2(S, S.r, tile, s_rcl2, blockIdx.x, gridDim.x, max_slot_of(S));
 }
 
-__global__ void __launch_bounds__(128) k_build_cell(const Sys S)
+static __global__ void __launch_bounds__(128) k_build_cell(const Sys S)
 {
     if (!rebuild_requested(S)) return;
     __shared__ float s_rcl2[RUMD_MAXT * RUMD_MAXT];
@@ -491,63 +491,63 @@ __global__ void __launch_bounds__(128) k_build_cell(const Sys S)
     build_cell_dispatch(S, S.r, s_rcl2, first, stride, max_slot_of(S));
 }
 
-__global__ void k_cell_assign(const Sys S)
+static __global__ void k_cell_assign(const Sys S)
 {
     if (!sort_requested(S)) return;
     VGRID;
     ph_cell_assign(S, S.r, first, stride);
 }
 
-__global__ void __launch_bounds__(SCAN_THREADS) k_scan_sums(const Sys S)
+static __global__ void __launch_bounds__(SCAN_THREADS) k_scan_sums(const Sys S)
 {
     if (!sort_requested(S)) return;
     __shared__ int s_warp[33];
     ph_scan_sums(S, s_warp, blockIdx.x, gridDim.x);
 }
 
-__global__ void __launch_bounds__(SCAN_THREADS) k_scan_blocks(const Sys S)
+static __global__ void __launch_bounds__(SCAN_THREADS) k_scan_blocks(const Sys S)
 {
     if (!sort_requested(S)) return;
     __shared__ int s_warp[33];
     ph_scan_blocks(S, s_warp);
 }
 
-__global__ void __launch_bounds__(SCAN_THREADS) k_scan_apply(const Sys S)
+static __global__ void __launch_bounds__(SCAN_THREADS) k_scan_apply(const Sys S)
 {
     if (!sort_requested(S)) return;
     __shared__ int s_warp[33];
     ph_scan_apply(S, s_warp, blockIdx.x, gridDim.x);
 }
 
-__global__ void __launch_bounds__(SCAN_THREADS) k_scan_single(const Sys S)
+static __global__ void __launch_bounds__(SCAN_THREADS) k_scan_single(const Sys S)
 {
     if (!sort_requested(S)) return;
     __shared__ int s_warp[33];
     ph_scan_single_block(S, s_warp);
 }
 
-__global__ void k_cell_scatter(const Sys S)
+static __global__ void k_cell_scatter(const Sys S)
 {
     if (!sort_requested(S)) return;
     VGRID;
     ph_cell_scatter(S, first, stride);
 }
 
-__global__ void k_cell_finish(const Sys S)
+static __global__ void k_cell_finish(const Sys S)
 {
     if (!sort_requested(S)) return;
     VGRID;
     ph_cell_finish(S, first, stride);
 }
 
-__global__ void k_permute_gather(const Sys S)
+static __global__ void k_permute_gather(const Sys S)
 {
     if (!sort_requested(S)) return;
     VGRID;
     ph_permute_gather(S, S.r, first, stride);
 }
 
-__global__ void k_permute_store(const Sys S)
+static __global__ void k_permute_store(const Sys S)
 {
     if (!sort_requested(S)) return;
     VGRID;

@@ -84,7 +84,7 @@ __device__ __forceinline__ double warp_sum_partials(const double* p, int n)
     return warp_sum(a);
 }
 
-template <int TP, bool COUL, bool ONE_TYPE, int UNROLL>
+template <int TP, int COUL, bool ONE_TYPE, int UNROLL>
 __global__ void __launch_bounds__(PERSIST_THREADS, PERSIST_MINB) k_persist(const Sys S, const int nsteps, const int nvt)
 {
     __shared__ float4 s_pp[4 * RUMD_MAXT * RUMD_MAXT];
