@@ -395,6 +395,8 @@ __device__ __forceinline__ void ph_build_cell(const Sys& S, const float4* r, con
         // this particle's row of the tiled list: entry k at rowbase[(k >> tp_shift) * 32 + (k & (tp - 1))]
         int* rowbase = S.nbl + ((size_t)(i >> S.ppw_shift) * S.cap_it * 32 + ((i & ((1 << S.ppw_shift) - 1)) << S.tp_shift));
         const int tmask = (1 << S.tp_shift) - 1;
+        // list cutoffs of this particle's type against every type (S4), held in registers
+        const float c0 = s_rcl2[trow], c1 = s_rcl2[trow + 1], c2 = s_rcl2[trow + 2], c3 = s_rcl2[trow + 3];
         int2 na, nb;
         float nsy, nsz;
         ranges_of(l, na, nb, nsy, nsz);
@@ -402,40 +404,45 @@ __device__ __forceinline__ void ph_build_cell(const Sys& S, const float4* r, con
             const int2 a = na, b = nb;
             const float syh = nsy, szh = nsz;
             if (q0 + G < 25) ranges_of(q0 + G + l, na, nb, nsy, nsz); // one-ahead prefetch of the next round's ranges
-            const int n0 = a.y - a.x, n = n0 + (b.y - b.x);
-            const int nmax = __reduce_max_sync(FULLMASK, n);
-            const float ay = ri.y - syh, az = ri.z - szh, axw = ri.x - sxh;
-            constexpr int U = 4; // candidates in flight per lane
-            for (int it0 = 0; it0 < nmax; it0 += U) {
-                float4 rj[U];
-                int j[U];
+            const float ay = ri.y - syh, az = ri.z - szh;
+            // the main piece of the row, then its x-wrapped piece (empty except next to the x faces)
 #pragma unroll
-                for (int q = 0; q < U; ++q) {
-                    const int it = it0 + q;
-                    j[q] = it < n0 ? a.x + it : b.x + (it - n0);
-                    if (it >= n) j[q] = i; // masked: gather the particle itself (always valid when n > 0)
-                    if (!have_i) j[q] = 0;
-                    rj[q] = r[j[q]];
-                }
+            for (int piece = 0; piece < 2; ++piece) {
+                const int start = piece == 0 ? a.x : b.x;
+                const int n = piece == 0 ? a.y - a.x : b.y - b.x;
+                const int nmax = __reduce_max_sync(FULLMASK, n);
+                const float shx = piece == 0 ? 0.f : sxh;
+                const float ax = ri.x - shx;
+                constexpr int U = 4; // candidates in flight per lane
+                for (int it0 = 0; it0 < nmax; it0 += U) {
+                    float4 rj[U];
+                    int j[U];
 #pragma unroll
-                for (int q = 0; q < U; ++q) {
-                    const bool inwrap = it0 + q >= n0;
-                    const float dx = inwrap ? axw - (rj[q].x + sxh) : ri.x - rj[q].x;
-                    const float dy = ay - (rj[q].y + syh), dz = az - (rj[q].z + szh);
-                    const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, dx * dx));
-                    const bool acc = have_i && j[q] != i && d2 < s_rcl2[trow + type_of(rj[q])];
-                    if (G == 1) { // the lane owns the row: no slot negotiation
-                        if (acc) {
-                            if (count < S.cap) rowbase[((count >> S.tp_shift) << 5) + (count & tmask)] = j[q];
-                            ++count;
+                    for (int q = 0; q < U; ++q) {
+                        j[q] = it0 + q < n ? start + it0 + q : i; // masked: gather the particle itself (n > 0 => have_i)
+                        rj[q] = r[have_i ? j[q] : 0];
+                    }
+#pragma unroll
+                    for (int q = 0; q < U; ++q) {
+                        const float dx = piece == 0 ? ri.x - rj[q].x : ax - (rj[q].x + shx);
+                        const float dy = ay - (rj[q].y + syh), dz = az - (rj[q].z + szh);
+                        const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, dx * dx));
+                        const int tj = type_of(rj[q]);
+                        const float thr = S.ntypes <= 2 ? (tj ? c1 : c0) : (tj == 0 ? c0 : tj == 1 ? c1 : tj == 2 ? c2 : c3);
+                        const bool acc = have_i && j[q] != i && d2 < thr;
+                        if (G == 1) { // the lane owns the row: no slot negotiation
+                            if (acc) {
+                                if (count < S.cap) rowbase[((count >> S.tp_shift) << 5) + (count & tmask)] = j[q];
+                                ++count;
+                            }
+                        } else {
+                            const unsigned m = __ballot_sync(FULLMASK, acc);
+                            if (acc) {
+                                const int k = count + __popc(m & lt);
+                                if (k < S.cap) rowbase[((k >> S.tp_shift) << 5) + (k & tmask)] = j[q];
+                            }
+                            count += __popc(m & gmask);
                         }
-                    } else {
-                        const unsigned m = __ballot_sync(FULLMASK, acc);
-                        if (acc) {
-                            const int k = count + __popc(m & lt);
-                            if (k < S.cap) rowbase[((k >> S.tp_shift) << 5) + (k & tmask)] = j[q];
-                        }
-                        count += __popc(m & gmask);
                     }
                 }
             }
