@@ -807,3 +807,19 @@ def test_batched_ensemble_rejects_single_system_calls(rumd):
     with pytest.raises(rumd.RumdError):
         s.run_steps(1)
     s.close()
+
+
+def test_long_run_crosses_launch_chunks_and_conserves_energy(rumd):
+    """70 000 NVE steps of configs[0] in one rumd_run_steps call: more than one cooperative launch (a launch
+    runs at most 2^16 steps), thousands of in-kernel rebuilds; step count exact, energy conserved (S26 bar)."""
+    wl = make("lj", ncell=6)
+    s = rumd.from_workload(wl)
+    s.run_steps(2000)
+    th0 = s.get_thermo()
+    s.run_steps(70000)
+    th1 = s.get_thermo()
+    assert th1["n_steps"] - th0["n_steps"] == 70000
+    assert th1["n_rebuilds"] - th0["n_rebuilds"] > 2000
+    assert abs(th1["H"] - th0["H"]) / wl.N < 1e-4 * 7      # 1e-4 per particle per 10^4 steps
+    assert np.isfinite(th1["U"]) and th1["overflow"] == 0
+    s.close()
