@@ -176,6 +176,14 @@ rumd_status rumd_get_tuning(const rumd_system* s, rumd_tuning* out);
  * receives its time steps per second.  Synchronizes. */
 rumd_status rumd_autotune(rumd_system* s, rumd_tuning* out, int steps_per_trial, double* tps_out);
 
+/* The same with the paper's parameter file (P:382 step 8: the tuned parameters are written to a file and reused
+ * for runs with "the same user parameters"): cache_path (host string) names a text file with one JSON object
+ * per line, keyed by GPU name, N, box, potentials, integrator, dt, T, tau.  A cached entry for this key is
+ * applied without any trial run (*from_cache_out = 1); otherwise the autotuner runs and appends its result.
+ * cache_path NULL or "" = plain rumd_autotune.  from_cache_out: host, may be NULL. */
+rumd_status rumd_autotune_cached(rumd_system* s, rumd_tuning* out, int steps_per_trial, double* tps_out,
+                                 const char* cache_path, int* from_cache_out);
+
 /* Unconditional list rebuild with the current tuning.  Asynchronous. */
 rumd_status rumd_build_nblist(rumd_system* s);
 /* Rebuild iff the displacement flag is set, then forces / energies / virials into d_f,

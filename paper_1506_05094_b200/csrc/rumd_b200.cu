@@ -1267,3 +1267,88 @@ extern "C" rumd_status rumd_autotune(rumd_system* s, rumd_tuning* out, int steps
     if (tps_out) *tps_out = best_tps;
     return RUMD_OK;
 }
+
+// ---------------------------------------------------------------------------------------------- D10: tuning cache
+
+// P:382 step 8: the tuned parameters are written to a file and reused by later runs with "the same user
+// parameters" (system size, density, potential parameters, integrator, time step, temperature, GPU type).
+// One JSON object per line; the key is a canonical string of exactly those inputs.
+static std::string tuning_key(const rumd_system* s)
+{
+    char buf[256];
+    std::string k;
+    cudaDeviceProp prop;
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (cudaGetDeviceProperties(&prop, dev) == cudaSuccess) k += prop.name;
+    snprintf(buf, sizeof buf, "|N=%d|nt=%d|box=%.9g,%.9g,%.9g|int=%d|dt=%.9g|T=%.9g|tau=%.9g|rep=%d", s->N, s->ntypes,
+             s->box[0], s->box[1], s->box[2], s->integ, s->dt, s->T0, s->tau, s->nrep);
+    k += buf;
+    for (int a = 0; a < s->ntypes; ++a)
+        for (int b = a; b < s->ntypes; ++b) {
+            const PotSlot& p = s->pot[a][b];
+            snprintf(buf, sizeof buf, "|%d%d:lj=%d,%.9g,%.9g,%.9g,%d;x=%d,%d,%.9g,%.9g,%.9g,%.9g,%d", a, b, (int)p.lj, p.eps,
+                     p.sig, p.rc_lj, p.cut_lj, (int)p.coul, p.kind2, p.qq, p.b2, p.c2, p.rc_c, p.cut_c);
+            k += buf;
+        }
+    return k;
+}
+
+static bool cache_lookup(const char* path, const std::string& key, rumd_tuning* t, double* tps)
+{
+    FILE* f = fopen(path, "r");
+    if (!f) return false;
+    bool found = false;
+    std::vector<char> line(8192);
+    const std::string want = "{\"key\": \"" + key + "\", ";
+    while (fgets(line.data(), (int)line.size(), f)) {
+        if (strncmp(line.data(), want.c_str(), want.size()) != 0) continue;
+        rumd_tuning c;
+        double v = 0;
+        if (sscanf(line.data() + want.size(),
+                   "\"method\": %d, \"pb\": %d, \"tp\": %d, \"skin\": %f, \"sort_interval\": %d, \"use_graph\": %d, "
+                   "\"steps_per_graph\": %d, \"persistent\": %d, \"build_tp\": %d, \"timesteps_per_s\": %lf",
+                   &c.method, &c.pb, &c.tp, &c.skin, &c.sort_interval, &c.use_graph, &c.steps_per_graph, &c.persistent,
+                   &c.build_tp, &v) == 10) {
+            *t = c; // the LAST matching line wins (a re-tune appends)
+            *tps = v;
+            found = true;
+        }
+    }
+    fclose(f);
+    return found;
+}
+
+// rumd_autotune with the paper's parameter file: a cached setting for the same inputs is applied without any
+// trial run; otherwise the autotuner runs and its result is appended to the file.
+extern "C" rumd_status rumd_autotune_cached(rumd_system* s, rumd_tuning* out, int steps_per_trial, double* tps_out,
+                                            const char* cache_path, int* from_cache_out)
+{
+    if (!s) return RUMD_ERR_INVALID_ARG;
+    if (from_cache_out) *from_cache_out = 0;
+    if (!cache_path || !*cache_path) return rumd_autotune(s, out, steps_per_trial, tps_out);
+    rumd_status st = ready(s, true);
+    if (st != RUMD_OK) return st;
+    const std::string key = tuning_key(s);
+    rumd_tuning t;
+    double tps = 0;
+    if (cache_lookup(cache_path, key, &t, &tps) && rumd_set_tuning(s, &t) == RUMD_OK && refresh(s) == RUMD_OK) {
+        if (out) *out = t;
+        if (tps_out) *tps_out = tps;
+        if (from_cache_out) *from_cache_out = 1;
+        return RUMD_OK;
+    }
+    st = rumd_autotune(s, &t, steps_per_trial, &tps);
+    if (st != RUMD_OK) return st;
+    if (out) *out = t;
+    if (tps_out) *tps_out = tps;
+    FILE* f = fopen(cache_path, "a");
+    if (!f) return fail(s, RUMD_ERR_INVALID_ARG, "cannot write the tuning cache %s", cache_path);
+    fprintf(f,
+            "{\"key\": \"%s\", \"method\": %d, \"pb\": %d, \"tp\": %d, \"skin\": %.9g, \"sort_interval\": %d, \"use_graph\": %d, "
+            "\"steps_per_graph\": %d, \"persistent\": %d, \"build_tp\": %d, \"timesteps_per_s\": %.6g}\n",
+            key.c_str(), t.method, t.pb, t.tp, (double)t.skin, t.sort_interval, t.use_graph, t.steps_per_graph, t.persistent,
+            t.build_tp, tps);
+    fclose(f);
+    return RUMD_OK;
+}

@@ -25,7 +25,7 @@ NB_N2, NB_CELL, NB_NONE = 0, 1, 2
 EXPORTS = [
     "rumd_create", "rumd_destroy", "rumd_bind_state", "rumd_workspace_bytes", "rumd_bind_workspace",
     "rumd_set_pair_potential", "rumd_set_integrator", "rumd_default_tuning", "rumd_set_tuning",
-    "rumd_get_tuning", "rumd_autotune", "rumd_build_nblist", "rumd_compute_forces", "rumd_run_steps",
+    "rumd_get_tuning", "rumd_autotune", "rumd_autotune_cached", "rumd_build_nblist", "rumd_compute_forces", "rumd_run_steps",
     "rumd_export_nblist", "rumd_get_thermo", "rumd_snapshot", "rumd_restore", "rumd_upload_state",
     "rumd_download_state", "rumd_launch_count", "rumd_profile_step", "rumd_time_force", "rumd_profile_persistent", "rumd_set_replicas", "rumd_get_thermo_replicas", "rumd_last_error", "rumd_version",
 ]
@@ -80,6 +80,7 @@ def lib():
         L.rumd_set_tuning.argtypes = [vp, C.POINTER(Tuning)]
         L.rumd_get_tuning.argtypes = [vp, C.POINTER(Tuning)]
         L.rumd_autotune.argtypes = [vp, C.POINTER(Tuning), ip, C.POINTER(C.c_double)]
+        L.rumd_autotune_cached.argtypes = [vp, C.POINTER(Tuning), ip, C.POINTER(C.c_double), C.c_char_p, C.POINTER(ip)]
         L.rumd_build_nblist.argtypes = [vp]
         L.rumd_compute_forces.argtypes = [vp]
         L.rumd_run_steps.argtypes = [vp, C.c_long]
@@ -234,10 +235,18 @@ class System:
         self._check(self.L.rumd_set_tuning(self.h, C.byref(t)))
         return t
 
-    def autotune(self, steps_per_trial=200):
+    def autotune(self, steps_per_trial=200, cache_path=None):
+        """-> (Tuning, timesteps/s).  With cache_path the paper's parameter file is consulted first and
+        appended to after a tuning run; ``self.tuning_from_cache`` tells which happened."""
         t = Tuning()
         tps = C.c_double()
-        self._check(self.L.rumd_autotune(self.h, C.byref(t), int(steps_per_trial), C.byref(tps)))
+        hit = C.c_int(0)
+        if cache_path:
+            self._check(self.L.rumd_autotune_cached(self.h, C.byref(t), int(steps_per_trial), C.byref(tps),
+                                                   os.fsencode(cache_path), C.byref(hit)))
+        else:
+            self._check(self.L.rumd_autotune(self.h, C.byref(t), int(steps_per_trial), C.byref(tps)))
+        self.tuning_from_cache = bool(hit.value)
         return t, tps.value
 
     def build_nblist(self):

@@ -823,3 +823,33 @@ def test_long_run_crosses_launch_chunks_and_conserves_energy(rumd):
     assert abs(th1["H"] - th0["H"]) / wl.N < 1e-4 * 7      # 1e-4 per particle per 10^4 steps
     assert np.isfinite(th1["U"]) and th1["overflow"] == 0
     s.close()
+
+
+def test_autotune_cache_file_is_written_and_reused(rumd, tmp_path):
+    """D10 / P:382 step 8: the tuned parameters go to a file keyed by the user's parameters; a second system
+    with the same parameters takes them from the file without a trial run, a different one does not."""
+    path = str(tmp_path / "tuning.jsonl")
+    wl = perturbed(make("ka", N=1000))
+    s = rumd.from_workload(wl)
+    s.run_steps(20)
+    t1, tps1 = s.autotune(steps_per_trial=40, cache_path=path)
+    assert not s.tuning_from_cache and tps1 > 0
+    lines = open(path).read().strip().splitlines()
+    assert len(lines) == 1
+    import json as _json
+    rec = _json.loads(lines[0])
+    assert rec["tp"] == t1.tp and rec["method"] == t1.method and "N=1000" in rec["key"] and "B200" in rec["key"]
+    s.close()
+    s2 = rumd.from_workload(wl)
+    n0 = s2.launch_count()
+    t2, tps2 = s2.autotune(steps_per_trial=40, cache_path=path)
+    assert s2.tuning_from_cache and t2.as_dict() == t1.as_dict() and tps2 == pytest.approx(tps1, rel=1e-5)
+    assert s2.launch_count() - n0 <= 3                      # no trial runs
+    assert s2.get_tuning().as_dict() == t1.as_dict()
+    s2.run_steps(10)
+    s2.close()
+    wl3 = perturbed(make("ka", N=512))
+    s3 = rumd.from_workload(wl3)
+    s3.autotune(steps_per_trial=40, cache_path=path)
+    assert not s3.tuning_from_cache and len(open(path).read().strip().splitlines()) == 2
+    s3.close()
