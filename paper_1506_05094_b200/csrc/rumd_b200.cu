@@ -1240,6 +1240,13 @@ extern "C" rumd_status rumd_autotune(rumd_system* s, rumd_tuning* out, int steps
                 });
             if (T.cur_tps < 1.02 * before) break;
         }
+        if (method == RUMD_NB_N2 && s->N >= 1024) { // P:379 step 5: with n2, how often to re-sort the particles
+            rumd_tuning c = T.cur;
+            for (int si : {1, 4, 16}) {
+                c.sort_interval = si;
+                T.try_setting(c);
+            }
+        }
         {   // per-step kernels in CUDA graphs instead of the persistent kernel; there the block size matters
             rumd_tuning c = T.cur;
             c.persistent = 0;

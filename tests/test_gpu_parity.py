@@ -853,3 +853,35 @@ def test_autotune_cache_file_is_written_and_reused(rumd, tmp_path):
     s3.autotune(steps_per_trial=40, cache_path=path)
     assert not s3.tuning_from_cache and len(open(path).read().strip().splitlines()) == 2
     s3.close()
+
+
+@pytest.mark.parametrize("persistent", [1, 0])
+def test_n2_method_with_periodic_sort(rumd, persistent):
+    """P:379 step 5 (K13): with the N^2 build the particles are spatially re-sorted at every sort_interval-th
+    rebuild.  The permutation must be transparent: same trajectory (to fp32 summation order) as without sorting,
+    list and forces against the oracle in the sorted order."""
+    wl = perturbed(make("ka", N=2048))
+    res = []
+    for si in (0, 2):
+        s = rumd.from_workload(wl)
+        s.set_tuning(method=rumd.NB_N2, tp=16, pb=16, sort_interval=si, persistent=persistent, use_graph=0, skin=0.3)
+        s.run_steps(60)
+        th = s.get_thermo()
+        assert th["n_rebuilds"] >= 3
+        ids = s.d_id.cpu().numpy()
+        assert sorted(ids.tolist()) == list(range(wl.N))
+        assert (ids != np.arange(wl.N)).any() == (si > 0)
+        st = s.state()
+        res.append(st)
+        if si:
+            s.build_nblist()
+            s.compute_forces()
+            st2 = s.state()
+            r64 = st2["r"].astype(np.float64)
+            check_nblist(s, r64, wl.types, wl.box.astype(np.float64), wl.pot, 0.3)
+            check_forces(s, r64, wl.types, wl.box.astype(np.float64), wl.pot)
+        s.close()
+    d = res[0]["r"].astype(np.float64) - res[1]["r"]
+    box = wl.box.astype(np.float64)
+    d -= box * np.rint(d / box)
+    assert np.abs(d).max() < 2e-4
