@@ -1,5 +1,6 @@
 // rumd_b200.cu -- host side of librumd_b200.so: C ABI (include/rumd_b200.h), workspace carving, launch
 // chains, whole-timestep CUDA graphs and the Blackwell autotuner.  Product code: shares nothing with oracle/.
+#define RUMD_MAIN_TU 1
 #include "../../include/rumd_b200.h"
 #include "rumd_dispatch.cuh"
 #include "rumd_persist.cuh"

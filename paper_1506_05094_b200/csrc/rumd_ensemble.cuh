@@ -17,7 +17,11 @@
 #include "rumd_force.cuh"
 
 #define ENS_THREADS 256
+#ifndef ENS_MINB
+#define ENS_MINB 3
+#endif
 
+#ifdef RUMD_MAIN_TU // non-template kernels: compiled once, in rumd_b200.cu
 static __global__ void k_ens_reset(DevScalars* sc, int nrep)
 {
     const int q = blockIdx.x * blockDim.x + threadIdx.x;
@@ -33,6 +37,7 @@ static __global__ void k_ens_request_rebuild(DevScalars* sc, int nrep)
     const int q = blockIdx.x * blockDim.x + threadIdx.x;
     if (q < nrep) sc[q].flag = 1u;
 }
+#endif // RUMD_MAIN_TU
 
 // fixed-order block sum of a double (result valid in thread 0); s: ENS_THREADS / 32 doubles
 __device__ __forceinline__ double ens_block_sum(double x, double* s)
@@ -49,7 +54,7 @@ __device__ __forceinline__ double ens_block_sum(double x, double* s)
 }
 
 template <int TP, int COUL, bool ONE_TYPE, int UNROLL>
-__global__ void __launch_bounds__(ENS_THREADS, 3) k_ensemble(const Sys* __restrict__ systems, const int nsteps, const int nvt)
+__global__ void __launch_bounds__(ENS_THREADS, ENS_MINB) k_ensemble(const Sys* __restrict__ systems, const int nsteps, const int nvt)
 {
     __shared__ Sys R; // this replica's parameter block
     __shared__ float4 s_pp[4 * RUMD_MAXT * RUMD_MAXT];

@@ -427,6 +427,7 @@ __device__ __forceinline__ void step_tail(const Sys& S, bool nvt, double kt, dou
 }
 
 #define INT_THREADS 128
+#ifdef RUMD_MAIN_TU // non-template kernels: compiled once, in rumd_b200.cu
 static __global__ void __launch_bounds__(INT_THREADS) k_integrate(const Sys S, int nvt)
 {
     float a, b;
@@ -444,6 +445,7 @@ static __global__ void __launch_bounds__(INT_THREADS) k_integrate(const Sys S, i
     }
     step_tail<INT_THREADS / 32>(S, nvt != 0, kt, mv2, moved, gridDim.x);
 }
+#endif // RUMD_MAIN_TU
 
 // A5 + A6 fused for the per-step path: forces of r(t) read from S.r, leap-frog update written to S.r_out
 // (the OTHER position buffer: nobody reads a position that was already advanced), then the same block tail as
@@ -490,6 +492,7 @@ __global__ void __launch_bounds__(1024, 1) k_step(const Sys S, int nvt)
 
 // ------------------------------------------------------------------------------------------ small kernels
 
+#ifdef RUMD_MAIN_TU // non-template kernels: compiled once, in rumd_b200.cu
 static __global__ void k_request_rebuild(const Sys S)
 {
     S.sc->flag = 1u;
@@ -556,3 +559,4 @@ static __global__ void k_copy_state(int N, const float4* r, const float4* v, con
     im2[i] = im[i];
     id2[i] = id[i];
 }
+#endif // RUMD_MAIN_TU

@@ -478,6 +478,7 @@ __device__ __forceinline__ void build_cell_dispatch(const Sys& S, const float4* 
 
 __device__ __forceinline__ int* max_slot_of(const Sys& S) { return &S.sc->max_nbrs[S.sc->n_rebuilds & 1]; }
 
+#ifdef RUMD_MAIN_TU // non-template kernels: compiled once, in rumd_b200.cu
 static __global__ void __launch_bounds__(128) k_build_n2(const Sys S)
 {
     if (!rebuild_requested(S)) return;
@@ -560,3 +561,4 @@ static __global__ void k_permute_store(const Sys S)
     VGRID;
     ph_permute_store(S, S.r, first, stride);
 }
+#endif // RUMD_MAIN_TU
