@@ -50,7 +50,15 @@ typedef enum { /* P:73 pair potentials; the first is the LJ slot of a type pair,
     RUMD_POT_IPL = 2,           /* {a, n, rcut}             u = a r^-n   (inverse power law) */
     RUMD_POT_YUKAWA = 3,        /* {a, b, rcut}             u = a exp(-r / b) / r */
     RUMD_POT_GAUSSIAN_CORE = 4, /* {a, b, rcut}             u = a exp(-(r / b)^2) */
-    RUMD_POT_BUCKINGHAM = 5     /* {a, b, c, rcut}          u = a exp(-r / b) - c / r^6 */
+    RUMD_POT_BUCKINGHAM = 5,    /* {a, b, c, rcut}          u = a exp(-r / b) - c / r^6 */
+    RUMD_POT_GEN_LJ = 6,        /* {epsilon, sigma, m, n, rcut}  u = eps / (m - n) [n (s/r)^m - m (s/r)^n], m > n > 0:
+                                   minimum -eps at r = sigma.  Takes the place of the 12-6 term: a type pair
+                                   with this kind must have no RUMD_POT_LJ_12_6 term (RUMD_ERR_INVALID_ARG) */
+    RUMD_POT_GIRIFALCO = 7,     /* {alpha, beta, d, rcut}   u = -alpha [1/(s(s-1)^3) + 1/(s(s+1)^3) - 2/s^4]
+                                   + beta [1/(s(s-1)^9) + 1/(s(s+1)^9) - 2/s^10], s = r / d; defined for r > d only */
+    RUMD_POT_DZUGUTOV = 8       /* {epsilon, sigma, rcut}   u = eps [A (x^-16 - B) exp(c/(x-a)) (x < a)
+                                   + B exp(d/(x-b)) (x < b)], x = r / sigma, A 5.82, B 1.28, a 1.87, b 1.94, c 1.1,
+                                   d 0.27; it vanishes smoothly at x = b, so rcut = b sigma with RUMD_CUT_NONE is natural */
 } rumd_pot_kind;
 typedef enum { /* P:73-75 "the cutoff methods: no shift, shifted potential and shifted force" */
     RUMD_CUT_SHIFTED_FORCE = 0,     /* f = f(r) - f(rc), u = u(r) - u(rc) + (r - rc) f(rc): the hot-path default */
@@ -153,7 +161,7 @@ rumd_status rumd_bind_workspace(rumd_system* s, void* d_ws, size_t bytes, int nb
 /* P:49-50 `pot.SetParams(i, j, Sigma, Epsilon, Rcut)`; symmetric in (type_i, type_j).  params: host.
  *   RUMD_POT_LJ_12_6 : {epsilon, sigma, rcut}   u = 4 eps [(s/r)^12 - (s/r)^6]           (O3)
  *   RUMD_POT_COULOMB : {k*q_i*q_j, rcut}        u = k q_i q_j / r, no self term          (O4, S6)
- *   RUMD_POT_IPL / YUKAWA / GAUSSIAN_CORE / BUCKINGHAM : see rumd_pot_kind; they occupy the same slot as
+ *   RUMD_POT_IPL / YUKAWA / GAUSSIAN_CORE / BUCKINGHAM / GEN_LJ / GIRIFALCO / DZUGUTOV : see rumd_pot_kind; they occupy the same slot as
  *   Coulomb (a type pair has the LJ term plus at most ONE of these; setting one replaces the other).
  * rcut is an ABSOLUTE distance (S2).  cutoff: one of rumd_cutoff, applied for r < rcut, zero beyond (S3).
  * One slot per kind per type pair: the same kind again overwrites, different kinds add, each with its own

@@ -26,7 +26,7 @@ _SRC = os.path.join(_HERE, "rumd_oracle.c")
 _LIB = os.path.join(_HERE, "librumd_oracle.so")
 
 NVE, NVT = 0, 1
-POT_STRIDE = 10
+POT_STRIDE = 11
 
 
 def build(force: bool = False) -> str:
@@ -56,8 +56,8 @@ def lib():
         L.orc_coulomb_sf.argtypes = [C.c_double] * 3 + [_dp, _dp]
         L.orc_lj_cut.argtypes = [C.c_double] * 4 + [C.c_int, _dp, _dp]
         L.orc_coulomb_cut.argtypes = [C.c_double] * 3 + [C.c_int, _dp, _dp]
-        L.orc_extra_raw.argtypes = [C.c_int] + [C.c_double] * 4 + [_dp, _dp]
-        L.orc_extra_cut.argtypes = [C.c_int] + [C.c_double] * 5 + [C.c_int, _dp, _dp]
+        L.orc_extra_raw.argtypes = [C.c_int] + [C.c_double] * 5 + [_dp, _dp]
+        L.orc_extra_cut.argtypes = [C.c_int] + [C.c_double] * 6 + [C.c_int, _dp, _dp]
         L.orc_pair_sf.argtypes = [_dp, C.c_double, _dp, _dp]
         L.orc_pair_rc.argtypes = [_dp]
         L.orc_pair_rc.restype = C.c_double
@@ -133,13 +133,14 @@ def coulomb_cut(r, qq, rc, method):
     return _pair(lib().orc_coulomb_cut, float(r), float(qq), float(rc), int(method))
 
 
-def extra_raw(kind, r, a, b=0.0, c=0.0):
-    """(u, f) of the unshifted second-term potentials: 0 Coulomb, 1 IPL, 2 Yukawa, 3 Gaussian core, 4 Buckingham."""
-    return _pair(lib().orc_extra_raw, int(kind), float(r), float(a), float(b), float(c))
+def extra_raw(kind, r, a, b=0.0, c=0.0, d=0.0):
+    """(u, f) of the unshifted second-term potentials: 0 Coulomb, 1 IPL, 2 Yukawa, 3 Gaussian core, 4 Buckingham,
+    5 generalized LJ, 6 Girifalco, 7 Dzugutov."""
+    return _pair(lib().orc_extra_raw, int(kind), float(r), float(a), float(b), float(c), float(d))
 
 
-def extra_cut(kind, r, a, b, c, rc, method):
-    return _pair(lib().orc_extra_cut, int(kind), float(r), float(a), float(b), float(c), float(rc), int(method))
+def extra_cut(kind, r, a, b, c, rc, method, d=0.0):
+    return _pair(lib().orc_extra_cut, int(kind), float(r), float(a), float(b), float(c), float(d), float(rc), int(method))
 
 
 def pair_sf(rec, r):

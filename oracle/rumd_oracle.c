@@ -37,6 +37,12 @@
  *            2 Yukawa         u = a exp(-r / b) / r
  *            3 Gaussian core  u = a exp(-(r / b)^2)
  *            4 Buckingham     u = a exp(-r / b) - c / r^6
+ *            5 generalized LJ u = a / (c - d) [ d (b/r)^c - c (b/r)^d ]   (a = epsilon, b = sigma, exponents
+ *                             c = m > d = n; minimum -epsilon at r = sigma; pot[10] = d)
+ *            6 Girifalco      u = -a [1/(s(s-1)^3) + 1/(s(s+1)^3) - 2/s^4]
+ *                                 + b [1/(s(s-1)^9) + 1/(s(s+1)^9) - 2/s^10],  s = r / c   (r > c)
+ *            7 Dzugutov       u = a [ A (x^-16 - B) exp(cc / (x - aa)) (x < aa) + B exp(dd / (x - bb)) (x < bb) ],
+ *                             x = r / b, with the published constants A 5.82, B 1.28, aa 1.87, bb 1.94, cc 1.1, dd 0.27
  * rc values are ABSOLUTE distances (S2).
  */
 #include <math.h>
@@ -46,7 +52,7 @@
 #include <omp.h>
 #endif
 
-#define ORC_POT_STRIDE 10
+#define ORC_POT_STRIDE 11
 
 int orc_num_threads(void)
 {
@@ -150,9 +156,37 @@ void orc_coulomb_cut(double r, double qq, double rc, int method, double *u, doub
 }
 
 /* The other pair potentials of P:73 ("IPL, Gaussian core, Buckingham, ..., Yukawa"), unshifted: (u, f = -du/dr). */
-void orc_extra_raw(int kind, double r, double a, double b, double c, double *u, double *f)
+void orc_extra_raw(int kind, double r, double a, double b, double c, double d, double *u, double *f)
 {
-    if (kind == 1) {          /* inverse power law: u = a r^-b, f = b a r^-(b+1) */
+    if (kind == 5) {          /* generalized LJ (m = c, n = d): f = a c d / (c - d) [ (b/r)^c - (b/r)^d ] / r */
+        const double sm = pow(b / r, c), sn = pow(b / r, d);
+        *u = a / (c - d) * (d * sm - c * sn);
+        *f = a * c * d / (c - d) * (sm - sn) / r;
+    } else if (kind == 6) {   /* Girifalco: s = r / c, f = -(1/c) du/ds, term by term */
+        const double s = r / c, m = s - 1.0, p = s + 1.0;
+        *u = -a * (1.0 / (s * pow(m, 3)) + 1.0 / (s * pow(p, 3)) - 2.0 / pow(s, 4)) +
+             b * (1.0 / (s * pow(m, 9)) + 1.0 / (s * pow(p, 9)) - 2.0 / pow(s, 10));
+        /* d/ds 1/(s (s-+1)^k) = -((k+1) s -+ 1) / (s^2 (s-+1)^(k+1)),  d/ds (-2 s^-q) = 2 q s^-(q+1) */
+        const double du = -a * (-(4.0 * s - 1.0) / (s * s * pow(m, 4)) - (4.0 * s + 1.0) / (s * s * pow(p, 4)) + 8.0 / pow(s, 5)) +
+                          b * (-(10.0 * s - 1.0) / (s * s * pow(m, 10)) - (10.0 * s + 1.0) / (s * s * pow(p, 10)) + 20.0 / pow(s, 11));
+        *f = -du / c;
+    } else if (kind == 7) {   /* Dzugutov, x = r / b */
+        const double A = 5.82, B = 1.28, aa = 1.87, bb = 1.94, cc = 1.1, dd = 0.27;
+        const double x = r / b;
+        double uu = 0.0, du = 0.0;
+        if (x < aa) {
+            const double e = exp(cc / (x - aa)), g = pow(x, -16.0) - B;
+            uu += A * g * e;
+            du += A * e * (-16.0 * pow(x, -17.0) - g * cc / ((x - aa) * (x - aa)));
+        }
+        if (x < bb) {
+            const double e = exp(dd / (x - bb));
+            uu += B * e;
+            du += -B * e * dd / ((x - bb) * (x - bb));
+        }
+        *u = a * uu;
+        *f = -a * du / b;
+    } else if (kind == 1) {          /* inverse power law: u = a r^-b, f = b a r^-(b+1) */
         *u = a * pow(r, -b);
         *f = b * a * pow(r, -b - 1.0);
     } else if (kind == 2) {   /* Yukawa: u = a e^(-r/b) / r, f = u (1/r + 1/b) */
@@ -170,11 +204,12 @@ void orc_extra_raw(int kind, double r, double a, double b, double c, double *u, 
     }
 }
 
-void orc_extra_cut(int kind, double r, double a, double b, double c, double rc, int method, double *u, double *f)
+void orc_extra_cut(int kind, double r, double a, double b, double c, double d, double rc, int method, double *u,
+                   double *f)
 {
     double ur, fr, uc, fc;
-    orc_extra_raw(kind, r, a, b, c, &ur, &fr);
-    orc_extra_raw(kind, rc, a, b, c, &uc, &fc);
+    orc_extra_raw(kind, r, a, b, c, d, &ur, &fr);
+    orc_extra_raw(kind, rc, a, b, c, d, &uc, &fc);
     orc_apply_cutoff(method, r, rc, ur, fr, uc, fc, u, f);
 }
 
@@ -188,7 +223,7 @@ void orc_pair_sf(const double *p, double r, double *u, double *f)
         ft += ff;
     }
     if (p[4] > 0.0) {
-        orc_extra_cut((int)p[7], r, p[3], p[8], p[9], p[4], (int)p[6], &uu, &ff);
+        orc_extra_cut((int)p[7], r, p[3], p[8], p[9], p[10], p[4], (int)p[6], &uu, &ff);
         ut += uu;
         ft += ff;
     }

@@ -18,8 +18,8 @@ struct PotSlot {
     bool lj = false, coul = false;
     double eps = 0, sig = 0, rc_lj = 0, qq = 0, rc_c = 0; // qq: prefactor a of the second term
     int cut_lj = 0, cut_c = 0; // rumd_cutoff of each term
-    int kind2 = 0;             // second term: 0 Coulomb, 1 IPL, 2 Yukawa, 3 Gaussian core, 4 Buckingham
-    double b2 = 0, c2 = 0;     // its further parameters
+    int kind2 = 0;             // second term: rumd_pot_kind - 1 (0 Coulomb ... 7 Dzugutov)
+    double b2 = 0, c2 = 0, d2 = 0; // its further parameters
 };
 
 struct GraphCache {
@@ -367,9 +367,9 @@ extern "C" rumd_status rumd_set_pair_potential(rumd_system* s, int ti, int tj, r
             p.rc_lj = params[2];
             p.cut_lj = (int)cutoff;
             if (p.lj && !(p.sig > 0)) return fail(s, RUMD_ERR_INVALID_ARG, "sigma must be > 0");
-        } else if (kind == RUMD_POT_COULOMB || kind == RUMD_POT_IPL || kind == RUMD_POT_YUKAWA ||
-                   kind == RUMD_POT_GAUSSIAN_CORE || kind == RUMD_POT_BUCKINGHAM) {
-            const int want = kind == RUMD_POT_COULOMB ? 2 : kind == RUMD_POT_BUCKINGHAM ? 4 : 3;
+        } else if (kind >= RUMD_POT_COULOMB && kind <= RUMD_POT_DZUGUTOV) {
+            static const int n_of[8] = {2, 3, 3, 3, 4, 5, 4, 3}; // parameters incl. rcut, by kind - 1
+            const int want = n_of[(int)kind - 1];
             if (n_params != want) return fail(s, RUMD_ERR_INVALID_ARG, "this potential takes %d parameters (see rumd_pot_kind)", want);
             const float rc = params[want - 1];
             p.coul = rc > 0.f;
@@ -379,8 +379,14 @@ extern "C" rumd_status rumd_set_pair_potential(rumd_system* s, int ti, int tj, r
             p.kind2 = (int)kind - 1;
             p.b2 = want >= 3 ? params[1] : 0.0;
             p.c2 = want >= 4 ? params[2] : 0.0;
-            if (p.coul && (kind == RUMD_POT_YUKAWA || kind == RUMD_POT_GAUSSIAN_CORE || kind == RUMD_POT_BUCKINGHAM) && !(p.b2 > 0))
-                return fail(s, RUMD_ERR_INVALID_ARG, "the length parameter b must be > 0");
+            p.d2 = want >= 5 ? params[3] : 0.0;
+            if (p.coul && (kind == RUMD_POT_YUKAWA || kind == RUMD_POT_GAUSSIAN_CORE || kind == RUMD_POT_BUCKINGHAM ||
+                           kind == RUMD_POT_GEN_LJ || kind == RUMD_POT_DZUGUTOV) && !(p.b2 > 0))
+                return fail(s, RUMD_ERR_INVALID_ARG, "the length parameter (second one) must be > 0");
+            if (p.coul && kind == RUMD_POT_GEN_LJ && !(p.c2 > p.d2 && p.d2 > 0))
+                return fail(s, RUMD_ERR_INVALID_ARG, "generalized LJ needs exponents m > n > 0");
+            if (p.coul && kind == RUMD_POT_GIRIFALCO && !(p.c2 > 0 && rc > p.c2))
+                return fail(s, RUMD_ERR_INVALID_ARG, "Girifalco needs a diameter d > 0 and rcut > d");
         } else
             return fail(s, RUMD_ERR_INVALID_ARG, "unknown potential kind");
     }
@@ -520,8 +526,48 @@ static rumd_status refresh(rumd_system* s)
             if (p.coul) {
                 // second term at the cutoff, in double: u(rc), f(rc) of the raw potential
                 const double a = p.qq, b = p.b2, c = p.c2, rcc = p.rc_c;
-                double uraw, fraw, p1 = 0.0, p2 = 0.0;
+                double uraw, fraw, p1 = 0.0, p2 = 0.0, amp = a;
                 switch (p.kind2) {
+                case 5: { // generalized LJ as A r^-m - B r^-n; B rides in the (unused) 12-6 slot of the pair
+                    if (p.lj) return fail(s, RUMD_ERR_INVALID_ARG, "generalized LJ takes the place of the 12-6 term: a type pair has both");
+                    const double m = c, n = p.d2, A = a * n * std::pow(b, m) / (m - n), B = a * m * std::pow(b, n) / (m - n);
+                    uraw = A * std::pow(rcc, -m) - B * std::pow(rcc, -n);
+                    fraw = (m * A * std::pow(rcc, -m) - n * B * std::pow(rcc, -n)) / rcc;
+                    amp = A;
+                    p1 = m;
+                    p2 = n;
+                    q.c12x12 = (float)B;
+                    break;
+                }
+                case 6: { // Girifalco, s = r / d
+                    const double sg = rcc / c, m = sg - 1.0, pl = sg + 1.0;
+                    uraw = -a * (1.0 / (sg * std::pow(m, 3)) + 1.0 / (sg * std::pow(pl, 3)) - 2.0 / std::pow(sg, 4)) +
+                           b * (1.0 / (sg * std::pow(m, 9)) + 1.0 / (sg * std::pow(pl, 9)) - 2.0 / std::pow(sg, 10));
+                    const double du = -a * (-(4 * sg - 1) / (sg * sg * std::pow(m, 4)) - (4 * sg + 1) / (sg * sg * std::pow(pl, 4)) + 8.0 / std::pow(sg, 5)) +
+                                      b * (-(10 * sg - 1) / (sg * sg * std::pow(m, 10)) - (10 * sg + 1) / (sg * sg * std::pow(pl, 10)) + 20.0 / std::pow(sg, 11));
+                    fraw = -du / c;
+                    p1 = b;
+                    p2 = 1.0 / c;
+                    break;
+                }
+                case 7: { // Dzugutov, x = r / sigma
+                    const double x = rcc / b;
+                    double uu = 0.0, du = 0.0;
+                    if (x < DZ_a) {
+                        const double e = std::exp(DZ_c / (x - DZ_a)), g = std::pow(x, -16.0) - DZ_B;
+                        uu += DZ_A * g * e;
+                        du += DZ_A * e * (-16.0 * std::pow(x, -17.0) - g * DZ_c / ((x - DZ_a) * (x - DZ_a)));
+                    }
+                    if (x < DZ_b) {
+                        const double e = std::exp(DZ_d / (x - DZ_b));
+                        uu += DZ_B * e;
+                        du -= DZ_B * e * DZ_d / ((x - DZ_b) * (x - DZ_b));
+                    }
+                    uraw = a * uu;
+                    fraw = -a * du / b;
+                    p1 = 1.0 / b;
+                    break;
+                }
                 case 1: uraw = a * std::pow(rcc, -b); fraw = b * a * std::pow(rcc, -b - 1.0); p1 = b; break;
                 case 2: uraw = a * std::exp(-rcc / b) / rcc; fraw = uraw * (1.0 / rcc + 1.0 / b); p1 = 1.0 / b; break;
                 case 3: uraw = a * std::exp(-(rcc / b) * (rcc / b)); fraw = 2.0 * rcc * uraw / (b * b); p1 = 1.0 / (b * b); break;
@@ -533,7 +579,7 @@ static rumd_status refresh(rumd_system* s)
                     break;
                 default: uraw = a / rcc; fraw = a / (rcc * rcc); break;
                 }
-                q.qq = (float)a;
+                q.qq = (float)amp;
                 q.rc2_c = (float)(rcc * rcc);
                 const double ucc = p.cut_c == RUMD_CUT_NONE ? 0.0 : uraw;
                 const double fcc = p.cut_c == RUMD_CUT_SHIFTED_FORCE ? fraw : 0.0;
@@ -1295,8 +1341,8 @@ static std::string tuning_key(const rumd_system* s)
     for (int a = 0; a < s->ntypes; ++a)
         for (int b = a; b < s->ntypes; ++b) {
             const PotSlot& p = s->pot[a][b];
-            snprintf(buf, sizeof buf, "|%d%d:lj=%d,%.9g,%.9g,%.9g,%d;x=%d,%d,%.9g,%.9g,%.9g,%.9g,%d", a, b, (int)p.lj, p.eps,
-                     p.sig, p.rc_lj, p.cut_lj, (int)p.coul, p.kind2, p.qq, p.b2, p.c2, p.rc_c, p.cut_c);
+            snprintf(buf, sizeof buf, "|%d%d:lj=%d,%.9g,%.9g,%.9g,%d;x=%d,%d,%.9g,%.9g,%.9g,%.9g,%.9g,%d", a, b, (int)p.lj, p.eps,
+                     p.sig, p.rc_lj, p.cut_lj, (int)p.coul, p.kind2, p.qq, p.b2, p.c2, p.d2, p.rc_c, p.cut_c);
             k += buf;
         }
     return k;

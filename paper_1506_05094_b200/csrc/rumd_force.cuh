@@ -68,6 +68,34 @@ __device__ __forceinline__ void pair_accumulate(const float4 pf, const float4 pc
             fx_r = __fmaf_rn(e * px.z, r, -6.0f * c6) * rinv2;
             break;
         }
+        case 5: { // generalized LJ: u = A r^-m - B r^-n, m = p1, n = p2, B in the (unused) 12-6 slot pf.x
+            const float l = -0.5f * __log2f(r2);
+            const float tm = pc.x * exp2f(px.z * l), tn = pf.x * exp2f(px.w * l);
+            ux = tm - tn;
+            fx_r = __fmaf_rn(px.z, tm, -px.w * tn) * rinv2;
+            break;
+        }
+        case 6: { // Girifalco: s = r / d (p2 = 1 / d), alpha = a, beta = p1; f = -(1/d) du/ds
+            const float s = r * px.w, is = __frcp_approx(s), im = __frcp_approx(s - 1.0f), ip = __frcp_approx(s + 1.0f);
+            const float is2 = is * is, is4 = is2 * is2, im3 = im * im * im, ip3 = ip * ip * ip;
+            const float im9 = im3 * im3 * im3, ip9 = ip3 * ip3 * ip3, is10 = is4 * is4 * is2;
+            ux = -pc.x * __fmaf_rn(is, im3 + ip3, -2.0f * is4) + px.z * __fmaf_rn(is, im9 + ip9, -2.0f * is10);
+            const float d3 = is2 * ((4.0f * s - 1.0f) * im3 * im + (4.0f * s + 1.0f) * ip3 * ip) - 8.0f * is4 * is;
+            const float d9 = is2 * ((10.0f * s - 1.0f) * im9 * im + (10.0f * s + 1.0f) * ip9 * ip) - 20.0f * is10 * is;
+            fx_r = (px.z * d9 - pc.x * d3) * px.w * y; // -du/ds = beta d9 - alpha d3
+            break;
+        }
+        case 7: { // Dzugutov: x = r / sigma (p1 = 1 / sigma); both pieces vanish with all derivatives at their edge
+            const float x = r * px.z, ix2 = __frcp_approx(x * x), ix4 = ix2 * ix2, ix8 = ix4 * ix4, ix16 = ix8 * ix8;
+            const float t1 = __frcp_approx(fminf(x - (float)DZ_a, -1e-6f)), t2 = __frcp_approx(fminf(x - (float)DZ_b, -1e-6f));
+            const float e1 = x < (float)DZ_a ? (float)DZ_A * __expf((float)DZ_c * t1) : 0.f;
+            const float e2 = x < (float)DZ_b ? (float)DZ_B * __expf((float)DZ_d * t2) : 0.f;
+            const float g = ix16 - (float)DZ_B;
+            ux = pc.x * __fmaf_rn(g, e1, e2);
+            const float du = e1 * (-16.0f * ix16 * x * ix2 - g * (float)DZ_c * t1 * t1) - e2 * (float)DZ_d * t2 * t2;
+            fx_r = -pc.x * du * px.z * y;
+            break;
+        }
         }
         fr += in_c ? __fmaf_rn(-pc.z, y, fx_r) : 0.f;                     // f / r - fc / r
         if (ENERGY) uu += in_c ? ux + __fmaf_rn(pc.z, r, -pe.w) : 0.f; // u + fc r - k0

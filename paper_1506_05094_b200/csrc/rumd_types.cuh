@@ -5,6 +5,13 @@
 #include <stdint.h>
 
 #define RUMD_MAXT 4
+// Dzugutov potential, published constants (u = A (x^-16 - B) exp(c / (x - a)) [x < a] + B exp(d / (x - b)) [x < b])
+#define DZ_A 5.82
+#define DZ_B 1.28
+#define DZ_a 1.87
+#define DZ_b 1.94
+#define DZ_c 1.1
+#define DZ_d 0.27
 
 // One record per ORDERED type pair; all derived constants are computed on the host in double precision
 // from the user's fp32 parameters and rounded once.

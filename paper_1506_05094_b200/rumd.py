@@ -18,6 +18,8 @@ _LIBPATH = os.environ.get("RUMD_B200_LIB") or os.path.join(_HERE, "librumd_b200.
 
 OK, ERR_INVALID_ARG, ERR_NOT_READY, ERR_CUDA, ERR_NBL_OVERFLOW, ERR_BOX_TOO_SMALL, ERR_NONFINITE = range(7)
 POT_LJ_12_6, POT_COULOMB, POT_IPL, POT_YUKAWA, POT_GAUSSIAN_CORE, POT_BUCKINGHAM = range(6)
+POT_GEN_LJ, POT_GIRIFALCO, POT_DZUGUTOV = 6, 7, 8
+_SECOND_NPARAMS = (1, 2, 2, 2, 3, 4, 3, 2)  # of (a, b, c, d), by kind - 1; rcut follows
 CUT_SHIFTED_FORCE, CUT_SHIFTED_POTENTIAL, CUT_NONE = 0, 1, 2
 INT_NVE_LEAPFROG, INT_NVT_NOSE_HOOVER = 0, 1
 NB_N2, NB_CELL, NB_NONE = 0, 1, 2
@@ -174,7 +176,8 @@ class System:
                 if rcc > 0:
                     kind2 = int(pot[a, b, 7]) if pot.shape[-1] >= 10 else 0
                     pb, pc = (pot[a, b, 8], pot[a, b, 9]) if pot.shape[-1] >= 10 else (0.0, 0.0)
-                    params = {0: [qq, rcc], 4: [qq, pb, pc, rcc]}.get(kind2, [qq, pb, rcc])
+                    pd = pot[a, b, 10] if pot.shape[-1] >= 11 else 0.0
+                    params = [qq, pb, pc, pd][:_SECOND_NPARAMS[kind2]] + [rcc]
                     self.set_pair_potential(a, b, POT_COULOMB + kind2, params, cut_c)
         self.rc_max = float(max(pot[..., 2].max(), pot[..., 4].max()))
         self.density = self.N / float(np.prod(self.box.astype(np.float64)))

@@ -19,8 +19,10 @@ import numpy as np
 SEED0 = 150605094  # + 1000*config + index-in-sweep
 
 NVE, NVT = 0, 1
-POT_STRIDE = 10  # (epsilon, sigma, rc_LJ, a, rc_2, cut_LJ, cut_2, kind_2, b, c); rc <= 0 disables the term
+POT_STRIDE = 11  # (epsilon, sigma, rc_LJ, a, rc_2, cut_LJ, cut_2, kind_2, b, c, d); rc <= 0 disables the term
 KIND_COULOMB, KIND_IPL, KIND_YUKAWA, KIND_GAUSSIAN_CORE, KIND_BUCKINGHAM = 0, 1, 2, 3, 4  # second term
+KIND_GEN_LJ, KIND_GIRIFALCO, KIND_DZUGUTOV = 5, 6, 7
+KIND_NPARAMS = (1, 2, 2, 2, 3, 4, 3, 2)  # how many of (a, b, c, d) each kind takes
 CUT_SHIFTED_FORCE, CUT_SHIFTED_POTENTIAL, CUT_NONE = 0, 1, 2
 
 
@@ -128,12 +130,13 @@ def set_coulomb(pot, a, b, qq, rc, cut=CUT_SHIFTED_FORCE):
     set_second_term(pot, a, b, KIND_COULOMB, qq, 0.0, 0.0, rc, cut)
 
 
-def set_second_term(pot, a, b, kind, pa, pb, pc, rc, cut=CUT_SHIFTED_FORCE):
+def set_second_term(pot, a, b, kind, pa, pb, pc, rc, cut=CUT_SHIFTED_FORCE, pd=0.0):
     """The pair's second term: Coulomb pa/r, IPL pa r^-pb, Yukawa pa exp(-r/pb)/r, Gaussian core pa exp(-(r/pb)^2),
-    Buckingham pa exp(-r/pb) - pc/r^6."""
+    Buckingham pa exp(-r/pb) - pc/r^6, generalized LJ (epsilon pa, sigma pb, exponents pc > pd), Girifalco (alpha pa,
+    beta pb, diameter pc), Dzugutov (epsilon pa, sigma pb) (formulas in include/rumd_b200.h)."""
     for i, j in ((a, b), (b, a)):
         pot[i, j, 3], pot[i, j, 4], pot[i, j, 6] = f32(pa), f32(rc), float(cut)
-        pot[i, j, 7], pot[i, j, 8], pot[i, j, 9] = float(kind), f32(pb), f32(pc)
+        pot[i, j, 7], pot[i, j, 8], pot[i, j, 9], pot[i, j, 10] = float(kind), f32(pb), f32(pc), f32(pd)
 
 
 def lj_single() -> np.ndarray:

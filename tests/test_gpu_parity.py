@@ -501,14 +501,26 @@ def _extra_pot(which):
         W.set_lj(pot, 0, 0, 1.0, 1.0, 2.5)
         W.set_lj(pot, 1, 1, 0.5, 0.88, 2.2)
         W.set_second_term(pot, 0, 1, W.KIND_BUCKINGHAM, 2500.0, 0.2, 1.6, 2.4)
+    elif which == "glj":        # generalized LJ with three different exponent pairs (no 12-6 term)
+        for (a, b), (eps, sig, m, n) in {(0, 0): (1.0, 1.02, 12.0, 6.0), (0, 1): (1.5, 0.9, 9.0, 6.0), (1, 1): (0.5, 0.95, 10.0, 5.0)}.items():
+            W.set_second_term(pot, a, b, W.KIND_GEN_LJ, eps, sig, m, 2.3 * sig, pd=n)
+    elif which == "girifalco":  # C60-like ratio beta / alpha, diameters well below the nearest-neighbour distance
+        for (a, b), (al, d) in {(0, 0): (0.17, 0.6), (0, 1): (0.25, 0.55), (1, 1): (0.1, 0.5)}.items():
+            W.set_second_term(pot, a, b, W.KIND_GIRIFALCO, al, 1.814e-3 * al, d, 3.5 * d)
+    elif which == "dzugutov":   # vanishes smoothly at 1.94 sigma: plain truncation there
+        for (a, b), (eps, sig) in {(0, 0): (0.5, 0.92), (0, 1): (0.7, 0.85), (1, 1): (0.3, 0.88)}.items():
+            W.set_second_term(pot, a, b, W.KIND_DZUGUTOV, eps, sig, 0.0, 1.94 * sig, cut=W.CUT_NONE)
     return pot
 
 
 @pytest.mark.parametrize("which,method,tp,persistent", [("ipl", "cell", 8, 1), ("yukawa", "cell", 4, 1), ("gauss", "n2", 16, 0),
-                                                        ("buck", "cell", 2, 1), ("yukawa", "none", 32, 1)])
+                                                        ("buck", "cell", 2, 1), ("yukawa", "none", 32, 1),
+                                                        ("glj", "cell", 8, 1), ("girifalco", "cell", 4, 1),
+                                                        ("dzugutov", "n2", 16, 0), ("dzugutov", "none", 32, 1),
+                                                        ("glj", "n2", 1, 0)])
 def test_other_pair_potentials_match_oracle(rumd, which, method, tp, persistent):
-    """inverse power law, Yukawa, Gaussian core and Buckingham as the second term of a type pair, on the
-    same kernels: list, forces, energies and virials against the oracle, then a short trajectory."""
+    """inverse power law, Yukawa, Gaussian core, Buckingham, generalized LJ, Girifalco and Dzugutov as the
+    second term of a type pair, on the same kernels: list, forces, energies and virials against the oracle, then a short trajectory."""
     wl = perturbed(make("ka", N=4096 if method != "none" else 512))
     wl.pot = _extra_pot(which)
     s = rumd.from_workload(wl)
@@ -723,6 +735,16 @@ def test_invalid_arguments_are_rejected(rumd):
     with pytest.raises(rumd.RumdError) as e:
         s.compute_forces()
     assert e.value.status == rumd.ERR_BOX_TOO_SMALL
+    s.set_tuning(skin=0.3)
+    with pytest.raises(rumd.RumdError):     # generalized LJ needs m > n > 0
+        s.set_pair_potential(0, 0, rumd.POT_GEN_LJ, [1.0, 1.0, 6.0, 12.0, 2.5], 0)
+    with pytest.raises(rumd.RumdError):     # Girifalco: rcut must exceed the diameter
+        s.set_pair_potential(0, 0, rumd.POT_GIRIFALCO, [1.0, 0.002, 1.0, 0.9], 0)
+    with pytest.raises(rumd.RumdError):     # wrong parameter count
+        s.set_pair_potential(0, 0, rumd.POT_DZUGUTOV, [1.0, 1.0], 0)
+    s.set_pair_potential(0, 0, rumd.POT_GEN_LJ, [1.0, 1.0, 12.0, 6.0, 2.5], 0)
+    with pytest.raises(rumd.RumdError):     # ... and it replaces the 12-6 term, which this pair still has
+        s.compute_forces()
     s.close()
 
 

@@ -547,7 +547,7 @@ def test_cutoff_methods_closed_forms():
 
 @pytest.mark.parametrize("method", [0, 1, 2])
 def test_cutoff_methods_force_is_minus_gradient(method):
-    rec = np.array([1.5, 0.8, 2.0, -1.0, 3.0, method, method, 0, 0, 0])
+    rec = np.array([1.5, 0.8, 2.0, -1.0, 3.0, method, method, 0, 0, 0, 0])
     h = 1e-6
     for r in (0.8, 1.1, 1.7, 1.95, 2.5, 2.9):
         up, _ = oracle.pair_sf(rec, r + h)
@@ -636,7 +636,7 @@ def test_extra_potentials_closed_forms():
 @pytest.mark.parametrize("method", [0, 1, 2])
 def test_extra_potentials_force_is_minus_gradient_and_cutoffs(kind, a, b, c, method):
     rc, h = 2.4, 1e-6
-    rec = np.array([0.0, 0.0, 0.0, a, rc, 0, method, kind, b, c])
+    rec = np.array([0.0, 0.0, 0.0, a, rc, 0, method, kind, b, c, 0.0])
     for r in (0.85, 1.2, 1.9, 2.39):
         up, _ = oracle.pair_sf(rec, r + h)
         um, _ = oracle.pair_sf(rec, r - h)
@@ -645,6 +645,60 @@ def test_extra_potentials_force_is_minus_gradient_and_cutoffs(kind, a, b, c, met
     assert oracle.pair_sf(rec, rc) == (0.0, 0.0) and oracle.pair_sf(rec, 3.0) == (0.0, 0.0)
     ur, fr = oracle.extra_raw(kind, 1.3, a, b, c)
     uc, fc = oracle.extra_raw(kind, rc, a, b, c)
+    want = {0: (ur - uc + (1.3 - rc) * fc, fr - fc), 1: (ur - uc, fr), 2: (ur, fr)}[method]
+    assert oracle.pair_sf(rec, 1.3) == pytest.approx(want, rel=1e-13)
+
+
+def test_generalized_lj_girifalco_dzugutov_pins():
+    """The remaining pair potentials of P:73, pinned to what does not depend on this code: generalized LJ to the 12-6
+    potential and to its defining properties; Girifalco to the C60 figures of Girifalco, J. Phys. Chem. 96, 858 (1992)
+    (alpha 74.94e-15 erg, beta 135.95e-18 erg, 2a = 7.1 A: well depth 0.2773 eV = 3218 K at 10.056 A) and to its
+    van der Waals limit; Dzugutov to the extrema of Dzugutov, Phys. Rev. A 46, R2984 (1992) (minimum -0.581 at 1.13,
+    maximum 0.460 at 1.63, zero from 1.94)."""
+    from scipy.optimize import minimize_scalar
+    # generalized LJ: (m, n) = (12, 6) is 12-6 LJ with sigma_LJ = sigma / 2^(1/6); minimum -eps at r = sigma for any (m, n)
+    eps, sig = 1.7, 1.1
+    for r in (0.95, 1.1, 1.6, 2.3):
+        assert oracle.extra_raw(5, r, eps, sig, 12.0, 6.0) == pytest.approx(oracle.lj_raw(r, eps, sig / 2 ** (1 / 6)), rel=1e-12, abs=1e-14)
+    for m, n in ((12.0, 6.0), (9.0, 6.0), (18.0, 4.0), (7.5, 3.5)):
+        u, f = oracle.extra_raw(5, sig, eps, sig, m, n)
+        assert u == pytest.approx(-eps, rel=1e-14) and abs(f) < 1e-13
+        # r -> large: -eps m / (m - n) (sig / r)^n dominates
+        u, _ = oracle.extra_raw(5, 40.0 * sig, eps, sig, m, n)
+        assert u == pytest.approx(-eps * m / (m - n) * 40.0 ** -n, rel=1e-4)
+    # Girifalco, C60 (energies in eV, lengths in Angstrom)
+    al, be, d = 74.94e-15 / 1.602177e-12, 135.95e-18 / 1.602177e-12, 7.1
+    res = minimize_scalar(lambda r: oracle.extra_raw(6, r, al, be, d)[0], bounds=(9.0, 12.0), method="bounded", options={"xatol": 1e-10})
+    assert res.x == pytest.approx(10.056, abs=2e-3) and res.fun == pytest.approx(-0.2773, abs=2e-4)
+    assert res.fun * 11604.5 == pytest.approx(-3218.0, abs=2.0)
+    assert abs(oracle.extra_raw(6, res.x, al, be, d)[1]) < 1e-7
+    u, _ = oracle.extra_raw(6, 60.0 * d, al, be, d)  # s -> infinity: -12 alpha / s^6
+    assert u == pytest.approx(-12.0 * al / 60.0 ** 6, rel=2e-3)
+    # Dzugutov (eps = sigma = 1), then scaled
+    res = minimize_scalar(lambda r: oracle.extra_raw(7, r, 1.0, 1.0)[0], bounds=(1.0, 1.4), method="bounded", options={"xatol": 1e-10})
+    assert res.x == pytest.approx(1.13, abs=2e-3) and res.fun == pytest.approx(-0.581, abs=1e-3)
+    res = minimize_scalar(lambda r: -oracle.extra_raw(7, r, 1.0, 1.0)[0], bounds=(1.4, 1.9), method="bounded", options={"xatol": 1e-10})
+    assert res.x == pytest.approx(1.63, abs=3e-3) and -res.fun == pytest.approx(0.460, abs=1e-3)
+    assert oracle.extra_raw(7, 1.94, 1.0, 1.0) == (0.0, 0.0) and oracle.extra_raw(7, 2.5, 1.0, 1.0) == (0.0, 0.0)
+    u1, f1 = oracle.extra_raw(7, 1.2, 1.0, 1.0)
+    u2, f2 = oracle.extra_raw(7, 1.2 * 1.5, 2.5, 1.5)
+    assert (u2, f2) == pytest.approx((2.5 * u1, 2.5 * f1 / 1.5), rel=1e-13)
+
+
+@pytest.mark.parametrize("kind,a,b,c,d", [(5, 1.3, 1.05, 12.0, 6.0), (5, 0.8, 1.2, 9.5, 4.0), (6, 3.0, 0.004, 0.75, 0.0),
+                                          (7, 1.4, 1.1, 0.0, 0.0)])
+@pytest.mark.parametrize("method", [0, 1, 2])
+def test_more_potentials_force_is_minus_gradient_and_cutoffs(kind, a, b, c, d, method):
+    rc, h = 2.05, 1e-6
+    rec = np.array([0.0, 0.0, 0.0, a, rc, 0, method, kind, b, c, d])
+    for r in (0.98, 1.2, 1.45, 1.9, 2.04):
+        up, _ = oracle.pair_sf(rec, r + h)
+        um, _ = oracle.pair_sf(rec, r - h)
+        _, f = oracle.pair_sf(rec, r)
+        assert f == pytest.approx(-(up - um) / (2 * h), rel=1e-6, abs=1e-8)
+    assert oracle.pair_sf(rec, rc) == (0.0, 0.0) and oracle.pair_sf(rec, 3.0) == (0.0, 0.0)
+    ur, fr = oracle.extra_raw(kind, 1.3, a, b, c, d)
+    uc, fc = oracle.extra_raw(kind, rc, a, b, c, d)
     want = {0: (ur - uc + (1.3 - rc) * fc, fr - fc), 1: (ur - uc, fr), 2: (ur, fr)}[method]
     assert oracle.pair_sf(rec, 1.3) == pytest.approx(want, rel=1e-13)
 
