@@ -66,3 +66,19 @@ def test_product_does_not_import_oracle():
                 txt = open(os.path.join(dirpath, f)).read()
                 assert not re.search(r"^\s*(import|from)\s+oracle", txt, flags=re.M), f
                 assert "rumd_oracle" not in txt, f
+
+
+def test_binding_constants_match_the_header_enums():
+    """Every enumerator of include/rumd_b200.h has the same value in the ctypes binding (RUMD_X -> rumd.X), and
+    the tuning struct of the binding has the header's fields in the header's order."""
+    from paper_1506_05094_b200 import rumd
+
+    src = open(HEADER).read()
+    enums = dict((k, int(v)) for k, v in re.findall(r"\bRUMD_([A-Z][A-Z_0-9]*)\s*=\s*(\d+)", src))
+    assert len(enums) >= 24
+    for name, value in enums.items():
+        assert getattr(rumd, name) == value, name
+    body = re.search(r"typedef struct(?:\s+\w+)?\s*\{([^}]*)\}\s*rumd_tuning\s*;", src, flags=re.S).group(1)
+    body = re.sub(r"/\*.*?\*/", "", body, flags=re.S)
+    fields = [m.group(1) for m in re.finditer(r"\b(?:int|float)\s+(\w+)\s*;", body)]
+    assert fields == [f[0] for f in rumd.Tuning._fields_]
