@@ -413,7 +413,9 @@ __device__ __forceinline__ void ph_build_cell(const Sys& S, const float4* r, con
                 const int nmax = __reduce_max_sync(FULLMASK, n);
                 const float shx = piece == 0 ? 0.f : sxh;
                 const float ax = ri.x - shx;
-                constexpr int U = 4; // candidates in flight per lane
+                // candidates in flight per lane: a stencil row holds 12-17 of them; 6 with several lanes per particle
+                // (small N, latency bound: fewer dependent rounds), 4 with one lane (large N: fewer masked slots)
+                constexpr int U = G == 1 ? 4 : 6;
                 for (int it0 = 0; it0 < nmax; it0 += U) {
                     float4 rj[U];
                     int j[U];
