@@ -313,6 +313,32 @@ __device__ __forceinline__ void ph_permute_gather(const Sys& S, const float4* r,
     }
 }
 
+// (d) and the gather in one pass (persistent kernel: one grid barrier and one phase less per sort): destination
+// slot d of cell z takes the member of the cell with exactly d - cellStart(z) smaller old indices -- the same
+// order ph_cell_finish produces -- read from the UNORDERED perm of the scatter; the first slot of a cell clears
+// the cell's histogram entry for the next sort (empty cells are already 0).
+__device__ __forceinline__ void ph_permute_gather_ranked(const Sys& S, const float4* r, int first, int stride)
+{
+    for (int d = first; d < S.N; d += stride) {
+        int src = S.perm[d];
+        const int z = S.cell_of[src];
+        const int b = S.cstart_z[z], n = S.cstart_z[z + 1] - b, want = d - b;
+        if (n > 1) {
+            for (int a = 0; a < n; ++a) {
+                const int p = S.perm[b + a];
+                int less = 0;
+                for (int q = 0; q < n; ++q) less += S.perm[b + q] < p;
+                if (less == want) src = p;
+            }
+        }
+        if (want == 0) S.ccount[z] = 0;
+        S.tmp_r[d] = r[src];
+        S.tmp_v[d] = S.v[src];
+        S.tmp_image[d] = S.image[src];
+        S.tmp_id[d] = S.id[src];
+    }
+}
+
 __device__ __forceinline__ void ph_permute_store(const Sys& S, float4* r, int first, int stride)
 {
     for (int d = first; d < S.N; d += stride) {

@@ -142,6 +142,7 @@ __global__ void __launch_bounds__(PERSIST_THREADS, PERSIST_MINB) k_persist(const
         if (flag && S.method != 2) { // (the "none" method keeps no list)
             int* max_slot = &sc->max_nbrs[n_rebuilds & 1];
             if (blockIdx.x == 0 && threadIdx.x == 0) sc->max_nbrs[(n_rebuilds + 1) & 1] = 0;
+            const float4* rsrc = rc; // where the build reads the positions from
             if (sort_on_rebuild(S, n_rebuilds)) {
                 ph_cell_assign(S, rc, first, stride);
                 PB();
@@ -157,18 +158,18 @@ __global__ void __launch_bounds__(PERSIST_THREADS, PERSIST_MINB) k_persist(const
                 PB();
                 ph_cell_scatter(S, first, stride);
                 PB();
-                ph_cell_finish(S, first, stride);
+                ph_permute_gather_ranked(S, rc, first, stride);
                 PB();
-                ph_permute_gather(S, rc, first, stride);
-                PB();
+                // the copy back into the caller's arrays shares its phase with the build, which reads the
+                // sorted positions from the scratch copy
                 ph_permute_store(S, rc, first, stride);
-                PB();
+                rsrc = S.tmp_r;
             }
             if (prof) s_prof[2] += clock64() - s_prof[4];
             if (S.method == 1)
-                build_cell_dispatch(S, rc, s_rcl2, first, stride, max_slot);
+                build_cell_dispatch(S, rsrc, s_rcl2, first, stride, max_slot);
             else
-                ph_build_n2(S, rc, s_tile, s_rcl2, blockIdx.x, gridDim.x, max_slot);
+                ph_build_n2(S, rsrc, s_tile, s_rcl2, blockIdx.x, gridDim.x, max_slot);
             n_rebuilds += 1;
             PB();
         }
