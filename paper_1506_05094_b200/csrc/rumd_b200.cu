@@ -737,7 +737,7 @@ static int launch_rebuild_chain(rumd_system* s)
     // without a rebuild each kernel only reads the flag and exits, and that costs time per BLOCK.
     const int cap256 = s->num_sms * 8, cap128 = s->num_sms * 16;
     if (sorting) {
-        const int nbp = std::min((s->N + 255) / 256, cap256), nbc = std::min((S.grid.ncell + 255) / 256, cap256);
+        const int nbp = std::min((s->N + 255) / 256, cap256);
         const int nchunks = (S.grid.ncell + SCAN_CHUNK - 1) / SCAN_CHUNK;
         k_cell_assign<<<nbp, 256, 0, s->stream>>>(S);
         if (nchunks <= 8) {
@@ -750,10 +750,9 @@ static int launch_rebuild_chain(rumd_system* s)
             n += 4;
         }
         k_cell_scatter<<<nbp, 256, 0, s->stream>>>(S);
-        k_cell_finish<<<nbc, 256, 0, s->stream>>>(S);
         k_permute_gather<<<nbp, 256, 0, s->stream>>>(S);
         k_permute_store<<<nbp, 256, 0, s->stream>>>(S);
-        n += 4;
+        n += 3;
     }
     if (s->tune.method == RUMD_NB_CELL) {
         const long long threads = (long long)s->N << S.build_tp_shift;

@@ -133,7 +133,7 @@ __device__ __forceinline__ void ph_build_n2(const Sys& S, const float4* r, float
 
 // P:276 steps 1-3: cell of every particle, sort particles by cell, rearrange all particle data.  The paper
 // calls Thrust; here it is a counting sort written out: (a) histogram with slot = atomicAdd, (b) exclusive
-// scan, (c) scatter, (d) per-cell insertion sort of the (few) entries by old index, which removes the
+// scan, (c) scatter, (d) ordering of the (few) entries of each cell by old index, which removes the
 // atomic's arbitrary order so that the particle order -- and with it every later fp32 sum -- is
 // reproducible.  Sort key of cell (x, y, z) = rowrank[z][y] * nx + x, where rowrank numbers the (y, z) cell
 // columns along a 2-D Morton (Z-order) curve (table built once on the host): consecutive particles are
@@ -280,43 +280,13 @@ __device__ __forceinline__ void ph_cell_scatter(const Sys& S, int first, int str
     for (int i = first; i < S.N; i += stride) S.perm[S.cstart_z[S.cell_of[i]] + S.slot[i]] = i;
 }
 
-// One thread per cell: order its entries by old index (deterministic) and clear the histogram for the next
-// sort.  cellStart is the scan output cstart_z[key]; cellEnd of a cell = cellStart of the next key
-// (EXCLUSIVE, S20; cstart_z[ncell] = N).
-__device__ __forceinline__ void ph_cell_finish(const Sys& S, int first, int stride)
-{
-    for (int z = first; z < S.grid.ncell; z += stride) {
-        const int b = S.cstart_z[z], n = S.ccount[z];
-        for (int a = 1; a < n; ++a) {
-            const int key = S.perm[b + a];
-            int q = a - 1;
-            while (q >= 0 && S.perm[b + q] > key) {
-                S.perm[b + q + 1] = S.perm[b + q];
-                --q;
-            }
-            S.perm[b + q + 1] = key;
-        }
-        S.ccount[z] = 0;
-    }
-}
-
 // P:276 "rearrange all particle data into the sorted order": gather into scratch, then copy back (the
 // caller owns the arrays, so the pointers cannot be swapped).
-__device__ __forceinline__ void ph_permute_gather(const Sys& S, const float4* r, int first, int stride)
-{
-    for (int d = first; d < S.N; d += stride) {
-        const int src = S.perm[d];
-        S.tmp_r[d] = r[src];
-        S.tmp_v[d] = S.v[src];
-        S.tmp_image[d] = S.image[src];
-        S.tmp_id[d] = S.id[src];
-    }
-}
-
-// (d) and the gather in one pass (persistent kernel: one grid barrier and one phase less per sort): destination
-// slot d of cell z takes the member of the cell with exactly d - cellStart(z) smaller old indices -- the same
-// order ph_cell_finish produces -- read from the UNORDERED perm of the scatter; the first slot of a cell clears
-// the cell's histogram entry for the next sort (empty cells are already 0).
+// Step (d) and the gather in one pass: destination slot d of cell z takes the member of the cell with exactly
+// d - cellStart(z) smaller old indices (cells hold a handful of particles), read from the UNORDERED perm of the
+// scatter; the first slot of a cell clears the cell's histogram entry for the next sort (empty cells are
+// already 0).  cellStart is the scan output cstart_z[key]; cellEnd of a cell = cellStart of the next
+// key (EXCLUSIVE, S20; cstart_z[ncell] = N).
 __device__ __forceinline__ void ph_permute_gather_ranked(const Sys& S, const float4* r, int first, int stride)
 {
     for (int d = first; d < S.N; d += stride) {
@@ -569,18 +539,11 @@ static __global__ void k_cell_scatter(const Sys S)
     ph_cell_scatter(S, first, stride);
 }
 
-static __global__ void k_cell_finish(const Sys S)
-{
-    if (!sort_requested(S)) return;
-    VGRID;
-    ph_cell_finish(S, first, stride);
-}
-
 static __global__ void k_permute_gather(const Sys S)
 {
     if (!sort_requested(S)) return;
     VGRID;
-    ph_permute_gather(S, S.r, first, stride);
+    ph_permute_gather_ranked(S, S.r, first, stride);
 }
 
 static __global__ void k_permute_store(const Sys S)
