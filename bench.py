@@ -150,7 +150,7 @@ def whole_job_rate(units_per_rank: float, seconds_local: float, world: int, devi
 # DRAM bytes (read + write) per MD time step of the dominant kernel, from the committed ncu --set full captures
 # (profiles/r01_persist_c1_ncu.md: 4.87 MB per 200-step k_persist launch at C1; profiles/r01_force_lj1m_ncu.md:
 # 376.8 MB per k_force launch at C3).  Workloads without a capture report traffic = null.
-NCU_DRAM_BYTES_PER_TIMESTEP = {"ka8000": 4.87e6 / 200, "lj1m": 376.8e6}
+NCU_DRAM_BYTES_PER_TIMESTEP = {"ka8000": 4.70e6 / 200, "lj1m": 376.8e6}
 
 FLOP_PER_LISTED_PAIR_LJ = 42.0       # SURVEY.md 8(d) / DESIGN.md "Roofline": 21 always + 30 x 0.712 inside rc
 FLOP_PER_LISTED_PAIR_COUL = 50.0     # + the Coulomb term
