@@ -148,7 +148,7 @@ def whole_job_rate(units_per_rank: float, seconds_local: float, world: int, devi
 # ------------------------------------------------------------------------------------------------ GPU arm
 
 # DRAM bytes (read + write) per MD time step of the dominant kernel, from the committed ncu --set full captures
-# (profiles/r01_persist_c1_ncu.md: 4.87 MB per 200-step k_persist launch at C1; profiles/r01_force_lj1m_ncu.md:
+# (profiles/r01_persist_c1_ncu.md: 4.70 MB per 200-step k_persist launch at C1; profiles/r01_force_lj1m_ncu.md:
 # 376.8 MB per k_force launch at C3).  Workloads without a capture report traffic = null.
 NCU_DRAM_BYTES_PER_TIMESTEP = {"ka8000": 4.70e6 / 200, "lj1m": 376.8e6}
 
