@@ -282,30 +282,25 @@ __device__ __forceinline__ void ph_cell_scatter(const Sys& S, int first, int str
 
 // P:276 "rearrange all particle data into the sorted order": gather into scratch, then copy back (the
 // caller owns the arrays, so the pointers cannot be swapped).
-// Step (d) and the gather in one pass: destination slot d of cell z takes the member of the cell with exactly
-// d - cellStart(z) smaller old indices (cells hold a handful of particles), read from the UNORDERED perm of the
-// scatter; the first slot of a cell clears the cell's histogram entry for the next sort (empty cells are
-// already 0).  cellStart is the scan output cstart_z[key]; cellEnd of a cell = cellStart of the next
-// key (EXCLUSIVE, S20; cstart_z[ncell] = N).
+// Step (d) and the gather in one pass: the particle in (unordered) slot d of the scatter finds its rank among
+// the members of its cell by old index (cells hold a handful of particles) and moves its data to
+// cellStart + rank; the first slot of a cell clears the cell's histogram entry for the next sort (empty cells
+// are already 0).  cellStart is the scan output cstart_z[key]; cellEnd of a cell = cellStart of the
+// next key (EXCLUSIVE, S20; cstart_z[ncell] = N).
 __device__ __forceinline__ void ph_permute_gather_ranked(const Sys& S, const float4* r, int first, int stride)
 {
     for (int d = first; d < S.N; d += stride) {
-        int src = S.perm[d];
+        const int src = S.perm[d];
         const int z = S.cell_of[src];
-        const int b = S.cstart_z[z], n = S.cstart_z[z + 1] - b, want = d - b;
-        if (n > 1) {
-            for (int a = 0; a < n; ++a) {
-                const int p = S.perm[b + a];
-                int less = 0;
-                for (int q = 0; q < n; ++q) less += S.perm[b + q] < p;
-                if (less == want) src = p;
-            }
-        }
-        if (want == 0) S.ccount[z] = 0;
-        S.tmp_r[d] = r[src];
-        S.tmp_v[d] = S.v[src];
-        S.tmp_image[d] = S.image[src];
-        S.tmp_id[d] = S.id[src];
+        const int b = S.cstart_z[z], n = S.cstart_z[z + 1] - b;
+        int less = 0;
+        for (int q = 0; q < n; ++q) less += S.perm[b + q] < src;
+        if (d == b) S.ccount[z] = 0;
+        const int dst = b + less;
+        S.tmp_r[dst] = r[src];
+        S.tmp_v[dst] = S.v[src];
+        S.tmp_image[dst] = S.image[src];
+        S.tmp_id[dst] = S.id[src];
     }
 }
 
