@@ -5,6 +5,7 @@
 // stand-alone __global__ kernels (one phase each, early exit when no rebuild is requested) and the
 // persistent whole-run kernel (rumd_persist.cuh: all phases, grid barriers in between) both call the phases.
 #pragma once
+#include <type_traits>
 #include "rumd_types.cuh"
 
 #define FULLMASK 0xffffffffu
@@ -353,6 +354,9 @@ __device__ __forceinline__ void ph_build_cell(const Sys& S, const float4* r, con
             w1 = cx + 2 - nx;
         }
         int count = 0;
+        // warp-uniform fast path: no lane's stencil crosses a face of the box -> no wrapped x piece, no y / z shifts
+        const bool interior = __all_sync(FULLMASK, !have_i || (cx >= 2 && cx + 2 < nx && cy >= 2 && cy + 2 < ny &&
+                                                               cz >= 2 && cz + 2 < nz));
         // Minimum image without per-pair rounding work: all candidates of one range lie in cells reached with
         // the same periodic shift s in {-1, 0, +1} per axis (s != 0 where the stencil row, or the wrapped x
         // segment, crossed a face), and d = (x_i - s h) - (x_j + s h) is the exact nearest-image displacement
@@ -360,11 +364,16 @@ __device__ __forceinline__ void ph_build_cell(const Sys& S, const float4* r, con
         // n >= 5 cells per axis, S18).  sxh: shift of the wrapped x segment; the main segment has none.
         const float sxh = cx - 2 < 0 ? -S.h[0] : S.h[0];
         // particle ranges of stencil row q (0..24): main [a.x, a.y) and wrapped [b.x, b.y); its y / z shifts
-        auto ranges_of = [&](int q, int2& a, int2& b, float& syh, float& szh) {
+        auto ranges_of = [&](auto INT, int q, int2& a, int2& b, float& syh, float& szh) {
             a = b = make_int2(0, 0);
             syh = szh = 0.f;
             if (!have_i || q >= 25) return;
             int z = cz + q / 5 - 2, y = cy + q % 5 - 2;
+            if (decltype(INT)::value) {
+                const int* cs = S.cstart_z + S.rowrank[z * ny + y] * nx;
+                a = make_int2(cs[cx - 2], cs[cx + 3]);
+                return;
+            }
             if (z < 0) {
                 z += nz;
                 szh = -S.h[2];
@@ -388,17 +397,19 @@ __device__ __forceinline__ void ph_build_cell(const Sys& S, const float4* r, con
         const int tmask = (1 << S.tp_shift) - 1;
         // list cutoffs of this particle's type against every type (S4), held in registers
         const float c0 = s_rcl2[trow], c1 = s_rcl2[trow + 1], c2 = s_rcl2[trow + 2], c3 = s_rcl2[trow + 3];
+        auto walk = [&](auto INT) {
+        constexpr bool I = decltype(INT)::value;
         int2 na, nb;
         float nsy, nsz;
-        ranges_of(l, na, nb, nsy, nsz);
+        ranges_of(INT, l, na, nb, nsy, nsz);
         for (int q0 = 0; q0 < 25; q0 += G) {
             const int2 a = na, b = nb;
             const float syh = nsy, szh = nsz;
-            if (q0 + G < 25) ranges_of(q0 + G + l, na, nb, nsy, nsz); // one-ahead prefetch of the next round's ranges
+            if (q0 + G < 25) ranges_of(INT, q0 + G + l, na, nb, nsy, nsz); // one-ahead prefetch of the next round's ranges
             const float ay = ri.y - syh, az = ri.z - szh;
             // the main piece of the row, then its x-wrapped piece (empty except next to the x faces)
 #pragma unroll
-            for (int piece = 0; piece < 2; ++piece) {
+            for (int piece = 0; piece < (I ? 1 : 2); ++piece) {
                 const int start = piece == 0 ? a.x : b.x;
                 const int n = piece == 0 ? a.y - a.x : b.y - b.x;
                 const int nmax = __reduce_max_sync(FULLMASK, n);
@@ -418,7 +429,9 @@ __device__ __forceinline__ void ph_build_cell(const Sys& S, const float4* r, con
 #pragma unroll
                     for (int q = 0; q < U; ++q) {
                         const float dx = piece == 0 ? ri.x - rj[q].x : ax - (rj[q].x + shx);
-                        const float dy = ay - (rj[q].y + syh), dz = az - (rj[q].z + szh);
+                        // interior: syh = szh = 0, the same values without the two additions
+                        const float dy = I ? ri.y - rj[q].y : ay - (rj[q].y + syh);
+                        const float dz = I ? ri.z - rj[q].z : az - (rj[q].z + szh);
                         const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, dx * dx));
                         const int tj = type_of(rj[q]);
                         const float thr = S.ntypes <= 2 ? (tj ? c1 : c0) : (tj == 0 ? c0 : tj == 1 ? c1 : tj == 2 ? c2 : c3);
@@ -440,6 +453,9 @@ __device__ __forceinline__ void ph_build_cell(const Sys& S, const float4* r, con
                 }
             }
         }
+        };
+        if (interior) walk(std::true_type{});
+        else walk(std::false_type{});
         if (have_i && l == 0) {
             S.num_nbrs[i] = min(count, S.cap);
             S.r_build[i] = ri;
