@@ -354,6 +354,7 @@ __device__ __forceinline__ void ph_build_cell(const Sys& S, const float4* r, con
             w1 = cx + 2 - nx;
         }
         int count = 0;
+        const int isafe = have_i ? i : 0; // in-bounds stand-in for the masked slots of lanes past the last particle
         // warp-uniform fast path: no lane's stencil crosses a face of the box -> no wrapped x piece, no y / z shifts
         const bool interior = __all_sync(FULLMASK, !have_i || (cx >= 2 && cx + 2 < nx && cy >= 2 && cy + 2 < ny &&
                                                                cz >= 2 && cz + 2 < nz));
@@ -423,8 +424,8 @@ __device__ __forceinline__ void ph_build_cell(const Sys& S, const float4* r, con
                     int j[U];
 #pragma unroll
                     for (int q = 0; q < U; ++q) {
-                        j[q] = it0 + q < n ? start + it0 + q : i; // masked: gather the particle itself (n > 0 => have_i)
-                        rj[q] = r[have_i ? j[q] : 0];
+                        j[q] = it0 + q < n ? start + it0 + q : isafe; // masked: gather the particle itself (n > 0 => have_i)
+                        rj[q] = r[j[q]];
                     }
 #pragma unroll
                     for (int q = 0; q < U; ++q) {
