@@ -438,10 +438,8 @@ __device__ __forceinline__ void ph_build_cell(const Sys& S, const float4* r, con
                         const float thr = S.ntypes <= 2 ? (tj ? c1 : c0) : (tj == 0 ? c0 : tj == 1 ? c1 : tj == 2 ? c2 : c3);
                         const bool acc = have_i && j[q] != i && d2 < thr;
                         if (G == 1) { // the lane owns the row: no slot negotiation
-                            if (acc) {
-                                if (count < S.cap) rowbase[((count >> S.tp_shift) << 5) + (count & tmask)] = j[q];
-                                ++count;
-                            }
+                            if (acc && count < S.cap) rowbase[((count >> S.tp_shift) << 5) + (count & tmask)] = j[q];
+                            count += acc ? 1 : 0;
                         } else {
                             const unsigned m = __ballot_sync(FULLMASK, acc);
                             if (acc) {
