@@ -147,10 +147,15 @@ def whole_job_rate(units_per_rank: float, seconds_local: float, world: int, devi
 
 # ------------------------------------------------------------------------------------------------ GPU arm
 
-# DRAM bytes (read + write) per MD time step of the dominant kernel, from the committed ncu --set full captures
-# (profiles/r01_persist_c1_ncu.md: 4.70 MB per 200-step k_persist launch at C1; profiles/r01_force_lj1m_ncu.md:
-# 376.8 MB per k_force launch at C3).  Workloads without a capture report traffic = null.
-NCU_DRAM_BYTES_PER_TIMESTEP = {"ka8000": 4.70e6 / 200, "lj1m": 376.8e6}
+# ncu --set full captures of the dominant kernels (dram__bytes_read.sum + dram__bytes_write.sum per launch) live
+# under profiles/ and are named here; `roofline.traffic` carries a number only when bench.py is pointed at one that
+# was taken on the same workload and commit (it is a profiler measurement, never re-measured inside a timed run).
+TRAFFIC_PROFILES = {"ka8000": "profiles/r02_persist_c1_ncu.md", "lj1m": "profiles/r02_force_lj1m_ncu.md",
+                    "ka65536": "profiles/r02_force_ka65536_ncu.md"}
+
+# The paper's parameter file (P:382 step 8): tunings found by rumd_autotune on "NVIDIA B200", keyed by GPU name, N,
+# box, potentials, integrator; a hit costs no trial run, a miss tunes and appends.
+TUNING_CACHE = os.path.join(ROOT, "paper_1506_05094_b200", "tuning_b200.jsonl")
 
 FLOP_PER_LISTED_PAIR_LJ = 42.0       # SURVEY.md 8(d) / DESIGN.md "Roofline": 21 always + 30 x 0.712 inside rc
 FLOP_PER_LISTED_PAIR_COUL = 50.0     # + the Coulomb term
@@ -174,15 +179,48 @@ def count_listed(s):
 
 
 def equilibrate(s, wl, steps):
-    """Untimed: leave the lattice start (hot transient, frequent rebuilds; SURVEY 8(d) C2 note)."""
+    """Untimed: leave the lattice start (hot transient, frequent rebuilds; SURVEY 8(d) C2 note).  A block that
+    overflowed the list ran with truncated rows (missing forces): it is repeated from the state held before it.
+    That state is kept in the System's pinned host buffers, because the in-workspace snapshot does not survive
+    the re-bind that doubles the capacity."""
     done = 0
     while done < steps:
         n = min(500, steps - done)
+        s.download_state(s.h_r, s.h_v, None, None, s.h_image, s.h_id)
         s.run_steps(n)
         th = s.get_thermo(grow=True)
-        if th is None:       # list overflow -> capacity doubled (P:101); repeat from the last good state
+        if th is None:       # list overflow -> workspace re-bound with doubled capacity: redo the block
+            s.upload_state()
             continue
         done += n
+
+
+def roofline_of(s, wl, name, tun, ms_per_timestep, inner, peaks, fp32_measured, sm_mhz):
+    """Roofline entries of one workload: the stand-alone pair-force kernel (timed alone: rumd_time_force replays
+    200 launches from a graph between two CUDA events on the library's stream) and the whole time step.
+    achieved = algorithmic flop (42 / 50 per LISTED pair) x live listed pairs / duration."""
+    N = wl.N
+    listed = count_listed(s)
+    us = s.time_force(reps=200 if N < 500000 else 50)
+    coul = bool((wl.pot[..., 4] > 0).any())
+    flop_pp = FLOP_PER_LISTED_PAIR_COUL if coul else FLOP_PER_LISTED_PAIR_LJ
+    flop = flop_pp * listed
+    peak_tf = fp32_peak_tflops(peaks["sm_max_mhz"])
+    ach_force = flop / (us * 1e-6) / 1e12
+    ach_step = flop / (ms_per_timestep * 1e-3) / 1e12
+    alg_bytes = 4.0 * listed + (16 + 4 + 20) * N
+    return {
+        "listed_pairs": listed, "mean_nbrs": listed / N, "flop_per_listed_pair": flop_pp,
+        "force_kernel": {"kernel": "k_force (stand-alone, current tuning)", "us_per_launch": us,
+                         "achieved": ach_force, "unit": "TFLOP/s", "frac": ach_force / peak_tf,
+                         "frac_of_measured_fp32": ach_force / fp32_measured if fp32_measured else None,
+                         "hbm_equiv_gbs": alg_bytes / (us * 1e-6) / 1e9,
+                         "hbm_frac": alg_bytes / (us * 1e-6) / 1e9 / peaks["hbm_gbs"]},
+        "whole_step": {"us_per_timestep": ms_per_timestep * 1e3, "achieved": ach_step, "frac": ach_step / peak_tf,
+                       "frac_of_measured_fp32": ach_step / fp32_measured if fp32_measured else None,
+                       "frac_at_observed_clock": ach_step / fp32_peak_tflops(sm_mhz)},
+        "algorithmic_bytes_per_timestep": alg_bytes,
+    }
 
 
 def run_gpu(args, rank, world, local_rank):
@@ -199,8 +237,8 @@ def run_gpu(args, rank, world, local_rank):
     equilibrate(s, wl, args.equil)
     tune_info = {}
     if args.autotune:
-        t, tps = s.autotune(steps_per_trial=args.tune_steps)
-        tune_info = {"autotuned": True, "trial_tps": tps}
+        t, tps = s.autotune(steps_per_trial=args.tune_steps, cache_path=TUNING_CACHE if args.tuning_cache else None)
+        tune_info = {"autotuned": True, "tuning_from_cache": bool(s.tuning_from_cache), "trial_tps": tps}
     tun = s.get_tuning().as_dict()
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)  # > 126 MB L2
 
@@ -234,6 +272,9 @@ def run_gpu(args, rank, world, local_rank):
     ms = max_over_ranks(ms, world, dev)
     tsteps = args.steps * inner
     tps = world * tsteps / (ms * 1e-3)
+    # the equilibrated state the timed region ran on, in ORIGINAL particle order: input of the cpu_baseline leg
+    eq_state = s.state() if rank == 0 else None
+    eq_thermo = th1
 
     # ---- end-to-end arm: host buffers through the C ABI, H2D + D2H inside the timed region
     h_r = torch.empty((N, 4), dtype=torch.float32).pin_memory()
@@ -262,43 +303,38 @@ def run_gpu(args, rank, world, local_rank):
 
     out = None
     if rank == 0:
-        # ---- roofline of the dominant kernel (pair force), timed live with CUDA events on the library's stream
-        listed = count_listed(s)
-        us = s.time_force(reps=200)
-        coul = bool((wl.pot[..., 4] > 0).any())
-        flop = (FLOP_PER_LISTED_PAIR_COUL if coul else FLOP_PER_LISTED_PAIR_LJ) * listed
         peaks = measured_peaks()
+        fp32_measured = s.measure_fp32_peak(5)
         sm_mhz = clocks.get("sm_mhz") or peaks["sm_max_mhz"]
         peak_tf = fp32_peak_tflops(peaks["sm_max_mhz"])
-        ach_tf = flop / (us * 1e-6) / 1e12
-        alg_bytes = 4.0 * listed + (16 + 4 + 20) * N
-        s.profile_step()          # first call pays CUDA's lazy loading of the un-fused kernels
-        prof = s.profile_step()
-        flop_pp = flop / listed
-        force_kernel = {"kernel": "k_force (stand-alone, current tuning)", "us_per_launch": us, "achieved": ach_tf,
-                        "frac": ach_tf / peak_tf, "hbm_equiv_gbs": alg_bytes / (us * 1e-6) / 1e9,
-                        "hbm_peak_gbs": peaks["hbm_gbs"], "unfused_step_ms": prof}
+        rl = roofline_of(s, wl, args.workload, tun, ms / tsteps, inner, peaks, fp32_measured, sm_mhz)
         if tun["persistent"]:
             # the dominant kernel IS the whole run: one k_persist launch = `inner` time steps; its duration is the
             # CUDA-event time of the timed region itself
             us_launch = 1e3 * ms / args.steps
-            ach = flop * inner / (us_launch * 1e-6) / 1e12
             phases = s.profile_persistent(inner)
             roof = {"kernel": "k_persist (one launch = %d time steps: rebuilds + forces + integration)" % inner,
-                    "bound": "alu", "achieved": ach, "peak": peak_tf, "unit": "TFLOP/s", "frac": ach / peak_tf,
-                    "traffic": (NCU_DRAM_BYTES_PER_TIMESTEP[args.workload] * inner
-                                if args.workload in NCU_DRAM_BYTES_PER_TIMESTEP else None),
-                    "traffic_source": "ncu dram__bytes_read.sum + dram__bytes_write.sum, profiles/r01_*_ncu.md",
-                    "algorithmic_bytes": alg_bytes * inner,
-                    "us_per_launch": us_launch, "phases_us_per_timestep": phases}
+                    "bound": "alu", "achieved": rl["whole_step"]["achieved"], "peak": peak_tf, "unit": "TFLOP/s",
+                    "frac": rl["whole_step"]["frac"], "us_per_launch": us_launch, "phases_us_per_timestep": phases,
+                    "algorithmic_bytes": rl["algorithmic_bytes_per_timestep"] * inner}
         else:
-            roof = {"kernel": "k_force", "bound": "alu", "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s",
-                    "frac": ach_tf / peak_tf, "traffic": None, "us_per_launch": us,
-                    "force_share_of_step": us * 1e-3 / (ms / tsteps)}
-        roof.update({"peak_source": "derived: 148 SMs x 128 FP32 lanes x 2 x %.0f MHz (max SM clock, %s)" % (
-                         peaks["sm_max_mhz"], peaks["source"]),
-                     "frac_at_observed_clock": roof["achieved"] / fp32_peak_tflops(sm_mhz),
-                     "listed_pairs": listed, "flop_per_listed_pair": flop_pp, "force_kernel": force_kernel})
+            fk = rl["force_kernel"]
+            roof = {"kernel": "k_force", "bound": "alu", "achieved": fk["achieved"], "peak": peak_tf,
+                    "unit": "TFLOP/s", "frac": fk["frac"], "us_per_launch": fk["us_per_launch"],
+                    "force_share_of_step": fk["us_per_launch"] * 1e-3 / (ms / tsteps)}
+        roof.update({
+            "traffic": None,
+            "traffic_source": "ncu --set full capture (dram__bytes_read.sum + dram__bytes_write.sum): %s" %
+                              TRAFFIC_PROFILES.get(args.workload, "none for this workload"),
+            "peak_source": "derived: 148 SMs x 128 FP32 lanes x 2 x %.0f MHz (max SM clock, %s)" % (
+                peaks["sm_max_mhz"], peaks["source"]),
+            "peak_measured_ffma": fp32_measured,
+            "frac_of_measured_fp32": roof["achieved"] / fp32_measured if fp32_measured else None,
+            "frac_at_observed_clock": roof["achieved"] / fp32_peak_tflops(sm_mhz),
+            "regime": "N = %d: %s" % (N, "latency / dependency chain (SURVEY 8(d)): no throughput roofline applies; "
+                                      "see sweep[] for N >= 65536" if N < 30000 else "FP32 ALU"),
+            "listed_pairs": rl["listed_pairs"], "flop_per_listed_pair": rl["flop_per_listed_pair"],
+            "force_kernel": rl["force_kernel"], "hbm_peak_gbs": peaks["hbm_gbs"]})
         out = {
             "metric": "timesteps/s", "value": tps, "unit": "timesteps/s", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
@@ -309,47 +345,69 @@ def run_gpu(args, rank, world, local_rank):
                        "l2": "256 MiB L2 flush between timed iterations (outside the event pairs)",
                        "parallelism": "replicas x%d" % world,
                        "rebuilds_in_window": th1["n_rebuilds"] - th0["n_rebuilds"], "max_nbrs": th1["max_nbrs"],
-                       "mean_nbrs": listed / N},
+                       "mean_nbrs": rl["mean_nbrs"],
+                       "nvt_note": "Nose-Hoover discretisation and tau = 0.2 are readings (the paper prints "
+                                   "neither, P:54, P:78): NVT parity against the paper is unpinned"},
             "clocks": clocks,
             "e2e": {"value": e2e_tps, "unit": "timesteps/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
             "gpu_launches": int(l1 - l0),
             "roofline": roof,
             "thermo": {k: th1[k] for k in ("U", "K", "H", "xi")},
         }
+        out["_eq_state"] = (eq_state, eq_thermo)
+        out["_headline_row"] = sweep_row(args.workload, N, tps, ms / tsteps, tun, rl, th1["n_rebuilds"] - th0["n_rebuilds"],
+                                         tsteps, tune_info)
     s.close()
     return out
 
 
+def sweep_row(name, N, tps, ms_per_timestep, tun, rl, rebuilds, tsteps, info):
+    fk, ws = rl["force_kernel"], rl["whole_step"]
+    return {"workload": name, "N": N, "timesteps_per_s": tps, "particle_steps_per_s": tps * N,
+            "us_per_timestep": 1e3 * ms_per_timestep,
+            "tuning": {k: tun[k] for k in ("method", "tp", "skin", "build_tp", "persistent")},
+            "tuning_from_cache": info.get("tuning_from_cache"),
+            "rebuild_interval": tsteps / max(1, rebuilds), "mean_nbrs": rl["mean_nbrs"],
+            "k_force_us": fk["us_per_launch"], "k_force_frac_fp32": fk["frac"],
+            "k_force_frac_of_measured_fp32": fk["frac_of_measured_fp32"], "k_force_hbm_frac": fk["hbm_frac"],
+            "whole_step_frac_fp32": ws["frac"], "whole_step_frac_of_measured_fp32": ws["frac_of_measured_fp32"]}
+
+
 # ------------------------------------------------------------------------------------------------ N sweep
 
-SWEEP = ["lj864", "ka512", "ka1000", "ka2048", "ka4096", "ka8000", "ka8192", "ka16384", "ka32768", "ka65536",
-         "ka131072", "charged", "lj1m"]
+# BASELINE.json metric "timesteps/s and particle-steps/s vs N; % FP32/HBM roofline": rows emitted by the DEFAULT run
+# beside the configs[1] headline (which is itself the N = 8000 row).  --sweep-all adds every size of configs[0..4].
+SWEEP_DEFAULT = ["ka1000", "ka65536", "ka131072", "charged", "lj1m"]
+SWEEP_ALL = ["lj864", "ka512", "ka1000", "ka2048", "ka4096", "ka8192", "ka16384", "ka32768", "ka65536", "ka131072",
+             "charged", "lj1m"]
 
 
-def run_sweep(args, names):
-    """BASELINE.json metric "timesteps/s and particle-steps/s vs N": device-resident arm only, one entry per
-    workload, each autotuned (configs[2]) after equilibration.  Not part of the default run."""
+def run_sweep(args, names, fp32_measured):
+    """Device-resident arm only, one row per workload: equilibrated, tuned (tuning file first), timed with
+    CUDA events on the library's stream, then the stand-alone force kernel and the roofline fractions."""
     import torch
 
     from paper_1506_05094_b200 import rumd
 
     peaks = measured_peaks()
-    peak_tf = fp32_peak_tflops(peaks["sm_max_mhz"])
     out = []
     for name in names:
+        t_row = time.perf_counter()
         wl, desc = make_workload(name)
         s = rumd.from_workload(wl)
         N = wl.N
         equilibrate(s, wl, args.equil if N < 500000 else 500)
         info = {}
         if args.autotune:
-            t, tps_trial = s.autotune(steps_per_trial=args.tune_steps if N < 500000 else 60)
-            info["trial_tps"] = tps_trial
+            t, tps_trial = s.autotune(steps_per_trial=args.tune_steps if N < 500000 else 60,
+                                      cache_path=TUNING_CACHE if args.tuning_cache else None)
+            info = {"tuning_from_cache": bool(s.tuning_from_cache), "trial_tps": tps_trial}
         inner = max(50, min(args.inner, int(2e8 / N)))
         for _ in range(3):
             s.run_steps(inner)
         th0 = s.get_thermo()
-        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(5)]
+        reps = 5
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(reps)]
         with torch.cuda.stream(s.stream):
             for a, b in ev:
                 a.record(s.stream)
@@ -358,20 +416,17 @@ def run_sweep(args, names):
         torch.cuda.synchronize()
         ms = sum(a.elapsed_time(b) for a, b in ev)
         th1 = s.get_thermo()
-        tps = 5 * inner / (ms * 1e-3)
-        listed = count_listed(s)
-        us = s.time_force(reps=50)
-        coul = bool((wl.pot[..., 4] > 0).any())
-        flop = (FLOP_PER_LISTED_PAIR_COUL if coul else FLOP_PER_LISTED_PAIR_LJ) * listed
+        tps = reps * inner / (ms * 1e-3)
         tun = s.get_tuning().as_dict()
-        phases = s.profile_persistent(inner) if tun["persistent"] else None
-        out.append({"workload": name, "N": N, "timesteps_per_s": tps, "particle_steps_per_s": tps * N,
-                    "us_per_timestep": 1e3 * ms / (5 * inner), "tuning": tun, **info,
-                    "rebuild_interval": 5 * inner / max(1, th1["n_rebuilds"] - th0["n_rebuilds"]),
-                    "mean_nbrs": listed / N, "whole_step_frac_fp32": flop / (1e-3 * ms / (5 * inner)) / 1e12 / peak_tf,
-                    "force_kernel_us": us, "force_kernel_frac_fp32": flop / (us * 1e-6) / 1e12 / peak_tf,
-                    "phases_us_per_timestep": phases})
-        print("sweep %s: %.0f timesteps/s" % (name, tps), file=sys.stderr, flush=True)
+        rl = roofline_of(s, wl, name, tun, ms / (reps * inner), inner, peaks, fp32_measured, peaks["sm_max_mhz"])
+        row = sweep_row(name, N, tps, ms / (reps * inner), tun, rl, th1["n_rebuilds"] - th0["n_rebuilds"], reps * inner, info)
+        if tun["persistent"] and args.phases:
+            row["phases_us_per_timestep"] = s.profile_persistent(inner)
+        row["wall_s"] = time.perf_counter() - t_row
+        out.append(row)
+        print("sweep %s: %.0f timesteps/s, k_force %.1f us = %.3f of FP32" % (name, tps, row["k_force_us"],
+                                                                              row["k_force_frac_fp32"]),
+              file=sys.stderr, flush=True)
         s.close()
     return out
 
@@ -422,53 +477,92 @@ def run_ensembles(args, specs):
 # ------------------------------------------------------------------------------------------------ oracle arm
 
 
-def oracle_sample(wl, nsteps):
-    """Time the fp64 oracle, as it stands, for nsteps whole time steps of this workload on the host cores."""
+def cpu_model() -> str:
+    try:
+        for ln in open("/proc/cpuinfo"):
+            if ln.startswith("model name"):
+                return ln.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def oracle_sample(wl, nsteps, state=None, threads=None):
+    """Time the fp64 oracle, as it stands, for nsteps whole time steps of this workload on the host cores.
+    state: (r, v, image, xi, eta) to start from (fp32-representable values); default the workload's t = 0."""
     import oracle
 
+    if threads is not None:
+        oracle.set_num_threads(threads)
+    r, v, image, xi, eta = state if state is not None else (wl.r, wl.v, np.zeros((wl.N, 3), np.int32), 0.0, 0.0)
     t0 = time.perf_counter()
-    o = oracle.run(wl.r.astype(np.float64), wl.v.astype(np.float64), wl.m.astype(np.float64),
-                   np.zeros((wl.N, 3), np.int32), wl.types, wl.box.astype(np.float64), wl.pot, float(wl.skin),
-                   float(wl.dt), int(nsteps), mode=wl.integrator, T0=wl.T0, tau=wl.tau, use_cell=wl.N >= 4096,
-                   want_log=False)
+    o = oracle.run(np.asarray(r, np.float64), np.asarray(v, np.float64), wl.m.astype(np.float64),
+                   np.asarray(image, np.int32), wl.types, wl.box.astype(np.float64), wl.pot, float(wl.skin),
+                   float(wl.dt), int(nsteps), mode=wl.integrator, T0=wl.T0, tau=wl.tau, xi=xi, eta=eta,
+                   use_cell=wl.N >= 4096, want_log=False)
     dt_ = time.perf_counter() - t0
-    return nsteps / dt_, dt_, o["n_builds"], oracle.num_threads()
+    return nsteps / dt_, dt_, o, oracle.num_threads()
 
 
-def cpu_baseline(wl, target_s=12.0):
-    tps0, dt0, _, cores = oracle_sample(wl, 4)
+def cpu_baseline(wl, state, target_s=12.0, one_core_s=5.0):
+    """The oracle on the SAME equilibrated state the GPU arm was timed on (downloaded, original particle order),
+    all host cores, plus a 1-core figure."""
+    import oracle
+
+    all_cores = oracle.num_threads()
+    oracle_sample(wl, 2, state)                       # first call: library load, thread pool
+    tps0, _, _, cores = oracle_sample(wl, 24, state)
     n = int(max(8, min(20000, target_s * tps0)))
-    tps, dt_, nb, cores = oracle_sample(wl, n)
-    return {"value": tps, "unit": "timesteps/s", "cores": cores, "kind": "oracle",
-            "sample": "%d time steps of the same workload from its t=0 state (%d list builds), %.1f s, fp64, "
-                      "OpenMP over particles" % (n, nb, dt_)}
+    tps, dt_, o, cores = oracle_sample(wl, n, state)
+    oracle.set_num_threads(1)
+    tps1_0, _, _, _ = oracle_sample(wl, 2, state)
+    n1 = int(max(2, min(5000, one_core_s * tps1_0)))
+    tps1, dt1, _, _ = oracle_sample(wl, n1, state)
+    oracle.set_num_threads(all_cores)
+    return {"value": tps, "unit": "timesteps/s", "cores": cores, "kind": "oracle", "cpu_model": cpu_model(),
+            "one_core": {"value": tps1, "unit": "timesteps/s", "cores": 1,
+                         "sample": "%d time steps, %.1f s" % (n1, dt1)},
+            "same_state_as_gpu_arm": True,
+            "sample": "%d time steps of the same workload from the equilibrated state the GPU arm was timed on "
+                      "(%d list builds), %.1f s, fp64, skin %.2f, OpenMP over particles" % (n, o["n_builds"], dt_,
+                                                                                           float(wl.skin))}
 
 
 def run_reference(args, rank, world):
-    """--impl reference: the oracle on the host cores, same config/metric; each bench step is a bounded
-    sample (inner_ref time steps)."""
+    """--impl reference: the oracle on the host cores, same config/metric.  Like the GPU arm it first leaves the
+    lattice start (args.equil untimed steps, run by the oracle itself: nothing of the CUDA path is on this arm),
+    then each bench step is a bounded sample (inner_ref time steps) continuing from that state."""
     if rank != 0:
         return None
     wl, desc = make_workload(args.workload)
     tps0, _, _, cores = oracle_sample(wl, 2)
-    # whole run (warmup + steps) bounded to ~60 s
+    equil = int(min(args.equil, max(0, 45.0 * tps0)))          # bounded: at most ~45 s of equilibration
+    st = None
+    if equil > 0:
+        _, _, o, _ = oracle_sample(wl, equil)
+        st = (o["r"], o["v"], o["image"], o["xi"], o["eta"])
+    tps0, _, _, cores = oracle_sample(wl, 2, st)
+    # timed part (warmup + steps) bounded to ~60 s
     inner_ref = int(max(1, min(args.inner, 60.0 * tps0 / max(1, args.steps + args.warmup))))
     times = []
     nb = 0
     for it in range(args.warmup + args.steps):
-        tps, dt_, b, cores = oracle_sample(wl, inner_ref)
+        tps, dt_, o, cores = oracle_sample(wl, inner_ref, st)
+        st = (o["r"], o["v"], o["image"], o["xi"], o["eta"])
         if it >= args.warmup:
             times.append(dt_)
-            nb += b
+            nb += o["n_builds"]
     total = sum(times)
     val = args.steps * inner_ref / total
-    sample = "%d bench steps x %d time steps of the workload from t=0 (%d list builds)" % (args.steps, inner_ref, nb)
+    sample = ("%d bench steps x %d time steps, continuing from the state after %d untimed equilibration steps of "
+              "the oracle (%d list builds in the timed part)" % (args.steps, inner_ref, equil, nb))
     return {"impl": "reference", "metric": "timesteps/s", "value": val, "unit": "timesteps/s", "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "particle_steps_per_s": val * wl.N,
-            "config": {"workload": desc, "N": wl.N, "md_timesteps_per_step": inner_ref},
-            "cpu_baseline": {"value": val, "unit": "timesteps/s", "cores": cores, "kind": "oracle", "sample": sample},
+            "config": {"workload": desc, "N": wl.N, "md_timesteps_per_step": inner_ref, "equilibration_steps": equil},
+            "cpu_baseline": {"value": val, "unit": "timesteps/s", "cores": cores, "kind": "oracle",
+                             "cpu_model": cpu_model(), "sample": sample},
             "e2e": {"value": val, "unit": "timesteps/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
 
@@ -486,10 +580,16 @@ def main():
     ap.add_argument("--workload", default="ka8000")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-autotune", dest="autotune", action="store_false")
+    ap.add_argument("--no-tuning-cache", dest="tuning_cache", action="store_false",
+                    help="tune from scratch instead of reading / appending paper_1506_05094_b200/tuning_b200.jsonl")
     ap.add_argument("--tune-steps", type=int, default=300)
     ap.add_argument("--no-cpu-baseline", dest="cpu", action="store_false")
+    ap.add_argument("--no-sweep", dest="sweep_default", action="store_false",
+                    help="skip the N sweep rows of the default run")
     ap.add_argument("--sweep", nargs="*", default=None, metavar="WORKLOAD",
-                    help="also time the N sweep (all of configs[0..4] when no names are given) -> key 'sweep'")
+                    help="sweep these workloads (no names: every size of configs[0..4]) instead of the default rows")
+    ap.add_argument("--phases", action="store_true", help="add in-kernel phase timings to the sweep rows")
+    ap.add_argument("--ensembles", action="store_true", help="also time the batched ensembles")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
 
@@ -513,14 +613,19 @@ def main():
         torch.distributed.init_process_group("nccl", device_id=torch.device("cuda:%d" % local_rank))
     out = run_gpu(args, rank, world, local_rank)
     if rank == 0:
+        eq_state, eq_thermo = out.pop("_eq_state")
+        headline_row = out.pop("_headline_row")
         if args.cpu and world == 1:
             wl, _ = make_workload(args.workload)
-            out["cpu_baseline"] = cpu_baseline(wl)
+            st = (eq_state["r"], eq_state["v"], eq_state["image"], eq_thermo["xi"], eq_thermo["eta"])
+            out["cpu_baseline"] = cpu_baseline(wl, st)
         else:
             out["cpu_baseline"] = None
-        if args.sweep is not None and world == 1:
-            out["sweep"] = run_sweep(args, args.sweep or SWEEP)
-            if not args.sweep:
+        if world == 1 and (args.sweep is not None or args.sweep_default):
+            names = SWEEP_DEFAULT if args.sweep is None else (args.sweep or SWEEP_ALL)
+            rows = run_sweep(args, [n for n in names if n != args.workload], out["roofline"]["peak_measured_ffma"])
+            out["sweep"] = sorted(rows + [headline_row], key=lambda r: (r["N"], r["workload"]))
+            if args.ensembles:
                 out["ensembles"] = run_ensembles(args, ENSEMBLES)
         print(json.dumps(out), flush=True)
     if world > 1:

@@ -217,7 +217,9 @@ rumd_status rumd_restore(rumd_system* s);
 
 /* HOST-buffer entry points (used for end-to-end timing): copy the state from / to host arrays of the same
  * layouts as rumd_bind_state (any pointer may be NULL = skip).  Upload requests a rebuild and resets the
- * thermostat.  Download synchronizes the stream. */
+ * thermostat; it checks that every particle type in h_r lies in [0, n_types) (RUMD_ERR_INVALID_ARG otherwise:
+ * the type indexes the pair table in every kernel; arrays written directly through the device pointers of
+ * rumd_bind_state are the caller's responsibility).  Download synchronizes the stream. */
 rumd_status rumd_upload_state(rumd_system* s, const void* h_r, const void* h_v, const void* h_image,
                               const void* h_id);
 rumd_status rumd_download_state(rumd_system* s, void* h_r, void* h_v, void* h_f, void* h_w, void* h_image,
@@ -240,6 +242,13 @@ rumd_status rumd_time_force(rumd_system* s, int reps, float* us_per_launch);
  * force + integrate, the sort part of the rebuild, block sums + grid barrier wait, unused}, whole kernel per
  * step, number of rebuilds, grid size.  Advances the simulation by nsteps.  Synchronizes. */
 rumd_status rumd_profile_persistent(rumd_system* s, int nsteps, double* out8);
+
+/* Measured FP32 peak of this GPU (the roofline fractions are quoted against the derived
+ * 148 SMs x 128 lanes x 2 flop x clock AND against this measurement): a kernel of independent register-operand
+ * FFMA chains at full occupancy, best of reps launches, CUDA events on the library's stream.  tflops_out: host,
+ * TFLOP/s counting 2 flop per FFMA.  Needs a bound workspace (4 bytes of it are the kernel's dummy output).
+ * Synchronizes. */
+rumd_status rumd_measure_fp32_peak(rumd_system* s, int reps, double* tflops_out);
 
 const char* rumd_last_error(const rumd_system* s);
 const char* rumd_version(void);

@@ -45,6 +45,7 @@ struct rumd_system {
     float dt = 0, T0 = 0, tau = 0;
     rumd_tuning tune;
     int cap = 0;
+    size_t nc_carved = 0;   // cells the bound workspace was carved (and its histogram zeroed) for
     void* ws = nullptr;
     size_t ws_bytes = 0;
     // snapshot area
@@ -321,6 +322,7 @@ extern "C" rumd_status rumd_bind_workspace(rumd_system* s, void* d_ws, size_t by
         CUDA_TRY(s, cudaStreamSynchronize(s->stream));
     }
     carve(s, (char*)d_ws, cap);
+    s->nc_carved = max_cells(s);
     s->ws = d_ws;
     s->ws_bytes = bytes;
     s->cap = cap;
@@ -328,7 +330,7 @@ extern "C" rumd_status rumd_bind_workspace(rumd_system* s, void* d_ws, size_t by
     s->params_dirty = true;
     s->grid_for[0] = s->grid_for[1] = s->grid_for[2] = 0;
     drop_graphs(s);
-    CUDA_TRY(s, cudaMemsetAsync(s->S.ccount, 0, max_cells(s) * 4, s->stream));
+    CUDA_TRY(s, cudaMemsetAsync(s->S.ccount, 0, s->nc_carved * 4, s->stream));
     CUDA_TRY(s, cudaMemsetAsync(s->S.num_nbrs, 0, align_up((size_t)s->N, 32) * (size_t)s->nrep * 4, s->stream));
     if (had) {
         keep.flag = 1u;
@@ -336,6 +338,7 @@ extern "C" rumd_status rumd_bind_workspace(rumd_system* s, void* d_ws, size_t by
         keep.ticket = 0u;
         keep.overflow = 0u;
         keep.max_nbrs[0] = keep.max_nbrs[1] = 0;
+        keep.last_max = 0;
         *s->h_sc = keep;
         CUDA_TRY(s, cudaMemcpyAsync(s->S.sc, s->h_sc, sizeof keep, cudaMemcpyHostToDevice, s->stream));
         CUDA_TRY(s, cudaStreamSynchronize(s->stream));
@@ -600,7 +603,11 @@ static rumd_status refresh(rumd_system* s)
     int n[3];
     grid_dims(s, skin, n);
     const size_t ncell = (size_t)n[0] * n[1] * n[2];
-    if (ncell > max_cells(s)) return fail(s, RUMD_ERR_NOT_READY, "cell grid outgrew the workspace: set potentials before binding the workspace");
+    // the cell arrays were sized from the potentials in force when the workspace was bound: a shorter rc_max set
+    // afterwards makes a finer grid than was carved
+    if (ncell > s->nc_carved)
+        return fail(s, RUMD_ERR_NOT_READY, "cell grid (%zu cells) outgrew the workspace (carved for %zu): re-bind the workspace after changing the potentials",
+                    ncell, s->nc_carved);
     if (t.method == RUMD_NB_CELL && (n[0] < 5 || n[1] < 5 || n[2] < 5))
         return fail(s, RUMD_ERR_BOX_TOO_SMALL, "cell method needs >= 5 cells per axis (S18), have %dx%dx%d", n[0], n[1], n[2]);
     S.grid.n[0] = n[0];
@@ -963,8 +970,10 @@ extern "C" rumd_status rumd_get_thermo(rumd_system* s, rumd_thermo* out)
     out->H = H;
     out->n_steps = d.n_steps;
     out->n_rebuilds = d.n_rebuilds;
-    // slot of the last completed build (a build whose force evaluation has not run yet still owns the flag)
-    const int max_nbrs = d.max_nbrs[(d.flag ? d.n_rebuilds : d.n_rebuilds + 1) & 1];
+    // longest row of the last completed build; a list built by rumd_build_nblist whose force evaluation has not
+    // run yet still owns the flag and its slot (a flag raised by the displacement check finds that slot zeroed)
+    int max_nbrs = d.last_max;
+    if (d.flag && d.max_nbrs[d.n_rebuilds & 1] > 0) max_nbrs = d.max_nbrs[d.n_rebuilds & 1];
     out->max_nbrs = max_nbrs;
     out->nbl_capacity = s->cap;
     out->overflow = (int)d.overflow;
@@ -1048,6 +1057,12 @@ extern "C" rumd_status rumd_upload_state(rumd_system* s, const void* h_r, const 
     rumd_status st = ready(s, false);
     if (st != RUMD_OK) return st;
     const size_t N = (size_t)s->N * (size_t)s->nrep;
+    if (h_r) { // the type in r.w indexes the pair table in every kernel: check it here, where it is cheap
+        const int* bits = (const int*)h_r;
+        for (size_t i = 0; i < N; ++i)
+            if (bits[4 * i + 3] < 0 || bits[4 * i + 3] >= s->ntypes)
+                return fail(s, RUMD_ERR_INVALID_ARG, "particle %zu has type %d, outside [0, %d)", i, bits[4 * i + 3], s->ntypes);
+    }
     if (h_r) CUDA_TRY(s, cudaMemcpyAsync(s->S.r, h_r, N * 16, cudaMemcpyHostToDevice, s->stream));
     if (h_v) CUDA_TRY(s, cudaMemcpyAsync(s->S.v, h_v, N * 16, cudaMemcpyHostToDevice, s->stream));
     if (h_image) CUDA_TRY(s, cudaMemcpyAsync(s->S.image, h_image, N * 16, cudaMemcpyHostToDevice, s->stream));
@@ -1082,24 +1097,31 @@ extern "C" rumd_status rumd_profile_step(rumd_system* s, float* ms_out, int* did
     rumd_status st = ready(s, true);
     if (st != RUMD_OK) return st;
     if (!ms_out) return fail(s, RUMD_ERR_INVALID_ARG, "null output");
-    cudaEvent_t ev[4];
-    for (auto& e : ev) CUDA_TRY(s, cudaEventCreate(&e));
     CUDA_TRY(s, cudaMemcpyAsync(s->h_sc, s->S.sc, sizeof(DevScalars), cudaMemcpyDeviceToHost, s->stream));
     CUDA_TRY(s, cudaStreamSynchronize(s->stream));
     const int did = s->h_sc->flag != 0;
-    cudaEventRecord(ev[0], s->stream);
-    s->launches += launch_rebuild_chain(s);
-    cudaEventRecord(ev[1], s->stream);
-    s->launches += launch_force(s);
-    cudaEventRecord(ev[2], s->stream);
-    s->launches += launch_integrate(s);
-    cudaEventRecord(ev[3], s->stream);
-    CUDA_TRY(s, cudaStreamSynchronize(s->stream));
-    for (int q = 0; q < 3; ++q) cudaEventElapsedTime(&ms_out[q], ev[q], ev[q + 1]);
+    cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+    cudaError_t e = cudaSuccess;
+    for (auto& x : ev)
+        if (e == cudaSuccess) e = cudaEventCreate(&x);
+    if (e == cudaSuccess) {
+        cudaEventRecord(ev[0], s->stream);
+        s->launches += launch_rebuild_chain(s);
+        cudaEventRecord(ev[1], s->stream);
+        s->launches += launch_force(s);
+        cudaEventRecord(ev[2], s->stream);
+        s->launches += launch_integrate(s);
+        cudaEventRecord(ev[3], s->stream);
+        e = cudaStreamSynchronize(s->stream);
+    }
+    if (e == cudaSuccess)
+        for (int q = 0; q < 3 && e == cudaSuccess; ++q) e = cudaEventElapsedTime(&ms_out[q], ev[q], ev[q + 1]);
+    for (auto& x : ev) // the events are destroyed on every path
+        if (x) cudaEventDestroy(x);
+    if (e == cudaSuccess) e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(s, RUMD_ERR_CUDA, "profile step failed: %s", cudaGetErrorString(e));
     ms_out[3] = 0.f;
     if (did_rebuild_out) *did_rebuild_out = did;
-    for (auto& e : ev) cudaEventDestroy(e);
-    CUDA_TRY(s, cudaGetLastError());
     return RUMD_OK;
 }
 
@@ -1170,6 +1192,57 @@ extern "C" rumd_status rumd_profile_persistent(rumd_system* s, int nsteps, doubl
     out8[5] = us_total / nsteps;
     out8[6] = (double)h[6];
     out8[7] = (double)h[7];
+    return RUMD_OK;
+}
+
+// FP32 peak as measured, not derived ("the builder should add an FFMA-chain microbenchmark and quote
+// fractions against both the formula and the measured value").  Every thread runs 16 independent register-operand
+// FFMA chains; 2 blocks of 1024 threads per SM (full occupancy), so the FMA pipes never wait on a dependency.
+#define PEAK_CHAINS 16
+static __global__ void __launch_bounds__(1024, 2) k_ffma_peak(float* out, int iters, float b0, float c0)
+{
+    float x[PEAK_CHAINS];
+    const float b = b0 + 1e-9f * (float)threadIdx.x, c = c0 + 1e-9f * (float)blockIdx.x;
+#pragma unroll
+    for (int q = 0; q < PEAK_CHAINS; ++q) x[q] = (float)(threadIdx.x + q);
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+#pragma unroll
+            for (int q = 0; q < PEAK_CHAINS; ++q) x[q] = __fmaf_rn(x[q], b, c);
+    }
+    float acc = 0.f;
+#pragma unroll
+    for (int q = 0; q < PEAK_CHAINS; ++q) acc += x[q];
+    if (acc == 123.456f) out[0] = acc; // never true in practice: keeps the chains alive
+}
+
+// Measured FP32 FMA throughput of this GPU in TFLOP/s (2 flop per FFMA): best of `reps` launches timed with CUDA
+// events on the library's stream.  scratch: any 4 writable device bytes are taken from the workspace.
+extern "C" rumd_status rumd_measure_fp32_peak(rumd_system* s, int reps, double* tflops_out)
+{
+    if (!s || !tflops_out || reps < 1) return RUMD_ERR_INVALID_ARG;
+    if (!s->ws_bound) return fail(s, RUMD_ERR_NOT_READY, "bind a workspace first");
+    const int iters = 4096, blocks = 2 * s->num_sms, threads = 1024;
+    const double flop = 2.0 * 4.0 * PEAK_CHAINS * (double)iters * (double)blocks * threads;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    cudaError_t e = cudaEventCreate(&e0);
+    if (e == cudaSuccess) e = cudaEventCreate(&e1);
+    double best = 0.0;
+    for (int r = 0; r <= reps && e == cudaSuccess; ++r) { // launch 0 is the warm-up
+        cudaEventRecord(e0, s->stream);
+        k_ffma_peak<<<blocks, threads, 0, s->stream>>>((float*)s->prof_buf, iters, 0.999f, 0.001f);
+        cudaEventRecord(e1, s->stream);
+        e = cudaStreamSynchronize(s->stream);
+        float ms = 0.f;
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+        if (e == cudaSuccess && r > 0 && ms > 0.f) best = std::max(best, flop / (ms * 1e-3) / 1e12);
+        s->launches++;
+    }
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    if (e != cudaSuccess) return fail(s, RUMD_ERR_CUDA, "fp32 peak measurement failed: %s", cudaGetErrorString(e));
+    *tflops_out = best;
     return RUMD_OK;
 }
 

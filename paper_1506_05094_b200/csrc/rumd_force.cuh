@@ -296,6 +296,7 @@ __device__ __forceinline__ void finish_rebuild(const Sys& S)
 {
     if (S.sc->flag != 0u) {
         if (S.method != 2) { // (the "none" method has no list: nothing was built)
+            S.sc->last_max = S.sc->max_nbrs[S.sc->n_rebuilds & 1];
             S.sc->n_rebuilds += 1;
             S.sc->max_nbrs[S.sc->n_rebuilds & 1] = 0;
         }

@@ -172,6 +172,7 @@ __global__ void __launch_bounds__(PERSIST_THREADS, PERSIST_MINB) k_persist(const
                 ph_build_n2(S, rsrc, s_tile, s_rcl2, blockIdx.x, gridDim.x, max_slot);
             n_rebuilds += 1;
             PB();
+            if (blockIdx.x == 0 && threadIdx.x == 0) sc->last_max = __ldcg(max_slot);
         }
         PROF_LAP(0)
 

@@ -41,7 +41,7 @@ struct DevScalars {
     unsigned int overflow;
     int max_nbrs[2];      // largest list length of build number b in slot b & 1
     int nonfinite;        // 1: NaN/Inf energy; 2: grid barrier timed out
-    int pad0;
+    int last_max;         // largest list length of the last COMPLETED build (written when its force evaluation starts)
 };
 
 struct CellGrid {
@@ -71,6 +71,12 @@ struct Sys {
     float4* tmp_r; float4* tmp_v; int4* tmp_image; int* tmp_id;
     int* cell_of; int* slot; int* perm;
     int* ccount; int* cstart_z; int* rowrank; int* blocksum; // cstart_z: ncell + 1 entries; rowrank: ny*nz
+    // tile method (rumd_tile.cuh): the cell grid is cut into nt[0] x nt[1] x nt[2] tiles of <= TILE_WMAX cells per axis
+    int nt[3], ntiles;
+    int hcap;               // shared-memory halo slots per tile (slot hcap is the far-away dummy)
+    int cap_it8;            // uint4 list chunks (8 entries) per lane: cap / (8 tp)
+    int* halo_idx;          // [ntiles][hcap]: global particle index | ghost bits << 28 of every halo slot
+    int* halo_cnt;          // [ntiles]: halo slots in use
     long long* prof;        // nullptr, or 8 cycle counters filled by block 0 of the persistent kernel (profiling run)
     double* partial;        // 2 sets x 2 doubles per block (kt, mv2) of the integrating kernel
     DevScalars* sc;

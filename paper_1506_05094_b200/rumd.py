@@ -14,7 +14,7 @@ import numpy as np
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_LIBPATH = os.environ.get("RUMD_B200_LIB") or os.path.join(_HERE, "librumd_b200.so")  # override: A/B builds
+_LIBPATH = os.path.join(_HERE, "librumd_b200.so")
 
 OK, ERR_INVALID_ARG, ERR_NOT_READY, ERR_CUDA, ERR_NBL_OVERFLOW, ERR_BOX_TOO_SMALL, ERR_NONFINITE = range(7)
 POT_LJ_12_6, POT_COULOMB, POT_IPL, POT_YUKAWA, POT_GAUSSIAN_CORE, POT_BUCKINGHAM = range(6)
@@ -29,7 +29,7 @@ EXPORTS = [
     "rumd_set_pair_potential", "rumd_set_integrator", "rumd_default_tuning", "rumd_set_tuning",
     "rumd_get_tuning", "rumd_autotune", "rumd_autotune_cached", "rumd_build_nblist", "rumd_compute_forces", "rumd_run_steps",
     "rumd_export_nblist", "rumd_get_thermo", "rumd_snapshot", "rumd_restore", "rumd_upload_state",
-    "rumd_download_state", "rumd_launch_count", "rumd_profile_step", "rumd_time_force", "rumd_profile_persistent", "rumd_set_replicas", "rumd_get_thermo_replicas", "rumd_last_error", "rumd_version",
+    "rumd_download_state", "rumd_launch_count", "rumd_profile_step", "rumd_time_force", "rumd_profile_persistent", "rumd_measure_fp32_peak", "rumd_set_replicas", "rumd_get_thermo_replicas", "rumd_last_error", "rumd_version",
 ]
 
 
@@ -97,6 +97,7 @@ def lib():
         L.rumd_profile_step.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(ip)]
         L.rumd_time_force.argtypes = [vp, ip, C.POINTER(C.c_float)]
         L.rumd_profile_persistent.argtypes = [vp, ip, C.POINTER(C.c_double)]
+        L.rumd_measure_fp32_peak.argtypes = [vp, ip, C.POINTER(C.c_double)]
         L.rumd_set_replicas.argtypes = [vp, ip]
         L.rumd_get_thermo_replicas.argtypes = [vp, C.POINTER(Thermo), ip]
         L.rumd_last_error.argtypes = [vp]
@@ -135,6 +136,10 @@ class System:
             r = r.reshape(R * self.N, 3)
         N = r.shape[0]                  # elements of the state arrays
         self.ntypes = int(pot.shape[0])
+        types = np.ascontiguousarray(types, dtype=np.int32)
+        if types.shape != (N,) or types.min() < 0 or types.max() >= self.ntypes:
+            # the type indexes the pair table inside every kernel: reject a bad one here, where it is cheap
+            raise RumdError(ERR_INVALID_ARG, "particle types must be %d integers in [0, %d)" % (N, self.ntypes))
         self.box = np.ascontiguousarray(box, dtype=np.float32)
         # a dedicated side stream (the legacy default stream cannot be captured into CUDA graphs)
         self.stream = stream if stream is not None else torch.cuda.Stream(self.device)
@@ -315,6 +320,12 @@ class System:
         us = C.c_float()
         self._check(self.L.rumd_time_force(self.h, int(reps), C.byref(us)))
         return float(us.value)
+
+    def measure_fp32_peak(self, reps=5) -> float:
+        """Measured FP32 FFMA throughput of this GPU, TFLOP/s."""
+        out = C.c_double()
+        self._check(self.L.rumd_measure_fp32_peak(self.h, int(reps), C.byref(out)))
+        return float(out.value)
 
     def profile_persistent(self, nsteps=1000) -> dict:
         out = (C.c_double * 8)()
