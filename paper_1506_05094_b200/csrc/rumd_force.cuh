@@ -350,7 +350,10 @@ __device__ __forceinline__ void integrate_particle(const Sys& S, float a, float 
     v.y = vy;
     v.z = vz;
     float x = __fmaf_rn(S.dt, vx, r.x), y = __fmaf_rn(S.dt, vy, r.y), z = __fmaf_rn(S.dt, vz, r.z);
-    const float nx = rintf(x * S.invL[0]), ny = rintf(y * S.invL[1]), nz = rintf(z * S.invL[2]);
+    // (tile method: no wrap between rebuilds, see ph_cell_assign)
+    const bool wrap = S.method != 3;
+    const float nx = wrap ? rintf(x * S.invL[0]) : 0.f, ny = wrap ? rintf(y * S.invL[1]) : 0.f,
+                nz = wrap ? rintf(z * S.invL[2]) : 0.f;
     x = __fmaf_rn(-nx, S.L[0], x);
     y = __fmaf_rn(-ny, S.L[1], y);
     z = __fmaf_rn(-nz, S.L[2], z);

@@ -79,6 +79,51 @@ __device__ __forceinline__ float list_dist2(const Sys& S, const float4& ri, cons
     return __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, dx * dx));
 }
 
+// ------------------------------------------------------------------------------------------ tile geometry
+// Tile method (RUMD_NB_TILE, rumd_tile.cuh): the cell grid of S17 is cut into nt[0] x nt[1] x nt[2] boxes of cells
+// ("tiles", balanced widths: tile j of an axis with n cells covers cells [j n / nt, (j+1) n / nt)).  Particles are
+// sorted TILE-MAJOR -- key = cells of all earlier tiles (tiles ordered z, y, x; x fastest) + row-major cell index
+// inside the tile -- so that the particles a tile owns are ONE contiguous range and the cells of one x-row of a
+// tile are contiguous too.
+struct TileGeo {
+    int x0, y0, z0, wx, wy, wz; // first cell and width per axis
+    int cellbase;               // sort key of the tile's first cell
+};
+
+__device__ __forceinline__ TileGeo tile_geo(const Sys& S, int t)
+{
+    const int nx = S.grid.n[0], ny = S.grid.n[1], nz = S.grid.n[2];
+    const int tx = t % S.nt[0], ty = (t / S.nt[0]) % S.nt[1], tz = t / (S.nt[0] * S.nt[1]);
+    TileGeo g;
+    g.x0 = tx * nx / S.nt[0];
+    g.wx = (tx + 1) * nx / S.nt[0] - g.x0;
+    g.y0 = ty * ny / S.nt[1];
+    g.wy = (ty + 1) * ny / S.nt[1] - g.y0;
+    g.z0 = tz * nz / S.nt[2];
+    g.wz = (tz + 1) * nz / S.nt[2] - g.z0;
+    // whole z-slabs of tiles below, whole rows of tiles at lower y in this slab, tiles at lower x in this row
+    g.cellbase = g.z0 * ny * nx + g.wz * (g.y0 * nx + g.wy * g.x0);
+    return g;
+}
+
+__device__ __forceinline__ int tile_of_cell(int c, int nt, int n) { return ((c + 1) * nt - 1) / n; }
+
+__device__ __forceinline__ int tile_index_of_cell(const Sys& S, int cx, int cy, int cz)
+{
+    return (tile_of_cell(cz, S.nt[2], S.grid.n[2]) * S.nt[1] + tile_of_cell(cy, S.nt[1], S.grid.n[1])) * S.nt[0] +
+           tile_of_cell(cx, S.nt[0], S.grid.n[0]);
+}
+
+__device__ __forceinline__ int tile_cell_key(const Sys& S, int cx, int cy, int cz)
+{
+    const TileGeo g = tile_geo(S, tile_index_of_cell(S, cx, cy, cz));
+    return g.cellbase + ((cz - g.z0) * g.wy + (cy - g.y0)) * g.wx + (cx - g.x0);
+}
+
+// List rows of the tile method are addressed by a PADDED particle index, so that the rows of one tile start at a
+// warp boundary: particle i of tile t (own range starting at o0) has row index pbase(t) + (i - o0).
+__device__ __forceinline__ int tile_pbase(int o0, int t) { return ((o0 + 31) & ~31) + 32 * t; }
+
 // ------------------------------------------------------------------------------------------ A2: N^2 build
 
 // P:173-224 Fig. 4.  One WARP per particle i; j-positions staged through shared memory in tiles
@@ -142,12 +187,30 @@ __device__ __forceinline__ void ph_build_n2(const Sys& S, const float4* r, float
 // order, so the 5 x-neighbour cells of a stencil row are ONE particle range (cellStart of the first cell to
 // cellStart of the cell after the last) -- the build then walks 25 ranges instead of 125 cells.
 
-__device__ __forceinline__ void ph_cell_assign(const Sys& S, const float4* r, int first, int stride)
+// Tile method: between rebuilds the integrator leaves coordinates that crossed a face UNWRAPPED (they stay within
+// skin/2 of the box, O9), so that the periodic images fixed in a tile's halo at build time stay valid; the wrap into
+// [-L/2, L/2) and the image counters (S7) are applied here, at the start of the next rebuild.
+__device__ __forceinline__ void ph_cell_assign(const Sys& S, float4* r, int first, int stride)
 {
     for (int i = first; i < S.N; i += stride) {
         int cx, cy, cz;
-        cell_coords(S, r[i], cx, cy, cz);
-        const int z = S.rowrank[cz * S.grid.n[1] + cy] * S.grid.n[0] + cx;
+        float4 p = r[i];
+        if (S.method == 3) {
+            const float nx = rintf(p.x * S.invL[0]), ny = rintf(p.y * S.invL[1]), nz = rintf(p.z * S.invL[2]);
+            if (nx != 0.f || ny != 0.f || nz != 0.f) {
+                p.x = __fmaf_rn(-nx, S.L[0], p.x);
+                p.y = __fmaf_rn(-ny, S.L[1], p.y);
+                p.z = __fmaf_rn(-nz, S.L[2], p.z);
+                int4 im = S.image[i];
+                im.x += (int)nx;
+                im.y += (int)ny;
+                im.z += (int)nz;
+                S.image[i] = im;
+                r[i] = p;
+            }
+        }
+        cell_coords(S, p, cx, cy, cz);
+        const int z = S.method == 3 ? tile_cell_key(S, cx, cy, cz) : S.rowrank[cz * S.grid.n[1] + cy] * S.grid.n[0] + cx;
         S.cell_of[i] = z;
         S.slot[i] = atomicAdd(&S.ccount[z], 1);
     }

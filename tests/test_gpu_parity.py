@@ -1094,7 +1094,9 @@ def test_particle_types_are_validated_on_the_host(rumd):
         rumd.System(wl.r, wl.v, wl.m, bad, wl.box, wl.pot)
     assert e.value.status == rumd.ERR_INVALID_ARG
     s = rumd.from_workload(wl)
-    s.h_r[5, 3] = np.array([-1], np.int32).view(np.float32)[0]
+    import torch
+
+    s.h_r.view(torch.int32)[5, 3] = -1
     with pytest.raises(rumd.RumdError) as e:
         s.upload_state()
     assert e.value.status == rumd.ERR_INVALID_ARG
