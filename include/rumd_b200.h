@@ -69,7 +69,13 @@ typedef enum { RUMD_INT_NVE_LEAPFROG = 0, RUMD_INT_NVT_NOSE_HOOVER = 1 } rumd_in
 typedef enum {
     RUMD_NB_N2 = 0,   /* P:173 "n2": tiled all-pairs list build */
     RUMD_NB_CELL = 1, /* P:276 "sort": spatial sort + cell-list build */
-    RUMD_NB_NONE = 2  /* P:371 "none": no list at all, every force evaluation loops over all pairs (small N) */
+    RUMD_NB_NONE = 2, /* P:371 "none": no list at all, every force evaluation loops over all pairs (small N) */
+    RUMD_NB_TILE = 3  /* spatial sort + cell-list build like RUMD_NB_CELL, with the j-particles staged in shared
+                         memory: the cell grid is cut into tiles, a thread block loads the positions of a tile and of
+                         the two cells around it once and both the build and the force kernel gather from there;
+                         16-bit list entries.  Needs tp <= 8 and >= 6 cells per axis.  Between list rebuilds the
+                         coordinates in d_r may leave [-L/2, L/2] by up to skin/2 (they are wrapped, and d_image
+                         updated, at the next rebuild); d_r + d_image * L is the unwrapped position at all times */
 } rumd_nb_method;
 
 /* Tunable launch parameters (Table 2: NB method, pb, tp, skin; P:379 sort interval).
@@ -89,7 +95,9 @@ typedef enum {
  *                 256 threads, pb is not used); 0: per-step kernels (early-exit rebuild chain, then force +
  *                 integrate, fused into one kernel per step inside CUDA graphs).
  *   build_tp      lanes per particle of the cell-list build, one of 1,2,4,8,16,32 ("not been tried
- *                 yet"); 0 = library default for this N. */
+ *                 yet"); 0 = library default for this N.
+ *   tile          RUMD_NB_TILE only: target edge of a tile in cells, 1..8 (a tile owns about tile^3 cells and stages
+ *                 (tile + 4)^3 of them in shared memory); 0 = library default for this N. */
 typedef struct {
     int method;
     int pb;
@@ -100,6 +108,7 @@ typedef struct {
     int steps_per_graph;
     int persistent;
     int build_tp;
+    int tile;
 } rumd_tuning;
 
 /* Thermodynamic scalars, all double, filled by rumd_get_thermo (host struct).

@@ -127,6 +127,10 @@ static size_t max_cells(const rumd_system* s)
     return t;
 }
 
+// tile method: bounds used to size the workspace (refresh() checks the actual tiling against them)
+static size_t tile_bound(const rumd_system* s) { return align_up((size_t)s->N, 32) / 32 - 1; } // tiles, at most
+static size_t halo_slots_bound(const rumd_system* s) { return s->nrep > 1 ? 64 : 20 * (size_t)s->N + 65536; }
+
 static uint32_t part1by1(uint32_t x) // spread the low 16 bits to the even bit positions
 {
     x &= 0x0000ffff;
@@ -154,6 +158,8 @@ static size_t carve(rumd_system* s, char* base, int cap)
     void* p;
     p = take(sizeof(DevScalars)); if (base) S.sc = (DevScalars*)p;
     p = take(sizeof(DevScalars)); if (base) s->snap_sc = (DevScalars*)p;
+    // (tile method: 16-bit entries, rows padded to a warp boundary per tile -> Npad + 32 (tiles + 1) rows of 2 cap
+    // bytes, which fits this array as long as there are at most Npad / 32 - 1 tiles: tile_bound)
     p = take(Npad * (size_t)cap * 4); if (base) S.nbl = (int*)p;
     p = take(Npad * 4); if (base) S.num_nbrs = (int*)p;
     p = take(N * 16); if (base) S.r_build = (float4*)p;
@@ -177,6 +183,8 @@ static size_t carve(rumd_system* s, char* base, int cap)
     const size_t nblk = std::max<size_t>(N + 1, 2 * 4096); // the fused per-step kernel may run N blocks (pb = 1)
     p = take(nblk * 16); if (base) S.partial = (double*)p;
     p = take(8 * 8); if (base) s->prof_buf = (long long*)p;
+    p = take(halo_slots_bound(s) * 4); if (base) S.halo_idx = (int*)p;
+    p = take((tile_bound(s) + 1) * 4); if (base) S.halo_cnt = (int*)p;
     if (R > 1) {
         p = take(R * sizeof(Sys)); if (base) s->d_systems = (Sys*)p;
         p = take(R * sizeof(DevScalars)); if (base) s->ens_sc = (DevScalars*)p;
@@ -427,6 +435,7 @@ extern "C" rumd_status rumd_default_tuning(const rumd_system* s, rumd_tuning* t)
     t->steps_per_graph = 0;
     t->persistent = 1;
     t->build_tp = 0;
+    t->tile = 0;
     return RUMD_OK;
 }
 
@@ -435,8 +444,10 @@ static bool valid_tp(int tp) { return tp == 1 || tp == 2 || tp == 4 || tp == 8 |
 extern "C" rumd_status rumd_set_tuning(rumd_system* s, const rumd_tuning* t)
 {
     if (!s || !t) return RUMD_ERR_INVALID_ARG;
-    if (t->method != RUMD_NB_N2 && t->method != RUMD_NB_CELL && t->method != RUMD_NB_NONE)
+    if (t->method != RUMD_NB_N2 && t->method != RUMD_NB_CELL && t->method != RUMD_NB_NONE && t->method != RUMD_NB_TILE)
         return fail(s, RUMD_ERR_INVALID_ARG, "bad method");
+    if (t->method == RUMD_NB_TILE && t->tp > 8) return fail(s, RUMD_ERR_INVALID_ARG, "the tile method takes tp <= 8");
+    if (t->tile < 0 || t->tile > TILE_WMAX) return fail(s, RUMD_ERR_INVALID_ARG, "tile must be 0..%d cells", TILE_WMAX);
     if (!valid_tp(t->tp)) return fail(s, RUMD_ERR_INVALID_ARG, "tp must be 1,2,4,8,16 or 32");
     if (t->pb < 1 || (t->pb * t->tp) % 32 || t->pb * t->tp > 1024) return fail(s, RUMD_ERR_INVALID_ARG, "pb*tp must be a multiple of 32 and <= 1024");
     if (!(t->skin > 0.f) || !std::isfinite(t->skin)) return fail(s, RUMD_ERR_INVALID_ARG, "skin must be > 0");
@@ -634,6 +645,47 @@ static rumd_status refresh(rumd_system* s)
         s->grid_for[1] = n[1];
         s->grid_for[2] = n[2];
     }
+    // tile method: cut the cell grid into tiles (balanced widths), size the shared-memory halo
+    S.nt[0] = S.nt[1] = S.nt[2] = 1;
+    S.ntiles = 0;
+    S.hcap = 0;
+    S.cap_it8 = 0;
+    if (t.method == RUMD_NB_TILE) {
+        if (s->nrep > 1) return fail(s, RUMD_ERR_INVALID_ARG, "replicas use the n2 or the none method (one block per replica)");
+        if (t.tp > 8) return fail(s, RUMD_ERR_INVALID_ARG, "the tile method takes tp <= 8");
+        const int T = t.tile > 0 ? t.tile : (s->N >= 500000 ? 6 : 4);
+        size_t ntl = 1;
+        double hcells = 1.0;
+        for (int k = 0; k < 3; ++k) {
+            // a tile plus its halo must stay narrower than the box (w + 4 <= n - 1): the periodic image of every
+            // halo particle is then unambiguous, also after a drift of skin/2
+            if (n[k] < 6)
+                return fail(s, RUMD_ERR_BOX_TOO_SMALL, "tile method needs >= 6 cells per axis, have %dx%dx%d", n[0], n[1], n[2]);
+            int ntk = std::max(1, (int)std::lround((double)n[k] / T));
+            auto wmax = [&](int q) { return (n[k] + q - 1) / q; };
+            while (wmax(ntk) > TILE_WMAX || wmax(ntk) + 5 > n[k]) ++ntk;
+            S.nt[k] = ntk;
+            ntl *= (size_t)ntk;
+            hcells *= wmax(ntk) + 4;
+        }
+        if (ntl > tile_bound(s))
+            return fail(s, RUMD_ERR_INVALID_ARG, "tile method: %zu tiles for %d particles (at most N/32 - 1): use a larger tile", ntl, s->N);
+        const double mean = (double)s->N / (double)ncell * hcells;
+        const size_t hcap = align_up((size_t)(1.3 * mean + 6.0 * std::sqrt(mean) + 64.0), 32);
+        if (hcap > 12000) return fail(s, RUMD_ERR_INVALID_ARG, "tile method: a halo of ~%zu particles does not fit shared memory: use a smaller tile", hcap);
+        if (ntl * hcap > halo_slots_bound(s))
+            return fail(s, RUMD_ERR_INVALID_ARG, "tile method: %zu tiles x %zu halo slots exceed the workspace: use a larger tile", ntl, hcap);
+        const int chunk = 8 * t.tp; // entries per list iteration of a particle's tp lanes
+        const int cap_eff = s->cap / chunk * chunk;
+        if (cap_eff < chunk) return fail(s, RUMD_ERR_INVALID_ARG, "list capacity %d below one chunk of the tile method", s->cap);
+        S.ntiles = (int)ntl;
+        S.hcap = (int)hcap;
+        S.cap = cap_eff;
+        S.cap_it = cap_eff / t.tp;
+        S.cap_it8 = cap_eff / chunk;
+        cudaError_t e = cudaFuncSetAttribute(k_build_tile, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tile_smem_bytes(S.hcap));
+        if (e != cudaSuccess) return fail(s, RUMD_ERR_CUDA, "tile method: %zu bytes of shared memory refused: %s", tile_smem_bytes(S.hcap), cudaGetErrorString(e));
+    }
     s->int_blocks = (s->N + INT_THREADS - 1) / INT_THREADS;
     s->persist_grid_for = -1;
     if (s->nrep > 1) {
@@ -695,6 +747,10 @@ static bool one_of(const rumd_system* s) { return s->ntypes == 1; }
 
 static int launch_force(rumd_system* s)
 {
+    if (s->tune.method == RUMD_NB_TILE) { // one block per tile, halo in shared memory
+        kernels_of(s)->force_tile(coul_of(s), one_of(s), s->S, s->S.ntiles, tile_smem_bytes(s->S.hcap), s->stream);
+        return 1;
+    }
     const int tp = s->tune.tp, nthreads = s->tune.pb * tp;
     const int nblocks = (int)(((size_t)s->N * tp + nthreads - 1) / nthreads);
     kernels_of(s)->force(coul_of(s), one_of(s), s->S, nblocks, nthreads, s->stream);
@@ -707,17 +763,21 @@ static int persist_threads_of(const rumd_tuning&) { return PERSIST_THREADS; }
 // co-resident, else to the co-residency limit (the kernel strides).
 static rumd_status launch_persistent(rumd_system* s, int nsteps)
 {
-    const void* fn = kernels_of(s)->persist[coul_of(s)][one_of(s) ? 1 : 0];
+    const bool tile = s->tune.method == RUMD_NB_TILE;
+    const void* fn = (tile ? kernels_of(s)->persist_tile : kernels_of(s)->persist)[coul_of(s)][one_of(s) ? 1 : 0];
+    if (!fn) return fail(s, RUMD_ERR_INVALID_ARG, "the tile method takes tp <= 8");
     const int threads = persist_threads_of(s->tune);
+    const size_t smem = tile ? tile_smem_bytes(s->S.hcap) : 0;
     const int sig = s->tune.tp * 4096 + threads + (s->any_coul ? 1 << 20 : 0) + (s->ntypes == 1 ? 1 << 21 : 0) +
-                    (s->any_generic ? 1 << 22 : 0);
-    if (sig != s->persist_grid_for) {
+                    (s->any_generic ? 1 << 22 : 0) + (tile ? 1 << 23 : 0);
+    if (sig != s->persist_grid_for) { // (refresh() resets persist_grid_for whenever the tiling changes)
+        if (tile) CUDA_TRY(s, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         int per_sm = 0;
-        CUDA_TRY(s, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, threads, 0));
+        CUDA_TRY(s, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, threads, smem));
         if (per_sm < 1) return fail(s, RUMD_ERR_CUDA, "persistent kernel does not fit an SM");
         // whole multiples of the SM count (every SM carries the same number of blocks; the kernel splits the
         // work into equal contiguous chunks per block), as many as the work can fill, at most what is co-resident
-        const long long want = ((long long)s->N * s->tune.tp + threads - 1) / threads;
+        const long long want = tile ? s->S.ntiles : ((long long)s->N * s->tune.tp + threads - 1) / threads;
         long long per = std::min<long long>(per_sm, (want + s->num_sms - 1) / s->num_sms);
         per = std::max<long long>(1, per);
         s->persist_grid = (int)std::min<long long>(per * s->num_sms, 4096);
@@ -727,7 +787,7 @@ static rumd_status launch_persistent(rumd_system* s, int nsteps)
     CUDA_TRY(s, cudaMemsetAsync(s->S.sc->bar, 0, 2 * sizeof(unsigned long long), s->stream));
     int nvt = s->integ == RUMD_INT_NVT_NOSE_HOOVER;
     void* args[] = {(void*)&s->S, (void*)&nsteps, (void*)&nvt};
-    CUDA_TRY(s, cudaLaunchCooperativeKernel(fn, dim3(s->persist_grid), dim3(s->persist_threads), args, 0, s->stream));
+    CUDA_TRY(s, cudaLaunchCooperativeKernel(fn, dim3(s->persist_grid), dim3(s->persist_threads), args, smem, s->stream));
     s->launches += 1;
     return RUMD_OK;
 }
@@ -739,7 +799,7 @@ static int launch_rebuild_chain(rumd_system* s)
     const Sys& S = s->S;
     int n = 0;
     if (s->tune.method == RUMD_NB_NONE) return 0; // no list to rebuild
-    const bool sorting = s->tune.method == RUMD_NB_CELL || s->tune.sort_interval > 0;
+    const bool sorting = s->tune.method == RUMD_NB_CELL || s->tune.method == RUMD_NB_TILE || s->tune.sort_interval > 0;
     // Every phase strides over its items, so the grids are capped at a few blocks per SM: on the (many) steps
     // without a rebuild each kernel only reads the flag and exits, and that costs time per BLOCK.
     const int cap256 = s->num_sms * 8, cap128 = s->num_sms * 16;
@@ -761,7 +821,9 @@ static int launch_rebuild_chain(rumd_system* s)
         k_permute_store<<<nbp, 256, 0, s->stream>>>(S);
         n += 3;
     }
-    if (s->tune.method == RUMD_NB_CELL) {
+    if (s->tune.method == RUMD_NB_TILE)
+        k_build_tile<<<std::min(S.ntiles, cap256), TILE_THREADS, tile_smem_bytes(S.hcap), s->stream>>>(S);
+    else if (s->tune.method == RUMD_NB_CELL) {
         const long long threads = (long long)s->N << S.build_tp_shift;
         k_build_cell<<<(unsigned)std::min<long long>((threads + 127) / 128, cap128), 128, 0, s->stream>>>(S);
     } else
@@ -856,7 +918,7 @@ static rumd_status get_graph(rumd_system* s, GraphCache& gc, int steps, int* ker
     cudaGraph_t g = nullptr;
     CUDA_TRY(s, cudaStreamBeginCapture(s->stream, cudaStreamCaptureModeThreadLocal));
     int n = 0;
-    if (steps % 2 == 0)
+    if (steps % 2 == 0 && s->tune.method != RUMD_NB_TILE) // (the tile method has no fused per-step kernel)
         for (int q = 0; q < steps; q += 2) n += launch_step_pair(s, q + 2 == steps);
     else
         for (int q = 0; q < steps; ++q) n += launch_step(s);
@@ -936,7 +998,10 @@ extern "C" rumd_status rumd_export_nblist(rumd_system* s, void* d_count, void* d
     rumd_status st = ready(s, false);
     if (st != RUMD_OK) return st;
     if (!d_count || !d_list || row_capacity < 1) return fail(s, RUMD_ERR_INVALID_ARG, "bad export arguments");
-    k_export_nbl<<<s->N, 128, 0, s->stream>>>(s->S, (int*)d_count, (int*)d_list, row_capacity);
+    if (s->tune.method == RUMD_NB_TILE)
+        k_export_nbl_tile<<<s->N, 128, 0, s->stream>>>(s->S, (int*)d_count, (int*)d_list, row_capacity);
+    else
+        k_export_nbl<<<s->N, 128, 0, s->stream>>>(s->S, (int*)d_count, (int*)d_list, row_capacity);
     s->launches++;
     CUDA_TRY(s, cudaGetLastError());
     return RUMD_OK;
@@ -978,7 +1043,9 @@ extern "C" rumd_status rumd_get_thermo(rumd_system* s, rumd_thermo* out)
     out->nbl_capacity = s->cap;
     out->overflow = (int)d.overflow;
     out->pad_ = 0;
-    if (d.overflow) return fail(s, RUMD_ERR_NBL_OVERFLOW, "neighbour list overflow: %d neighbours > capacity %d", max_nbrs, s->cap);
+    if (d.overflow == 2u)
+        return fail(s, RUMD_ERR_NBL_OVERFLOW, "tile method: a tile's halo holds more than %d particles (density far from uniform): use a smaller tile or the cell method", s->S.hcap);
+    if (d.overflow) return fail(s, RUMD_ERR_NBL_OVERFLOW, "neighbour list overflow: %d neighbours > capacity %d", max_nbrs, s->S.cap);
     if (d.nonfinite == 2) return fail(s, RUMD_ERR_CUDA, "persistent kernel: grid barrier timed out");
     if (d.nonfinite) return fail(s, RUMD_ERR_NONFINITE, "non-finite energy");
     return RUMD_OK;

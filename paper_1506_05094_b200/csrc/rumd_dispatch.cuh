@@ -10,10 +10,13 @@ template <int TP> struct UnrollOf { static constexpr int value = TP >= 16 ? 4 : 
 
 // coul: 0 no second term, 1 Coulomb only, 2 any second-term kind of P:73;  one: a single particle type
 struct KernelSet {
-    const void* persist[3][2];  // k_persist<TP, coul, one>
+    const void* persist[3][2];  // k_persist<TP, coul, one, unroll, false>
+    const void* persist_tile[3][2]; // k_persist<TP, coul, one, unroll, true> (tile method; null for tp > 8)
     const void* ensemble[3][2]; // k_ensemble<TP, coul, one>
     void (*force)(int coul, bool one, const Sys& S, int nblocks, int nthreads, cudaStream_t stream);
     void (*step)(int coul, bool one, bool energy, int nvt, const Sys& S, int nblocks, int nthreads, cudaStream_t stream);
+    // tile method: pair forces out of shared memory (smem = dynamic shared bytes; returns the CUDA status)
+    cudaError_t (*force_tile)(int coul, bool one, const Sys& S, int nblocks, size_t smem, cudaStream_t stream);
 };
 
 const KernelSet* rumd_kernels_tp1();

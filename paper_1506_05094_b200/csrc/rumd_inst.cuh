@@ -44,17 +44,51 @@ static void step_tp(int coul, bool one, bool energy, int nvt, const Sys& S, int 
     }
 }
 
+template <int TP, int COUL, bool ONE>
+static cudaError_t launch_force_tile_inst(const Sys& S, int nb, size_t smem, cudaStream_t st)
+{
+    auto fn = &k_force_tile<TP, COUL, ONE>;
+    cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    fn<<<nb, TILE_THREADS, smem, st>>>(S);
+    return cudaSuccess;
+}
+
+template <int TP> static cudaError_t force_tile_tp(int coul, bool one, const Sys& S, int nb, size_t smem, cudaStream_t st)
+{
+    if constexpr (TP > 8) return cudaErrorInvalidValue; // the tile method takes tp <= 8 (chunks of 8 entries per lane)
+    else
+    switch (coul * 2 + (one ? 1 : 0)) {
+    case 0: return launch_force_tile_inst<TP, 0, false>(S, nb, smem, st);
+    case 1: return launch_force_tile_inst<TP, 0, true>(S, nb, smem, st);
+    case 2: return launch_force_tile_inst<TP, 1, false>(S, nb, smem, st);
+    case 3: return launch_force_tile_inst<TP, 1, true>(S, nb, smem, st);
+    case 4: return launch_force_tile_inst<TP, 2, false>(S, nb, smem, st);
+    default: return launch_force_tile_inst<TP, 2, true>(S, nb, smem, st);
+    }
+}
+
+template <int TP, int COUL, bool ONE> static const void* persist_tile_fn()
+{
+    if constexpr (TP <= 8) return (const void*)&k_persist<TP, COUL, ONE, UnrollOf<TP>::value, true>;
+    else return nullptr;
+}
+
 template <int TP> static const KernelSet* kernel_set()
 {
     static const KernelSet ks = {
-        {{(const void*)&k_persist<TP, 0, false, UnrollOf<TP>::value>, (const void*)&k_persist<TP, 0, true, UnrollOf<TP>::value>},
-         {(const void*)&k_persist<TP, 1, false, UnrollOf<TP>::value>, (const void*)&k_persist<TP, 1, true, UnrollOf<TP>::value>},
-         {(const void*)&k_persist<TP, 2, false, UnrollOf<TP>::value>, (const void*)&k_persist<TP, 2, true, UnrollOf<TP>::value>}},
+        {{(const void*)&k_persist<TP, 0, false, UnrollOf<TP>::value, false>, (const void*)&k_persist<TP, 0, true, UnrollOf<TP>::value, false>},
+         {(const void*)&k_persist<TP, 1, false, UnrollOf<TP>::value, false>, (const void*)&k_persist<TP, 1, true, UnrollOf<TP>::value, false>},
+         {(const void*)&k_persist<TP, 2, false, UnrollOf<TP>::value, false>, (const void*)&k_persist<TP, 2, true, UnrollOf<TP>::value, false>}},
+        {{persist_tile_fn<TP, 0, false>(), persist_tile_fn<TP, 0, true>()},
+         {persist_tile_fn<TP, 1, false>(), persist_tile_fn<TP, 1, true>()},
+         {persist_tile_fn<TP, 2, false>(), persist_tile_fn<TP, 2, true>()}},
         {{(const void*)&k_ensemble<TP, 0, false, UnrollOf<TP>::value>, (const void*)&k_ensemble<TP, 0, true, UnrollOf<TP>::value>},
          {(const void*)&k_ensemble<TP, 1, false, UnrollOf<TP>::value>, (const void*)&k_ensemble<TP, 1, true, UnrollOf<TP>::value>},
          {(const void*)&k_ensemble<TP, 2, false, UnrollOf<TP>::value>, (const void*)&k_ensemble<TP, 2, true, UnrollOf<TP>::value>}},
         &force_tp<TP>,
         &step_tp<TP>,
+        &force_tile_tp<TP>,
     };
     return &ks;
 }

@@ -55,7 +55,7 @@ __device__ __forceinline__ bool rebuild_requested(const Sys& S) { return S.sc->f
 // sort on this rebuild?  cell method: always; n2 method: every sort_interval-th rebuild.
 __device__ __forceinline__ bool sort_on_rebuild(const Sys& S, long long n_rebuilds)
 {
-    if (S.method == 1) return true;
+    if (S.method == 1 || S.method == 3) return true; // cell and tile methods: at every rebuild
     return S.method == 0 && S.sort_interval > 0 && (n_rebuilds % S.sort_interval) == 0;
 }
 __device__ __forceinline__ bool sort_requested(const Sys& S)

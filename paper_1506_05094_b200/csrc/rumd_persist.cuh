@@ -11,7 +11,7 @@
 // Nose-Hoover variable is advanced redundantly, identically, by every block from per-block fp64 partial sums
 // added in a fixed order, so the run is bitwise reproducible and needs no second barrier.
 #pragma once
-#include "rumd_force.cuh"
+#include "rumd_tile.cuh"
 
 #ifndef PERSIST_THREADS
 #define PERSIST_THREADS 256
@@ -84,7 +84,9 @@ __device__ __forceinline__ double warp_sum_partials(const double* p, int n)
     return warp_sum(a);
 }
 
-template <int TP, int COUL, bool ONE_TYPE, int UNROLL>
+// TILE: the instantiation for the tile method (RUMD_NB_TILE: halo in dynamic shared memory); the other methods share
+// the TILE = false instantiation, whose register budget the tile code must not touch.
+template <int TP, int COUL, bool ONE_TYPE, int UNROLL, bool TILE>
 __global__ void __launch_bounds__(PERSIST_THREADS, PERSIST_MINB) k_persist(const Sys S, const int nsteps, const int nvt)
 {
     __shared__ float4 s_pp[4 * RUMD_MAXT * RUMD_MAXT];
@@ -97,6 +99,10 @@ __global__ void __launch_bounds__(PERSIST_THREADS, PERSIST_MINB) k_persist(const
     __shared__ int s_ab_step; // s_ab holds the leap-frog factors of every step < s_ab_step
     __shared__ double s_nh[4];       // xi, eta, xi_t, eta_t: kept by lane 0 of warp 0 (identical in every block)
     __shared__ long long s_prof[6];  // cycle counters of block 0 / thread 0 (profiling runs only)
+    extern __shared__ __align__(16) unsigned char tile_raw[]; // tile method only: halo positions + halo cell starts
+    float4* s_pos = nullptr;
+    int* s_hstart = nullptr;
+    if (TILE) tile_smem(S, tile_raw, s_pos, s_hstart);
 
     load_pair_table(S, s_pp);
     if (threadIdx.x < RUMD_MAXT * RUMD_MAXT) s_rcl2[threadIdx.x] = S.pp[threadIdx.x].rcl2;
@@ -166,7 +172,10 @@ __global__ void __launch_bounds__(PERSIST_THREADS, PERSIST_MINB) k_persist(const
                 rsrc = S.tmp_r;
             }
             if (prof) s_prof[2] += clock64() - s_prof[4];
-            if (S.method == 1)
+            if (TILE) {
+                for (int t = blockIdx.x; t < S.ntiles; t += gridDim.x)
+                    ph_build_tile(S, rsrc, t, s_pos, s_hstart, s_warp, s_rcl2, max_slot);
+            } else if (S.method == 1)
                 build_cell_dispatch(S, rsrc, s_rcl2, first, stride, max_slot);
             else
                 ph_build_n2(S, rsrc, s_tile, s_rcl2, blockIdx.x, gridDim.x, max_slot);
@@ -204,6 +213,43 @@ __global__ void __launch_bounds__(PERSIST_THREADS, PERSIST_MINB) k_persist(const
         const bool last = k == nsteps - 1;
         double kt = 0.0, mv2 = 0.0;
         bool moved = false;
+        // leap-frog update of one particle from its force: the epilogue of both force paths
+        auto advance = [&](int i, float4 ri, float fx, float fy, float fz, float u, float w, float4 v, int4 im, float4 rb) {
+            while (*((volatile int*)&s_ab_step) <= k) {} // factors of step k published? (warp 0, above)
+            __threadfence_block();
+            const float a = ((volatile float*)s_ab)[0], b = ((volatile float*)s_ab)[1];
+            const float4 f = make_float4(fx, fy, fz, 0.5f * u);
+            bool mv;
+            double kti, mv2i;
+            integrate_particle(S, a, b, ri, v, f, im, rb, mv, kti, mv2i);
+            rn[i] = ri;
+            S.v[i] = v;
+            S.image[i] = im;
+            if (last) { // forces / energies / virials of the LAST force evaluation are the outputs
+                S.f[i] = f;
+                S.w[i] = 0.5f * w;
+            }
+            moved |= mv;
+            kt += kti;
+            mv2 += mv2i;
+        };
+        if constexpr (TILE) {
+            // tile method: the block's tiles in turn -- halo into shared memory, forces of the owned particles out of
+            // it, leap-frog; the tiles are split into gridDim.x contiguous, equally long runs
+            const int t0 = (int)((long long)S.ntiles * blockIdx.x / gridDim.x), t1 = (int)((long long)S.ntiles * (blockIdx.x + 1) / gridDim.x);
+            for (int t = t0; t < t1; ++t) {
+                __syncthreads();
+                tile_load_halo<false>(S, rc, t, s_pos);
+                __syncthreads();
+                auto done = [&](int i, bool lead, const float4& ri, float fx, float fy, float fz, float u, float w) {
+                    if (lead) advance(i, ri, fx, fy, fz, u, w, S.v[i], S.image[i], S.r_build[i]);
+                };
+                if (last)
+                    tile_force_own<TP, COUL, ONE_TYPE, false, true>(S, rc, t, s_pos, s_pp, done);
+                else
+                    tile_force_own<TP, COUL, ONE_TYPE, false, false>(S, rc, t, s_pos, s_pp, done);
+            }
+        } else
         // the N*TP/32 warps of work are split into gridDim.x contiguous, equally long chunks (spatial locality
         // inside a block, every SM equally loaded); the block's warps take the warps of its chunk in turn
         for (long long vw = vw0 + wid; vw < vw1; vw += nw) {
@@ -233,28 +279,12 @@ __global__ void __launch_bounds__(PERSIST_THREADS, PERSIST_MINB) k_persist(const
             else
                 force_any<TP, COUL, ONE_TYPE, UNROLL, false, false>(S, rc, s_pp, (int)vw, i, t, have_i, ri, cnt, fx, fy, fz, u, w);
             if (have_i && t == 0) {
-                while (*((volatile int*)&s_ab_step) <= k) {} // factors of step k published? (warp 0, above)
-                __threadfence_block();
-                const float a = ((volatile float*)s_ab)[0], b = ((volatile float*)s_ab)[1];
-                const float4 f = make_float4(fx, fy, fz, 0.5f * u);
                 if (!EARLY) {
                     v = S.v[i];
                     im = S.image[i];
                     rb = S.r_build[i];
                 }
-                bool mv;
-                double kti, mv2i;
-                integrate_particle(S, a, b, ri, v, f, im, rb, mv, kti, mv2i);
-                rn[i] = ri;
-                S.v[i] = v;
-                S.image[i] = im;
-                if (last) { // forces / energies / virials of the LAST force evaluation are the outputs
-                    S.f[i] = f;
-                    S.w[i] = 0.5f * w;
-                }
-                moved |= mv;
-                kt += kti;
-                mv2 += mv2i;
+                advance(i, ri, fx, fy, fz, u, w, v, im, rb);
             }
         }
         PROF_LAP(1)

@@ -22,7 +22,7 @@ POT_GEN_LJ, POT_GIRIFALCO, POT_DZUGUTOV = 6, 7, 8
 _SECOND_NPARAMS = (1, 2, 2, 2, 3, 4, 3, 2)  # of (a, b, c, d), by kind - 1; rcut follows
 CUT_SHIFTED_FORCE, CUT_SHIFTED_POTENTIAL, CUT_NONE = 0, 1, 2
 INT_NVE_LEAPFROG, INT_NVT_NOSE_HOOVER = 0, 1
-NB_N2, NB_CELL, NB_NONE = 0, 1, 2
+NB_N2, NB_CELL, NB_NONE, NB_TILE = 0, 1, 2, 3
 
 EXPORTS = [
     "rumd_create", "rumd_destroy", "rumd_bind_state", "rumd_workspace_bytes", "rumd_bind_workspace",
@@ -36,7 +36,7 @@ EXPORTS = [
 class Tuning(C.Structure):
     _fields_ = [("method", C.c_int), ("pb", C.c_int), ("tp", C.c_int), ("skin", C.c_float),
                 ("sort_interval", C.c_int), ("use_graph", C.c_int), ("steps_per_graph", C.c_int),
-                ("persistent", C.c_int), ("build_tp", C.c_int)]
+                ("persistent", C.c_int), ("build_tp", C.c_int), ("tile", C.c_int)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}

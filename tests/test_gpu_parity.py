@@ -148,7 +148,16 @@ CASES = [
     ("ka", dict(N=2048), "n2", 1),            # orthorhombic box 16x16x8
     ("ch", dict(n=12), "cell", 8),            # charged, N = 1728, rc 4.0 + LJ 2.5
     ("ch", dict(n=10), "n2", 4),
+    # tile method (j-particles staged in shared memory, 16-bit slot lists)
+    ("lj", dict(ncell=10), "tile", 1),        # 12 cells per axis -> 3x3x3 tiles, every tile touches a face
+    ("lj", dict(ncell=16), "tile", 2),        # N = 16384, 19 cells per axis: interior and boundary tiles
+    ("ka", dict(N=8000), "tile", 8),          # configs[1]
+    ("ka", dict(N=4096), "tile", 4),
+    ("ka", dict(N=16384), "tile", 1),         # orthorhombic 32x32x16 lattice
+    ("ch", dict(n=16), "tile", 2),            # charged, rc 4.0: 9 cells per axis
 ]
+
+METHODS = {"n2": 0, "cell": 1, "none": 2, "tile": 3}
 
 
 def test_one_lane_build_wide_box_matches_oracle(rumd):
@@ -357,7 +366,7 @@ def test_c3_nve_energy_drift(rumd):
 def test_nblist_and_forces_match_oracle(rumd, kind, kw, method, tp):
     wl = perturbed(make(kind, **kw))
     s = rumd.from_workload(wl)
-    s.set_tuning(method=rumd.NB_CELL if method == "cell" else rumd.NB_N2, tp=tp, pb=max(32 // tp, 128 // tp))
+    s.set_tuning(method=METHODS[method], tp=tp, pb=max(32 // tp, 128 // tp))
     s.compute_forces()
     r64 = wl.r.astype(np.float64)
     box = wl.box.astype(np.float64)
@@ -1118,3 +1127,150 @@ def test_max_nbrs_survives_a_pending_rebuild_flag(rumd):
             seen = max(seen, th["n_rebuilds"])
         assert seen >= 3                           # several runs ended with the flag raised
         s.close()
+
+
+# ------------------------------------------------------------------ tile method (shared-memory j staging)
+
+
+def fold(r, box):
+    """Positions folded into [-L/2, L/2): the tile method wraps coordinates only at list rebuilds (between them
+    they may leave the box by up to skin/2; r + image L is the unwrapped position at all times)."""
+    r = np.asarray(r, np.float64)
+    return r - box * np.rint(r / box)
+
+
+@pytest.mark.parametrize("kind,kw,tp,tile,nsteps", [
+    ("lj", dict(ncell=10), 1, 0, 75),
+    ("ka", dict(N=8000), 8, 3, 60),
+    ("ka", dict(N=16384), 2, 4, 41),          # odd: positions end in the alternate buffer
+    ("ch", dict(n=16), 4, 0, 40),
+])
+def test_tile_method_persistent_equals_per_step_bitwise_and_tracks_the_cell_method(rumd, kind, kw, tp, tile, nsteps):
+    """RUMD_NB_TILE: the persistent kernel and the per-step kernels (k_build_tile, k_force_tile, k_integrate) run
+    the same arithmetic in the same order -> NVE bit-identical across rebuilds, sorts and lazily wrapped
+    coordinates; and the trajectory stays with the cell method's (same displacements, other summation order)."""
+    wl = perturbed(make(kind, **kw))
+    wl.integrator = W.NVE
+    box = wl.box.astype(np.float64)
+    res = []
+    for method, persistent in ((rumd.NB_TILE, 1), (rumd.NB_TILE, 0), (rumd.NB_CELL, 1)):
+        s = rumd.from_workload(wl)
+        s.set_tuning(method=method, tp=tp, pb=256 // tp, tile=tile, persistent=persistent, use_graph=0, skin=0.25)
+        s.run_steps(nsteps)
+        s.run_steps(7)
+        th = s.get_thermo()
+        st = s.state()
+        assert th["n_steps"] == nsteps + 7 and th["n_rebuilds"] >= 3 and th["overflow"] == 0
+        res.append((st, th))
+        s.close()
+    (a, ta), (b, tb), (c, tc) = res
+    assert ta["n_rebuilds"] == tb["n_rebuilds"]
+    for key in ("r", "v", "F", "u", "w", "image"):
+        assert np.array_equal(a[key], b[key]), key
+    assert ta["U"] == tb["U"] and ta["max_nbrs"] == tb["max_nbrs"]
+    d = (a["r"].astype(np.float64) + a["image"] * box) - (c["r"].astype(np.float64) + c["image"] * box)
+    assert np.abs(d).max() < 2e-4
+    assert ta["U"] == pytest.approx(tc["U"], rel=1e-4)
+
+
+def test_tile_method_lockstep_with_particles_crossing_the_faces(rumd):
+    """Protocol (3) for the tile method over several rebuilds: at every stop the list in use (halo slots mapped back
+    to particles) contains every interacting pair, forces match the oracle, coordinates that left the box are within
+    skin/2 of it and r + image L is continuous; some particles do cross faces during the run."""
+    wl = perturbed(make("lj", ncell=10))
+    wl.integrator = W.NVE
+    s = rumd.from_workload(wl)
+    s.set_tuning(method=rumd.NB_TILE, tp=2, pb=128, skin=0.3)
+    box = wl.box.astype(np.float64)
+    crossed = 0
+    for _ in range(6):
+        s.run_steps(53)
+        s.compute_forces()
+        st = s.state()
+        out = np.abs(st["r"].astype(np.float64)) - 0.5 * box
+        assert out.max() <= 0.5 * 0.3 + 1e-5
+        crossed += int((np.abs(st["image"]).sum(1) > 0).sum())
+        r64 = fold(st["r"], box)
+        cnt, lst = s.export_nblist()
+        ids = s.d_id.cpu().numpy().astype(np.int64)
+        have = np.unique(pair_keys(cnt, lst, ids))
+        assert have.size == cnt.sum()
+        oc, ol = oracle.nblist(r64, wl.types, box, wl.pot, 0.0)
+        assert np.isin(pair_keys(oc, ol), have).all(), "list in use misses interacting pairs"
+        check_forces(s, r64, wl.types, box, wl.pot)
+    assert crossed > 0 and s.get_thermo()["n_rebuilds"] >= 8
+    s.close()
+
+
+def test_tile_method_full_size_million_particles_whole_system(rumd):
+    """configs[3] with the tile method at its default tile size: the whole list (every row, as sets, 1e-6 band), every
+    force, U and W against the oracle; then one whole step and a short run (rebuilds with the sort in flight)."""
+    wl = perturbed(make("lj", ncell=64))
+    s = rumd.from_workload(wl)
+    s.set_tuning(method=rumd.NB_TILE, tp=1, pb=256)
+    s.compute_forces()
+    r64 = wl.r.astype(np.float64)
+    box = wl.box.astype(np.float64)
+    gcnt, npairs, nband = check_nblist_rows(s, r64, wl.types, box, wl.pot, float(wl.skin))
+    assert npairs > 7e7
+    check_forces(s, r64, wl.types, box, wl.pot)
+    th = s.get_thermo()
+    assert th["overflow"] == 0 and th["max_nbrs"] == gcnt.max()
+    s.run_steps(50)
+    s.compute_forces()
+    st = s.state()
+    assert s.get_thermo()["n_rebuilds"] >= 3
+    check_forces(s, fold(st["r"], box), wl.types, box, wl.pot)
+    s.close()
+
+
+@pytest.mark.parametrize("kind,kw,tuning", [
+    ("ka", dict(N=8000), dict(method=3, tp=8, pb=32, tile=3, skin=0.35)),
+    ("ch", dict(n=32), dict(method=3, tp=2, pb=128)),
+    ("ka", dict(N=65536), dict(method=3, tp=1, pb=256, tile=4)),
+])
+def test_tile_method_one_step_matches_oracle(rumd, kind, kw, tuning):
+    """One whole step (build -> forces -> integrate) of the tile method from identical inputs: U, K, xi, positions and
+    velocities against the oracle, then U, W, forces of the new configuration."""
+    wl = make(kind, **kw)
+    wl = perturbed(wl) if kind != "ka" else wl
+    s0 = rumd.from_workload(wl)
+    s0.set_tuning(**tuning)
+    s0.run_steps(300)
+    st0 = s0.state()
+    s0.close()
+    box = wl.box.astype(np.float64)
+    wl.r = fold(st0["r"], box).astype(np.float32)
+    wl.r = np.where(wl.r >= 0.5 * wl.box, wl.r - wl.box, wl.r).astype(np.float32)
+    wl.v = st0["v"].copy()
+    s = rumd.from_workload(wl)
+    s.set_tuning(**tuning)
+    N = wl.N
+    skin = float(s.get_tuning().skin)
+    o = oracle.run(wl.r.astype(np.float64), wl.v.astype(np.float64), wl.m.astype(np.float64), np.zeros((N, 3), np.int32),
+                   wl.types, box, wl.pot, skin, float(wl.dt), 1, mode=wl.integrator, T0=wl.T0, tau=wl.tau, use_cell=N >= 4096)
+    s.run_steps(1)
+    th1 = s.get_thermo()
+    st = s.state()
+    d = st["r"].astype(np.float64) + st["image"] * box - (o["r"] + o["image"] * box)
+    assert np.abs(d).max() < max(2e-6, 6e-8 * box.max())
+    assert np.abs(st["v"] - o["v"]).max() < 1e-5 * max(1.0, np.abs(o["v"]).max())
+    assert th1["U"] == pytest.approx(o["log"][0, 0], rel=ENERGY_TOL)
+    assert th1["K"] == pytest.approx(o["log"][0, 1], rel=ENERGY_TOL)
+    if wl.integrator == W.NVT:
+        assert th1["xi"] == pytest.approx(o["xi"], rel=1e-4, abs=1e-7)
+    s.compute_forces()
+    check_forces(s, fold(s.state()["r"], box), wl.types, box, wl.pot)
+    s.close()
+
+
+def test_tile_method_refuses_what_it_cannot_do(rumd):
+    wl = make("lj", ncell=6)                       # 7 cells per axis: fine (6 is the minimum)
+    s = rumd.from_workload(wl)
+    with pytest.raises(rumd.RumdError):
+        s.set_tuning(method=rumd.NB_TILE, tp=16, pb=16)
+    s.set_tuning(method=rumd.NB_TILE, tp=8, pb=32, skin=1.0)   # rc + skin = 3.5 -> 5 cells per axis
+    with pytest.raises(rumd.RumdError) as e:
+        s.compute_forces()
+    assert e.value.status == rumd.ERR_BOX_TOO_SMALL
+    s.close()
