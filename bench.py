@@ -365,7 +365,7 @@ def sweep_row(name, N, tps, ms_per_timestep, tun, rl, rebuilds, tsteps, info):
     fk, ws = rl["force_kernel"], rl["whole_step"]
     return {"workload": name, "N": N, "timesteps_per_s": tps, "particle_steps_per_s": tps * N,
             "us_per_timestep": 1e3 * ms_per_timestep,
-            "tuning": {k: tun[k] for k in ("method", "tp", "skin", "build_tp", "persistent")},
+            "tuning": {k: tun[k] for k in ("method", "tp", "skin", "build_tp", "persistent", "tile")},
             "tuning_from_cache": info.get("tuning_from_cache"),
             "rebuild_interval": tsteps / max(1, rebuilds), "mean_nbrs": rl["mean_nbrs"],
             "k_force_us": fk["us_per_launch"], "k_force_frac_fp32": fk["frac"],

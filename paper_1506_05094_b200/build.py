@@ -17,8 +17,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJDIR = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "librumd_b200.so")
 SOURCES = ["rumd_b200.cu"] + ["rumd_inst_tp%d.cu" % tp for tp in (1, 2, 4, 8, 16, 32)]
-HEADERS = ["rumd_types.cuh", "rumd_kernels.cuh", "rumd_force.cuh", "rumd_persist.cuh", "rumd_ensemble.cuh",
-           "rumd_dispatch.cuh", "rumd_inst.cuh", "../../include/rumd_b200.h"]
+HEADERS = sorted(f for f in os.listdir(CSRC) if f.endswith(".cuh")) + ["../../include/rumd_b200.h"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC"]
 
 

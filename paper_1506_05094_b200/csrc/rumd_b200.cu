@@ -61,6 +61,7 @@ struct rumd_system {
     long long launches = 0;
     int int_blocks = 0;
     int num_sms = 148;
+    int force_grid_for = -1, force_per_sm = 1; // co-resident blocks per SM of the stand-alone force kernel
     int persist_grid_for = -1; // tuning signature the cached persistent grid belongs to
     int persist_grid = 0, persist_threads = 0;
     long long* prof_buf = nullptr;
@@ -671,12 +672,16 @@ static rumd_status refresh(rumd_system* s)
         if (ntl > tile_bound(s))
             return fail(s, RUMD_ERR_INVALID_ARG, "tile method: %zu tiles for %d particles (at most N/32 - 1): use a larger tile", ntl, s->N);
         const double mean = (double)s->N / (double)ncell * hcells;
-        const size_t hcap = align_up((size_t)(1.3 * mean + 6.0 * std::sqrt(mean) + 64.0), 32);
-        if (hcap > 12000) return fail(s, RUMD_ERR_INVALID_ARG, "tile method: a halo of ~%zu particles does not fit shared memory: use a smaller tile", hcap);
+        // 16-bit list entries hold the slot's byte offset in the shared-memory halo: 16 * slot <= 65535
+        // (margin: 15 % + 4 Poisson sigmas; a liquid's density fluctuations on the scale of a halo are far smaller.  A
+        // halo that does overflow raises the sticky overflow error of rumd_get_thermo.)
+        const size_t hcap = std::min<size_t>(align_up((size_t)(1.15 * mean + 4.0 * std::sqrt(mean) + 32.0), 32), 4095);
+        if ((double)hcap < 1.08 * mean + 3.0 * std::sqrt(mean))
+            return fail(s, RUMD_ERR_INVALID_ARG, "tile method: a halo of ~%.0f particles does not fit 4095 slots: use a smaller tile", mean);
         if (ntl * hcap > halo_slots_bound(s))
             return fail(s, RUMD_ERR_INVALID_ARG, "tile method: %zu tiles x %zu halo slots exceed the workspace: use a larger tile", ntl, hcap);
         const int chunk = 8 * t.tp; // entries per list iteration of a particle's tp lanes
-        const int cap_eff = s->cap / chunk * chunk;
+        const int cap_eff = std::min(s->cap, TILE_ROW_MAX) / chunk * chunk; // (rows are staged in shared memory by the build)
         if (cap_eff < chunk) return fail(s, RUMD_ERR_INVALID_ARG, "list capacity %d below one chunk of the tile method", s->cap);
         S.ntiles = (int)ntl;
         S.hcap = (int)hcap;
@@ -748,12 +753,14 @@ static bool one_of(const rumd_system* s) { return s->ntypes == 1; }
 static int launch_force(rumd_system* s)
 {
     if (s->tune.method == RUMD_NB_TILE) { // one block per tile, halo in shared memory
-        kernels_of(s)->force_tile(coul_of(s), one_of(s), s->S, s->S.ntiles, tile_smem_bytes(s->S.hcap), s->stream);
+        kernels_of(s)->force_tile(coul_of(s), one_of(s), s->S, s->S.ntiles, tile_smem_bytes_force(s->S.hcap), s->stream);
         return 1;
     }
     const int tp = s->tune.tp, nthreads = s->tune.pb * tp;
-    const int nblocks = (int)(((size_t)s->N * tp + nthreads - 1) / nthreads);
-    kernels_of(s)->force(coul_of(s), one_of(s), s->S, nblocks, nthreads, s->stream);
+    // one virtual warp per warp of the grid: the block scheduler balances better than equal static runs (measured:
+    // 156 vs 168 us at N = 10^6)
+    const long long nblocks = ((long long)s->N * tp + nthreads - 1) / nthreads;
+    kernels_of(s)->force(coul_of(s), one_of(s), s->S, (int)nblocks, nthreads, s->stream);
     return 1;
 }
 
@@ -1392,10 +1399,15 @@ extern "C" rumd_status rumd_autotune(rumd_system* s, rumd_tuning* out, int steps
     if (s->N <= 5000) methods.push_back(RUMD_NB_NONE); // "none" is not tried above 5000 particles
     if (s->N <= 20000) methods.push_back(RUMD_NB_N2); // n2 is not tried for large systems
     methods.push_back(RUMD_NB_CELL);
+    if (s->N >= 4096) methods.push_back(RUMD_NB_TILE); // shared-memory staging needs tiles of >= 32 particles
     for (int method : methods) {
         rumd_tuning start;
         rumd_default_tuning(s, &start);
         start.method = method;
+        if (method == RUMD_NB_TILE && start.tp > 8) {
+            start.tp = 8;
+            start.pb = 32;
+        }
         start.skin = std::min(saved.skin, skin_max);
         if (!(start.skin > 0.f)) continue;
         Tuner T{s, steps_per_trial, start};
@@ -1404,7 +1416,7 @@ extern "C" rumd_status rumd_autotune(rumd_system* s, rumd_tuning* out, int steps
             const double before = T.cur_tps;
             T.descend([](rumd_tuning& c, int dir) { // threads per particle
                 const int tp = dir < 0 ? c.tp / 2 : c.tp * 2;
-                if (tp < 1 || tp > 32) return false;
+                if (tp < 1 || tp > (c.method == RUMD_NB_TILE ? 8 : 32)) return false;
                 const int threads = std::max(32, c.pb * c.tp);
                 c.tp = tp;
                 c.pb = std::max(1, threads / tp);
@@ -1424,6 +1436,14 @@ extern "C" rumd_status rumd_autotune(rumd_system* s, rumd_tuning* out, int steps
                     c.build_tp = b;
                     return true;
                 });
+            if (method == RUMD_NB_TILE)
+                T.descend([&](rumd_tuning& c, int dir) { // tile edge in cells: halo overhead against blocks per SM
+                    const int cur_t = c.tile > 0 ? c.tile : (s->N >= 500000 ? 6 : 4);
+                    const int tl = cur_t + dir;
+                    if (tl < 2 || tl > TILE_WMAX) return false;
+                    c.tile = tl;
+                    return true;
+                });
             if (T.cur_tps < 1.02 * before) break;
         }
         if (method == RUMD_NB_N2 && s->N >= 1024) { // P:379 step 5: with n2, how often to re-sort the particles
@@ -1433,7 +1453,7 @@ extern "C" rumd_status rumd_autotune(rumd_system* s, rumd_tuning* out, int steps
                 T.try_setting(c);
             }
         }
-        {   // per-step kernels in CUDA graphs instead of the persistent kernel; there the block size matters
+        if (method != RUMD_NB_TILE) { // per-step kernels in CUDA graphs instead of the persistent kernel; there the block size matters
             rumd_tuning c = T.cur;
             c.persistent = 0;
             c.use_graph = 1;
@@ -1500,9 +1520,9 @@ static bool cache_lookup(const char* path, const std::string& key, rumd_tuning* 
         double v = 0;
         if (sscanf(line.data() + want.size(),
                    "\"method\": %d, \"pb\": %d, \"tp\": %d, \"skin\": %f, \"sort_interval\": %d, \"use_graph\": %d, "
-                   "\"steps_per_graph\": %d, \"persistent\": %d, \"build_tp\": %d, \"timesteps_per_s\": %lf",
+                   "\"steps_per_graph\": %d, \"persistent\": %d, \"build_tp\": %d, \"tile\": %d, \"timesteps_per_s\": %lf",
                    &c.method, &c.pb, &c.tp, &c.skin, &c.sort_interval, &c.use_graph, &c.steps_per_graph, &c.persistent,
-                   &c.build_tp, &v) == 10) {
+                   &c.build_tp, &c.tile, &v) == 11) {
             *t = c; // the LAST matching line wins (a re-tune appends)
             *tps = v;
             found = true;
@@ -1539,9 +1559,9 @@ extern "C" rumd_status rumd_autotune_cached(rumd_system* s, rumd_tuning* out, in
     if (!f) return fail(s, RUMD_ERR_INVALID_ARG, "cannot write the tuning cache %s", cache_path);
     fprintf(f,
             "{\"key\": \"%s\", \"method\": %d, \"pb\": %d, \"tp\": %d, \"skin\": %.9g, \"sort_interval\": %d, \"use_graph\": %d, "
-            "\"steps_per_graph\": %d, \"persistent\": %d, \"build_tp\": %d, \"timesteps_per_s\": %.6g}\n",
+            "\"steps_per_graph\": %d, \"persistent\": %d, \"build_tp\": %d, \"tile\": %d, \"timesteps_per_s\": %.6g}\n",
             key.c_str(), t.method, t.pb, t.tp, (double)t.skin, t.sort_interval, t.use_graph, t.steps_per_graph, t.persistent,
-            t.build_tp, tps);
+            t.build_tp, t.tile, tps);
     fclose(f);
     return RUMD_OK;
 }

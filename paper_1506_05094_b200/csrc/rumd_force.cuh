@@ -23,13 +23,21 @@ __device__ __forceinline__ float __frcp_approx(float x)
     return y;
 }
 
+// MUFU.RSQ alone: rsqrtf() wraps it in four instructions of denormal handling, and r^2 is never denormal here
+__device__ __forceinline__ float __frsqrt_approx(float x)
+{
+    float y;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
 template <int COUL, bool ENERGY>
 __device__ __forceinline__ void pair_accumulate(const float4 pf, const float4 pc, const float4 pe, const float4 px, bool ok,
                                                 float dx, float dy, float dz, float& fx, float& fy, float& fz,
                                                 float& u, float& w)
 {
     const float r2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, dx * dx));
-    const float y = rsqrtf(r2);
+    const float y = __frsqrt_approx(r2);
     const float rinv2 = __frcp_approx(r2);
     const float rinv6 = rinv2 * rinv2 * rinv2;
     const float r = r2 * y;
@@ -304,6 +312,9 @@ __device__ __forceinline__ void finish_rebuild(const Sys& S)
     }
 }
 
+// The grid is sized to what is co-resident (a whole number of blocks per SM) and the N*TP/32 warps of work are cut
+// into gridDim.x contiguous, equally long runs: no partial last wave (at N = 65536 the one-thread-per-lane grid was
+// 1.7 waves), neighbouring particles stay on one SM.
 template <int TP, int COUL, bool ONE_TYPE, int UNROLL>
 __global__ void __launch_bounds__(1024, 1) k_force(const Sys S)
 {
@@ -311,21 +322,26 @@ __global__ void __launch_bounds__(1024, 1) k_force(const Sys S)
     load_pair_table(S, s_pp);
     __syncthreads();
     if (blockIdx.x == 0 && threadIdx.x == 0) finish_rebuild(S);
-    const int tid = blockIdx.x * blockDim.x + threadIdx.x;
-    const int i = tid / TP;
-    const int t = tid % TP;
-    const bool have_i = i < S.N;
-    float4 ri = make_float4(0.f, 0.f, 0.f, 0.f);
-    int cnt = 0;
-    if (have_i) {
-        ri = __ldg(&S.r[i]);
-        cnt = S.method == 2 ? 0 : S.num_nbrs[i];
-    }
-    float fx, fy, fz, u, w;
-    force_any<TP, COUL, ONE_TYPE, UNROLL, true, true>(S, S.r, s_pp, tid >> 5, i, t, have_i, ri, cnt, fx, fy, fz, u, w);
-    if (have_i && t == 0) {
-        S.f[i] = make_float4(fx, fy, fz, 0.5f * u); // P:160 "compensate for double counting"
-        S.w[i] = 0.5f * w;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    const long long nvwarps = ((long long)S.N * TP + 31) / 32;
+    const long long vw0 = nvwarps * blockIdx.x / gridDim.x, vw1 = nvwarps * (blockIdx.x + 1) / gridDim.x;
+    for (long long vw = vw0 + wid; vw < vw1; vw += nw) {
+        const long long tid = vw * 32 + lane;
+        const int i = (int)(tid / TP);
+        const int t = (int)(tid % TP);
+        const bool have_i = i < S.N;
+        float4 ri = make_float4(0.f, 0.f, 0.f, 0.f);
+        int cnt = 0;
+        if (have_i) {
+            ri = __ldg(&S.r[i]);
+            cnt = S.method == 2 ? 0 : S.num_nbrs[i];
+        }
+        float fx, fy, fz, u, w;
+        force_any<TP, COUL, ONE_TYPE, UNROLL, true, true>(S, S.r, s_pp, (int)vw, i, t, have_i, ri, cnt, fx, fy, fz, u, w);
+        if (have_i && t == 0) {
+            S.f[i] = make_float4(fx, fy, fz, 0.5f * u); // P:160 "compensate for double counting"
+            S.w[i] = 0.5f * w;
+        }
     }
 }
 

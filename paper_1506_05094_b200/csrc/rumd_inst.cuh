@@ -86,6 +86,9 @@ template <int TP> static const KernelSet* kernel_set()
         {{(const void*)&k_ensemble<TP, 0, false, UnrollOf<TP>::value>, (const void*)&k_ensemble<TP, 0, true, UnrollOf<TP>::value>},
          {(const void*)&k_ensemble<TP, 1, false, UnrollOf<TP>::value>, (const void*)&k_ensemble<TP, 1, true, UnrollOf<TP>::value>},
          {(const void*)&k_ensemble<TP, 2, false, UnrollOf<TP>::value>, (const void*)&k_ensemble<TP, 2, true, UnrollOf<TP>::value>}},
+        {{(const void*)&k_force<TP, 0, false, UnrollOf<TP>::value>, (const void*)&k_force<TP, 0, true, UnrollOf<TP>::value>},
+         {(const void*)&k_force<TP, 1, false, UnrollOf<TP>::value>, (const void*)&k_force<TP, 1, true, UnrollOf<TP>::value>},
+         {(const void*)&k_force<TP, 2, false, UnrollOf<TP>::value>, (const void*)&k_force<TP, 2, true, UnrollOf<TP>::value>}},
         &force_tp<TP>,
         &step_tp<TP>,
         &force_tile_tp<TP>,

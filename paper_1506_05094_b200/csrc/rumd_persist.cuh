@@ -101,8 +101,9 @@ __global__ void __launch_bounds__(PERSIST_THREADS, PERSIST_MINB) k_persist(const
     __shared__ long long s_prof[6];  // cycle counters of block 0 / thread 0 (profiling runs only)
     extern __shared__ __align__(16) unsigned char tile_raw[]; // tile method only: halo positions + halo cell starts
     float4* s_pos = nullptr;
-    int* s_hstart = nullptr;
-    if (TILE) tile_smem(S, tile_raw, s_pos, s_hstart);
+    unsigned short* s_hstart = nullptr;
+    unsigned char* s_scratch = nullptr;
+    if (TILE) tile_smem(S, tile_raw, s_pos, s_hstart, s_scratch);
 
     load_pair_table(S, s_pp);
     if (threadIdx.x < RUMD_MAXT * RUMD_MAXT) s_rcl2[threadIdx.x] = S.pp[threadIdx.x].rcl2;
@@ -174,7 +175,7 @@ __global__ void __launch_bounds__(PERSIST_THREADS, PERSIST_MINB) k_persist(const
             if (prof) s_prof[2] += clock64() - s_prof[4];
             if (TILE) {
                 for (int t = blockIdx.x; t < S.ntiles; t += gridDim.x)
-                    ph_build_tile(S, rsrc, t, s_pos, s_hstart, s_warp, s_rcl2, max_slot);
+                    ph_build_tile(S, rsrc, t, s_pos, s_hstart, s_scratch, s_warp, s_rcl2, max_slot);
             } else if (S.method == 1)
                 build_cell_dispatch(S, rsrc, s_rcl2, first, stride, max_slot);
             else

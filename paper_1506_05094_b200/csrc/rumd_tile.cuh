@@ -31,8 +31,13 @@
 #define TILE_IDX_MASK 0x0fffffff
 #define TILE_FAR 1.0e15f // coordinate of the dummy slot: r^2 = 3e30 is finite and beyond every cutoff
 
-// shared memory of a tile kernel: halo positions (hcap + 1 float4), then the halo cell starts of the build
-__host__ __device__ __forceinline__ size_t tile_smem_bytes(int hcap) { return (size_t)(hcap + 1) * 16 + (TILE_HC_MAX + 1) * 4; }
+// shared memory of a tile kernel: halo positions (hcap + 1 float4); kernels that build also hold the halo cell starts
+// (16-bit) and, per warp of a 256-thread block, a candidate buffer and a row buffer (TILE_WARP_SCRATCH)
+__host__ __device__ __forceinline__ size_t tile_smem_bytes_force(int hcap) { return (size_t)(hcap + 1) * 16; }
+__host__ __device__ __forceinline__ size_t tile_smem_bytes(int hcap)
+{
+    return tile_smem_bytes_force(hcap) + (TILE_THREADS / 32) * ((512 + 384) * 2) + ((TILE_HC_MAX + 1) * 2 + 15) / 16 * 16;
+}
 
 // half shift toward the origin: x - sign(x) L/2, exact for |x| >= L/4 (Sterbenz), which every particle that can be
 // paired across a face satisfies when L/2 >= 2 (rc + skin); in smaller boxes ulp(L/2) < 5e-7 bounds the error
@@ -65,7 +70,7 @@ __device__ __forceinline__ unsigned tile_wrap_axes(const Sys& S, const TileGeo& 
 // Fills s_hstart[0 .. nhc] (first slot of every halo cell), halo_idx / halo_cnt in global memory and the slot
 // values in shared memory.  Block-cooperative, blockDim.x >= SCAN_THREADS.
 __device__ __forceinline__ void tile_layout_halo(const Sys& S, const float4* r, int t, const TileGeo& g, float4* s_pos,
-                                                 int* s_hstart, int* s_warp)
+                                                 unsigned short* s_hstart, int* s_warp)
 {
     const int nx = S.grid.n[0], ny = S.grid.n[1], nz = S.grid.n[2];
     const int hx = g.wx + 4, hy = g.wy + 4, nhc = hx * hy * (g.wz + 4);
@@ -96,7 +101,7 @@ __device__ __forceinline__ void tile_layout_halo(const Sys& S, const float4* r, 
         if (threadIdx.x < SCAN_THREADS) {
 #pragma unroll
             for (int q = 0; q < SCAN_ITEMS; ++q) {
-                if (base + q <= nhc) s_hstart[base + q] = e; // (entry nhc = total)
+                if (base + q <= nhc) s_hstart[base + q] = (unsigned short)min(e, S.hcap); // (entry nhc = total)
                 e += c[q];
             }
         }
@@ -131,9 +136,22 @@ __device__ __forceinline__ void tile_load_halo(const Sys& S, const float4* r, in
 {
     const int nh = S.halo_cnt[t];
     const int* hidx = S.halo_idx + (size_t)t * S.hcap;
-    for (int slot = threadIdx.x; slot < nh; slot += blockDim.x) {
-        const int gi = NC ? __ldg(hidx + slot) : hidx[slot];
-        s_pos[slot] = tile_slot_value(S, load_pos<NC>(r + (gi & TILE_IDX_MASK)), (unsigned)gi >> TILE_GHOST_SHIFT);
+    constexpr int U = 4; // slots per thread in flight: index loads first, then the position loads they address
+    for (int s0 = threadIdx.x; s0 < nh; s0 += U * blockDim.x) {
+        int gi[U];
+        float4 p[U];
+#pragma unroll
+        for (int q = 0; q < U; ++q) {
+            const int slot = s0 + q * blockDim.x;
+            gi[q] = slot < nh ? (NC ? __ldg(hidx + slot) : hidx[slot]) : 0;
+        }
+#pragma unroll
+        for (int q = 0; q < U; ++q) p[q] = load_pos<NC>(r + (gi[q] & TILE_IDX_MASK));
+#pragma unroll
+        for (int q = 0; q < U; ++q) {
+            const int slot = s0 + q * blockDim.x;
+            if (slot < nh) s_pos[slot] = tile_slot_value(S, p[q], (unsigned)gi[q] >> TILE_GHOST_SHIFT);
+        }
     }
     if (threadIdx.x == 0) s_pos[S.hcap] = make_float4(TILE_FAR, TILE_FAR, TILE_FAR, 0.f);
 }
@@ -150,87 +168,135 @@ __device__ __forceinline__ size_t tile_entry_index(const Sys& S, int v, int k)
 }
 
 // ------------------------------------------------------------------------------------------ A4 from shared memory
-// P:226-268 Fig. 5 on the staged halo: one lane per owned particle; the 5 x-cells of each of its 25 stencil
-// rows are ONE contiguous slot range [s_hstart[row, lx - 2], s_hstart[row, lx + 3]).  Strict per-type-pair test
-// (P:251-255), entries written in the fixed order (row, slot) -> bitwise reproducible list.  GH: the tile has
-// periodic-image slots (block-uniform).
+// P:226-268 Fig. 5 on the staged halo, one WARP per owned cell.  All particles of a cell share the 5x5x5 stencil
+// (P:237-259): its 25 x-rows are 25 contiguous slot ranges, which the warp first writes out as one flat candidate
+// list in shared memory (~300 slots); then, for each particle of the cell in turn, the 32 lanes test 32 consecutive
+// candidates at a time -- the candidate positions are read with consecutive-slot LDS.128 (no bank conflicts), the
+// particle's position is a broadcast read, no lane idles on a short row and no two lanes diverge.  List slots are
+// handed out by ballot + popc in candidate order: the list is bitwise reproducible (the paper's atomicInc gives "an
+// unspecified sequential order").  Strict per-type-pair test.  GH: the tile has periodic-image
+// slots (block-uniform).  s_cand: TILE_CAND_MAX 16-bit slots per warp.
+#define TILE_CAND_MAX 512 // candidate slots per warp buffer (a 5x5x5 stencil holds ~300 at liquid densities), a multiple of 64
+#define TILE_ROW_MAX 384  // list entries staged per particle (>= the list capacity the tile method accepts)
+#define TILE_WARP_SCRATCH ((TILE_CAND_MAX + TILE_ROW_MAX) * 2) // bytes per warp
 template <bool GH>
-__device__ __forceinline__ void tile_build_rows(const Sys& S, const float4* r, int t, const TileGeo& g, const float4* s_pos,
-                                                const int* s_hstart, const float* s_rcl2, int* max_slot)
+__device__ __forceinline__ void tile_build_rows(const Sys& S, int t, const TileGeo& g, const float4* s_pos,
+                                                const unsigned short* s_hstart, unsigned char* s_scratch,
+                                                const float* s_rcl2, int* max_slot)
 {
     const int hx = g.wx + 4, hy = g.wy + 4;
-    const int o0 = S.cstart_z[g.cellbase], o1 = S.cstart_z[g.cellbase + g.wx * g.wy * g.wz];
+    const int o0 = S.cstart_z[g.cellbase];
     const int pbase = tile_pbase(o0, t);
-    unsigned short* list = reinterpret_cast<unsigned short*>(S.nbl);
-    const int lane = threadIdx.x & 31;
-    for (int o = threadIdx.x; o - lane < o1 - o0; o += blockDim.x) {
-        const int i = o0 + o;
-        const bool have_i = i < o1;
-        int count = 0;
-        if (have_i) {
-            const float4 ri = r[i];
-            int cx, cy, cz;
-            cell_coords(S, ri, cx, cy, cz);
-            const int lx = cx - g.x0 + 2, ly = cy - g.y0 + 2, lz = cz - g.z0 + 2;
-            const int key = g.cellbase + ((cz - g.z0) * g.wy + (cy - g.y0)) * g.wx + (cx - g.x0);
-            const int self = min(s_hstart[(lz * hy + ly) * hx + lx] + (i - S.cstart_z[key]), S.hcap);
-            const float ax = half_shift(ri.x, S.h[0]), ay = half_shift(ri.y, S.h[1]), az = half_shift(ri.z, S.h[2]);
-            const int trow = type_of(ri) * S.ntypes;
-            const float c0 = s_rcl2[trow], c1 = s_rcl2[trow + 1], c2 = s_rcl2[trow + 2], c3 = s_rcl2[trow + 3];
-            const size_t rowbase = tile_entry_index(S, pbase + o, 0);
-            const int tmask = (1 << S.tp_shift) - 1;
-            // entry k of this row: chunk k >> 3 -> (iteration, lane of the particle), then k & 7 inside the chunk
-            auto entry_at = [&](int k) -> unsigned short* {
-                const int c = k >> 3;
-                return list + rowbase + ((((size_t)(c >> S.tp_shift)) << 5) + (c & tmask)) * 8 + (k & 7);
-            };
-            for (int q = 0; q < 25; ++q) {
-                const int row = ((lz + q / 5 - 2) * hy + (ly + q % 5 - 2)) * hx + lx;
-                const int a = min(s_hstart[row - 2], S.hcap), b = min(s_hstart[row + 3], S.hcap);
-                constexpr int U = 4;
-                for (int c = a; c < b; c += U) {
-                    float4 pj[U];
-#pragma unroll
-                    for (int u = 0; u < U; ++u) pj[u] = s_pos[c + u < b ? c + u : self]; // masked: the particle itself
-#pragma unroll
-                    for (int u = 0; u < U; ++u) {
-                        const int w = __float_as_int(pj[u].w);
-                        const float dx = ((GH && (w & 0x100)) ? ax : ri.x) - pj[u].x;
-                        const float dy = ((GH && (w & 0x200)) ? ay : ri.y) - pj[u].y;
-                        const float dz = ((GH && (w & 0x400)) ? az : ri.z) - pj[u].z;
-                        const float d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, dx * dx));
-                        const int tj = GH ? (w & 0xff) : w;
-                        const float thr = S.ntypes <= 2 ? (tj ? c1 : c0) : (tj == 0 ? c0 : tj == 1 ? c1 : tj == 2 ? c2 : c3);
-                        const int slot = c + u < b ? c + u : self;
-                        if (slot != self && d2 < thr) { // strict <, per type pair
-                            if (count < S.cap) *entry_at(count) = (unsigned short)slot;
-                            ++count;
-                        }
-                    }
-                }
-            }
-            // the unused tail of the last chunk points at the far-away dummy slot: the force loop needs no masks
-            for (int k = count; k < S.cap && (k & 7); ++k) *entry_at(k) = (unsigned short)S.hcap;
-            S.num_nbrs[i] = min(count, S.cap);
-            S.r_build[i] = ri;
-            if (count > S.cap) S.sc->overflow = 1u;
+    uint4* list4 = reinterpret_cast<uint4*>(S.nbl);
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    const unsigned lt = (1u << lane) - 1u;
+    unsigned short* s_cand = reinterpret_cast<unsigned short*>(s_scratch + wid * TILE_WARP_SCRATCH);
+    unsigned short* s_row = s_cand + TILE_CAND_MAX; // 16-byte aligned: read back as uint4 chunks
+    const int tmask = (1 << S.tp_shift) - 1;
+    const int ncell_own = g.wx * g.wy * g.wz;
+    const int rowcap = min(S.cap, TILE_ROW_MAX);
+    int wmax = 0;
+    for (int oc = wid; oc < ncell_own; oc += nw) { // own cells in key order: key = cellbase + oc
+        const int lx = oc % g.wx + 2, ly = (oc / g.wx) % g.wy + 2, lz = oc / (g.wx * g.wy) + 2;
+        const int hc = (lz * hy + ly) * hx + lx;
+        const int s_first = s_hstart[hc], np = s_hstart[hc + 1] - s_first;
+        if (np <= 0) continue;
+        const int g_first = S.cstart_z[g.cellbase + oc];
+        // slot ranges of the 25 stencil rows, one per lane; their running offsets in the flat candidate list
+        int a = 0, len = 0;
+        if (lane < 25) {
+            const int row = ((lz + lane / 5 - 2) * hy + (ly + lane % 5 - 2)) * hx + lx;
+            a = s_hstart[row - 2];
+            len = min(s_hstart[row + 3] - a, TILE_CAND_MAX);
         }
-        const int wmax = __reduce_max_sync(FULLMASK, count);
-        if (lane == 0) atomicMax(max_slot, wmax);
+        int off = len; // inclusive scan
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int y = __shfl_up_sync(FULLMASK, off, o);
+            if (lane >= o) off += y;
+        }
+        const int total = __shfl_sync(FULLMASK, off, 31);
+        off -= len;
+        const bool one_batch = total <= TILE_CAND_MAX; // (nearly always: then the list is written once per cell)
+        for (int p = 0; p < np; ++p) {
+            const int self = s_first + p;
+            const float4 ri = s_pos[self]; // broadcast read; own cells are never periodic images
+            const float ax = half_shift(ri.x, S.h[0]), ay = half_shift(ri.y, S.h[1]), az = half_shift(ri.z, S.h[2]);
+            const float* thr_of = s_rcl2 + type_of(ri) * S.ntypes; // list cutoffs of this particle's type (S4)
+            const bool one_type = S.ntypes == 1;
+            const float thr_one = s_rcl2[0];
+            int count = 0;
+            for (int row0 = 0; row0 < 25;) {
+                // the batch of rows [row0, row1) that fits the candidate buffer
+                const int off0 = __shfl_sync(FULLMASK, off, row0);
+                const bool fits = lane >= row0 && lane < 25 && off + len - off0 <= TILE_CAND_MAX;
+                const int row1 = row0 + max(1, __popc(__ballot_sync(FULLMASK, fits)));
+                const int btotal = __shfl_sync(FULLMASK, off + len, row1 - 1) - off0;
+                if (p == 0 || !one_batch) {
+                    __syncwarp();
+                    if (lane >= row0 && lane < row1)
+                        for (int j = 0; j < len; ++j) s_cand[off - off0 + j] = (unsigned short)(a + j);
+                    // pad to a multiple of 64 with the far-away dummy slot: the passes below need no bounds checks
+                    for (int n = btotal + lane; n < ((btotal + 63) & ~63); n += 32) s_cand[n] = (unsigned short)S.hcap;
+                    __syncwarp();
+                }
+                // two passes of 32 candidates per iteration (two independent chains of shared-memory reads in flight)
+                for (int n0 = 0; n0 < btotal; n0 += 64) {
+                    const int slot0 = s_cand[n0 + lane], slot1 = s_cand[n0 + 32 + lane];
+                    const float4 p0 = s_pos[slot0], p1 = s_pos[slot1];
+                    const int w0 = __float_as_int(p0.w), w1 = __float_as_int(p1.w);
+                    const float dx0 = ((GH && (w0 & 0x100)) ? ax : ri.x) - p0.x, dx1 = ((GH && (w1 & 0x100)) ? ax : ri.x) - p1.x;
+                    const float dy0 = ((GH && (w0 & 0x200)) ? ay : ri.y) - p0.y, dy1 = ((GH && (w1 & 0x200)) ? ay : ri.y) - p1.y;
+                    const float dz0 = ((GH && (w0 & 0x400)) ? az : ri.z) - p0.z, dz1 = ((GH && (w1 & 0x400)) ? az : ri.z) - p1.z;
+                    const float d20 = __fmaf_rn(dz0, dz0, __fmaf_rn(dy0, dy0, dx0 * dx0));
+                    const float d21 = __fmaf_rn(dz1, dz1, __fmaf_rn(dy1, dy1, dx1 * dx1));
+                    const float t0 = one_type ? thr_one : thr_of[GH ? (w0 & 0xff) : w0];
+                    const float t1 = one_type ? thr_one : thr_of[GH ? (w1 & 0xff) : w1];
+                    // strict <, per type pair; bitwise &: both sides are always evaluated, no branch
+                    const bool acc0 = (slot0 != self) & (d20 < t0), acc1 = (slot1 != self) & (d21 < t1);
+                    const unsigned m0 = __ballot_sync(FULLMASK, acc0), m1 = __ballot_sync(FULLMASK, acc1);
+                    const int k0 = count + __popc(m0 & lt), k1 = count + __popc(m0) + __popc(m1 & lt);
+                    if (acc0 && k0 < rowcap) s_row[k0] = (unsigned short)(slot0 << 4);
+                    if (acc1 && k1 < rowcap) s_row[k1] = (unsigned short)(slot1 << 4);
+                    count += __popc(m0) + __popc(m1);
+                }
+                row0 = row1;
+            }
+            // close the row: pad the last chunk with the far-away dummy slot (the force loop needs no masks), then
+            // the chunks go out as 16-byte stores, chunk c to (iteration c / tp, lane c % tp of the particle)
+            const int i = g_first + p;
+            const int kept = min(count, rowcap), nch = (kept + 7) >> 3;
+            __syncwarp();
+            if (kept + lane < nch * 8) s_row[kept + lane] = (unsigned short)(S.hcap << 4); // (at most 7 pads)
+            __syncwarp();
+            if (lane < nch || lane + 32 < nch) {
+                const int v = pbase + (i - o0);
+                const size_t base4 = (((size_t)(v >> S.ppw_shift) * S.cap_it8) << 5) + ((v & ((1 << S.ppw_shift) - 1)) << S.tp_shift);
+                for (int c = lane; c < nch; c += 32)
+                    list4[base4 + ((size_t)(c >> S.tp_shift) << 5) + (c & tmask)] = reinterpret_cast<const uint4*>(s_row)[c];
+            }
+            if (lane == 0) {
+                S.num_nbrs[i] = kept;
+                S.r_build[i] = ri;
+                if (count > S.cap) S.sc->overflow = 1u;
+            }
+            wmax = max(wmax, count);
+        }
     }
+    if (lane == 0 && wmax > 0) atomicMax(max_slot, wmax);
 }
 
 // whole build of one tile by one block (halo layout, then the rows of the owned particles)
-__device__ __forceinline__ void ph_build_tile(const Sys& S, const float4* r, int t, float4* s_pos, int* s_hstart,
-                                              int* s_warp, const float* s_rcl2, int* max_slot)
+__device__ __forceinline__ void ph_build_tile(const Sys& S, const float4* r, int t, float4* s_pos, unsigned short* s_hstart,
+                                              unsigned char* s_scratch, int* s_warp, const float* s_rcl2, int* max_slot)
 {
     const TileGeo g = tile_geo(S, t);
     __syncthreads(); // the previous tile's rows are done with the shared arrays
     tile_layout_halo(S, r, t, g, s_pos, s_hstart, s_warp);
     if (tile_wrap_axes(S, g))
-        tile_build_rows<true>(S, r, t, g, s_pos, s_hstart, s_rcl2, max_slot);
+        tile_build_rows<true>(S, t, g, s_pos, s_hstart, s_scratch, s_rcl2, max_slot);
     else
-        tile_build_rows<false>(S, r, t, g, s_pos, s_hstart, s_rcl2, max_slot);
+        tile_build_rows<false>(S, t, g, s_pos, s_hstart, s_scratch, s_rcl2, max_slot);
 }
 
 // ------------------------------------------------------------------------------------------ A5 from shared memory
@@ -254,14 +320,25 @@ __device__ __forceinline__ void tile_force_loop(const Sys& S, const float4* s_po
         if (COUL == 2) px = s_pp[3];
     }
     const float ax = half_shift(ri.x, S.h[0]), ay = half_shift(ri.y, S.h[1]), az = half_shift(ri.z, S.h[2]);
-    const unsigned dummy = (unsigned)S.hcap * 0x00010001u;
-    for (int it = 0; it < nch_w; ++it) {
+    // list entries are slot numbers times 16 (the byte offset of the slot: hcap <= 4095 keeps them in 16 bits)
+    const unsigned dummy = (unsigned)(S.hcap << 4) * 0x00010001u;
+    const unsigned char* sbase = reinterpret_cast<const unsigned char*>(s_pos);
+    auto chunk = [&](int it) {
         uint4 e = make_uint4(dummy, dummy, dummy, dummy);
         if (it < nch) e = NC ? __ldg(chunks + (size_t)it * 32) : __ldcs(chunks + (size_t)it * 32);
+        return e;
+    };
+    // two chunks in flight ahead of the one being worked on: the list streams from L2 / HBM
+    uint4 e0 = chunk(0), e1 = chunk(1);
+    for (int it = 0; it < nch_w; ++it) {
+        const uint4 e = e0;
+        e0 = e1;
+        e1 = chunk(it + 2);
         const unsigned ew[4] = {e.x, e.y, e.z, e.w};
         float4 rj[8];
 #pragma unroll
-        for (int q = 0; q < 8; ++q) rj[q] = s_pos[(q & 1) ? (ew[q >> 1] >> 16) : (ew[q >> 1] & 0xffffu)];
+        for (int q = 0; q < 8; ++q)
+            rj[q] = *reinterpret_cast<const float4*>(sbase + ((q & 1) ? (ew[q >> 1] >> 16) : (ew[q >> 1] & 0xffffu)));
 #pragma unroll
         for (int q = 0; q < 8; ++q) {
             const int wj = __float_as_int(rj[q].w);
@@ -330,10 +407,12 @@ __device__ __forceinline__ void tile_force_own(const Sys& S, const float4* r, in
 // ------------------------------------------------------------------------------------------ stand-alone kernels
 
 // carve the dynamic shared memory of a tile kernel
-__device__ __forceinline__ void tile_smem(const Sys& S, unsigned char* raw, float4*& s_pos, int*& s_hstart)
+__device__ __forceinline__ void tile_smem(const Sys& S, unsigned char* raw, float4*& s_pos, unsigned short*& s_hstart,
+                                          unsigned char*& s_scratch)
 {
     s_pos = reinterpret_cast<float4*>(raw);
-    s_hstart = reinterpret_cast<int*>(raw + (size_t)(S.hcap + 1) * 16);
+    s_scratch = raw + (size_t)(S.hcap + 1) * 16;                                      // 16-byte aligned
+    s_hstart = reinterpret_cast<unsigned short*>(s_scratch + (TILE_THREADS / 32) * TILE_WARP_SCRATCH);
 }
 
 // A5 of the tile method as its own kernel (rumd_compute_forces, the per-step path, rumd_time_force): one block per
@@ -343,9 +422,7 @@ __global__ void __launch_bounds__(TILE_THREADS) k_force_tile(const Sys S)
 {
     extern __shared__ __align__(16) unsigned char tile_raw[];
     __shared__ float4 s_pp[4 * RUMD_MAXT * RUMD_MAXT];
-    float4* s_pos;
-    int* s_hstart;
-    tile_smem(S, tile_raw, s_pos, s_hstart);
+    float4* s_pos = reinterpret_cast<float4*>(tile_raw);
     load_pair_table(S, s_pp);
     if (blockIdx.x == 0 && threadIdx.x == 0) finish_rebuild(S);
     for (int t = blockIdx.x; t < S.ntiles; t += gridDim.x) {
@@ -370,11 +447,12 @@ static __global__ void __launch_bounds__(TILE_THREADS) k_build_tile(const Sys S)
     __shared__ float s_rcl2[RUMD_MAXT * RUMD_MAXT];
     __shared__ int s_warp[33];
     float4* s_pos;
-    int* s_hstart;
-    tile_smem(S, tile_raw, s_pos, s_hstart);
+    unsigned short* s_hstart;
+    unsigned char* s_scratch;
+    tile_smem(S, tile_raw, s_pos, s_hstart, s_scratch);
     if (threadIdx.x < RUMD_MAXT * RUMD_MAXT) s_rcl2[threadIdx.x] = S.pp[threadIdx.x].rcl2;
     for (int t = blockIdx.x; t < S.ntiles; t += gridDim.x)
-        ph_build_tile(S, S.r, t, s_pos, s_hstart, s_warp, s_rcl2, max_slot_of(S));
+        ph_build_tile(S, S.r, t, s_pos, s_hstart, s_scratch, s_warp, s_rcl2, max_slot_of(S));
 }
 
 // Row-major export of the tile method's list in SLOT numbering of the particles (inspection / parity tests): the
@@ -391,6 +469,6 @@ static __global__ void k_export_nbl_tile(const Sys S, int* count, int* list, int
     const unsigned short* l16 = reinterpret_cast<const unsigned short*>(S.nbl);
     if (threadIdx.x == 0) count[i] = c;
     for (int k = threadIdx.x; k < rowcap; k += blockDim.x)
-        list[(size_t)i * rowcap + k] = k < c ? (S.halo_idx[(size_t)t * S.hcap + l16[tile_entry_index(S, v, k)]] & TILE_IDX_MASK) : -1;
+        list[(size_t)i * rowcap + k] = k < c ? (S.halo_idx[(size_t)t * S.hcap + (l16[tile_entry_index(S, v, k)] >> 4)] & TILE_IDX_MASK) : -1;
 }
 #endif // RUMD_MAIN_TU
