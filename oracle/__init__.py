@@ -25,7 +25,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "rumd_oracle.c")
 _LIB = os.path.join(_HERE, "librumd_oracle.so")
 
-NVE, NVT = 0, 1
+NVE, NVT, NPT = 0, 1, 2
 POT_STRIDE = 11
 
 
@@ -74,6 +74,11 @@ def lib():
         L.orc_run.argtypes = [C.c_int, _dp, _dp, _dp, _ip, _ip, _dp, C.c_int, _dp, C.c_double, C.c_double,
                               C.c_int, C.c_double, C.c_double, _dp, C.c_long, C.c_int, _dp]
         L.orc_run.restype = C.c_long
+        L.orc_integrate_npt.argtypes = [C.c_int, _dp, _dp, _dp, _ip, _dp, C.c_double, _dp, C.c_double, C.c_double,
+                                        C.c_double, C.c_double, C.c_double, C.c_double, _dp, _dp]
+        L.orc_run_npt.argtypes = [C.c_int, _dp, _dp, _dp, _ip, _ip, _dp, C.c_int, _dp, C.c_double, C.c_double,
+                                  C.c_double, C.c_double, C.c_double, C.c_double, _dp, C.c_long, C.c_int, _dp]
+        L.orc_run_npt.restype = C.c_long
         _lib = L
     return _lib
 
@@ -247,3 +252,43 @@ def run(r, v, m, image, types, box, pot, skin, dt, nsteps, mode=NVE, T0=1.0, tau
     if nb < 0:
         raise MemoryError("orc_run")
     return dict(r=r, v=v, image=image, xi=float(th[0]), eta=float(th[1]), n_builds=int(nb), log=log)
+
+
+def integrate_npt(r, v, m, image, F, Wvir, box, dt, T0, tau, P0, tauP, xi=0.0, eta=0.0, nu=0.0):
+    """One NPT leap-frog step (reading S32) given F and the pair virial W; nu is the strain rate as the previous step
+    left it (nu_o of orc_integrate_npt).  Returns new (r, v, image, box, xi, eta, nu_o, K_t, sum_m_v2)."""
+    r = _f64(r).copy()
+    v = _f64(v).copy()
+    N = r.shape[0]
+    m = _f64(m, (N,))
+    image = _i32(image).copy()
+    F = _f64(F, (N, 3))
+    box = _f64(box, (3,)).copy()
+    st = np.array([xi, eta, nu, nu], dtype=np.float64)
+    out = np.zeros(2)
+    g = 3.0 * N - 3.0
+    lib().orc_integrate_npt(N, _d(r), _d(v), _d(m), _i(image), _d(F), float(Wvir), _d(box), float(dt), float(T0),
+                            float(tau), float(P0), float(tauP), g, _d(st), _d(out))
+    return r, v, image, box, float(st[0]), float(st[1]), float(st[2]), float(out[0]), float(out[1])
+
+
+def run_npt(r, v, m, image, types, box, pot, skin, dt, nsteps, T0, tau, P0, tauP, xi=0.0, eta=0.0, nu=0.0,
+            use_cell=False, want_log=True):
+    """nsteps of NPT dynamics.  Returns dict(r, v, image, box, xi, eta, nu, n_builds, log) with
+    log[s] = (U, K, W, xi, eta, H, nu, V, P) at integer time t_s (before the step's update)."""
+    r, N, types, box, pot, nt = _prep(r, types, box, pot)
+    r = r.copy()
+    box = box.copy()
+    v = _f64(v).copy()
+    m = _f64(m, (N,))
+    image = _i32(image).copy()
+    st = np.array([xi, eta, nu, nu], dtype=np.float64)
+    log = np.zeros((int(nsteps), 9)) if want_log else None
+    nb = lib().orc_run_npt(N, _d(r), _d(v), _d(m), _i(image), _i(types), _d(box), nt, _d(pot), float(skin), float(dt),
+                           float(T0), float(tau), float(P0), float(tauP), _d(st), int(nsteps), int(bool(use_cell)),
+                           _d(log) if want_log else None)
+    if nb < 0:
+        raise MemoryError("orc_run_npt")
+    return dict(r=r, v=v, image=image, box=box, xi=float(st[0]), eta=float(st[1]), nu=float(st[2]), n_builds=int(nb),
+                log=log)
+

@@ -24,6 +24,12 @@
  *       quantity H fluctuation ~ dt^2, <T_kin> -> T0.  The discretisation itself is a reading
  *       (S9): "parity unpinned" against the paper for NVT trajectories (the paper prints no
  *       Nose-Hoover equations).
+ *   orc_integrate_npt / orc_run_npt (NPT)   : barostat off (tau_P = inf, nu = 0) reproduces the NVT trajectory
+ *       bit for bit; free flight under a constant strain rate against the closed-form solution (box
+ *       L exp(nu t) exactly, velocity decay to second order in dt); conserved quantity fluctuation ~ dt^2;
+ *       <P> -> P0 and the volume moves toward the target.  The leap-frog discretisation of the
+ *       Martyna-Tobias-Klein equations (P:78 ref. [51]) is a reading (S32): "parity unpinned" against the
+ *       paper for NPT trajectories (the paper prints no equations of motion).
  *
  * Conventions: positions r[3*i+k], velocities v[3*i+k], forces F[3*i+k]; box[3] = (Lx,Ly,Lz),
  * orthorhombic, origin-centred, coordinates in [-L/2, L/2] (S7).  Potentials are one record of
@@ -548,3 +554,142 @@ long orc_run(int N, double *r, double *v, const double *m, int *image, const int
     free(w);
     return nbuild;
 }
+
+/* ---------------------------------------------------------------- NPT ("NPT [51]") ---------- */
+
+/* Isotropic constant-pressure dynamics of Martyna, Tobias and Klein (P:455 ref. [51]) with the Nose-Hoover
+ * thermostat of O7 acting on the particles; the paper prints no equations, so this is reading S32:
+ *     dr/dt = v + nu r                     nu = strain rate of the box, dL/dt = nu L (all three lengths)
+ *     dv/dt = F/m - [xi + (1 + 3/g) nu] v
+ *     dnu/dt = cP [ (1 + 3/g) sum m v^2 + W - 3 V P0 ],  cP = wP2 / ((g + 3) T0), wP2 = (2 pi / tau_P)^2
+ *              (= [3 V (P - P0) + (3/g) sum m v^2] / Wb with 3 V P = sum m v^2 + W, W = sum_i w_i the pair virial,
+ *               Wb = (g + 3) T0 / wP2)
+ *     dxi/dt = w2 (sum m v^2 / (g T0) - 1),  deta/dt = xi
+ * conserved: H = K + U + P0 V + Wb nu^2 / 2 + g T0 xi^2 / (2 w2) + g T0 eta.
+ * Leap-frog form in the order of O7.  xi and nu live at integer times.  The part of dnu/dt that depends on the
+ * positions, pos(t) = cP [W(t) - 3 V(t) P0], is applied as two half kicks around the force evaluation (closing the
+ * previous step, opening this one), the kinetic part as one whole kick with the half-step velocities:
+ *     nu(t)     = nu_o + dt/2 pos(t)                      nu_o: the strain rate as the previous step left it
+ *     gam       = xi(t) + (1 + 3/g) nu(t)
+ *     v(t+dt/2) = [ (1 - gam dt/2) v(t-dt/2) + dt F(t)/m ] / (1 + gam dt/2)
+ *     nu_h      = nu(t) + dt/2 pos(t) + dt/2 cP (1 + 3/g) sum m v(t-dt/2)^2        strain rate of the drift
+ *     sh = exp(nu_h dt / 2), s = sh^2 ;  r(t+dt) = s r(t) + dt sh v(t+dt/2) ;  L(t+dt) = s L(t) ;  wrap (new box, S7)
+ *     xi(t+dt)  = xi + dt w2 (sum m v(t+dt/2)^2 / (g T0) - 1) ;  eta(t+dt) = eta + dt/2 [xi(t) + xi(t+dt)]
+ *     nu_o'     = nu(t) + dt/2 pos(t) + dt cP (1 + 3/g) sum m v(t+dt/2)^2
+ * tau_P <= 0 or inf: cP = 0, the strain rate stays what it is (0: exactly the NVT step of orc_integrate).
+ * state[0] = xi, state[1] = eta, state[2] = nu_o (in: as left by the previous step; a run starts with nu_o = the
+ * wanted nu(0) minus its first closing half kick, normally 0), state[3] = nu(t) of THIS step (out, for H(t)).
+ * box is updated in place.  out[0] = K(t) (O10), out[1] = sum m |v(t+dt/2)|^2. */
+void orc_integrate_npt(int N, double *r, double *v, const double *m, int *image, const double *F, double Wvir,
+                       double *box, double dt, double T0, double tau, double P0, double tauP, double g,
+                       double *state, double *out)
+{
+    double w2 = 0.0, wP2 = 0.0;
+    if (tau > 0.0 && isfinite(tau)) w2 = (2.0 * M_PI / tau) * (2.0 * M_PI / tau);
+    if (tauP > 0.0 && isfinite(tauP)) wP2 = (2.0 * M_PI / tauP) * (2.0 * M_PI / tauP);
+    const double cP = wP2 / ((g + 3.0) * T0);
+    const double vol = box[0] * box[1] * box[2];
+    const double pos = cP * (Wvir - 3.0 * vol * P0);
+    const double xi = state[0];
+    const double nu = state[2] + 0.5 * dt * pos;
+    double mv2_old = 0.0;
+    for (int i = 0; i < N; ++i)
+        for (int k = 0; k < 3; ++k) mv2_old += m[i] * v[3 * i + k] * v[3 * i + k];
+    const double nu_h = nu + 0.5 * dt * pos + 0.5 * dt * cP * (1.0 + 3.0 / g) * mv2_old;
+    const double gam = xi + (1.0 + 3.0 / g) * nu;
+    const double sh = exp(0.5 * nu_h * dt), s = sh * sh;
+    double boxn[3];
+    for (int k = 0; k < 3; ++k) boxn[k] = s * box[k];
+    double Kt = 0.0, mv2 = 0.0;
+    for (int i = 0; i < N; ++i) {
+        for (int k = 0; k < 3; ++k) {
+            double vo = v[3 * i + k];
+            double vn = ((1.0 - 0.5 * gam * dt) * vo + dt * F[3 * i + k] / m[i]) / (1.0 + 0.5 * gam * dt);
+            double vh = 0.5 * (vo + vn);
+            Kt += 0.5 * m[i] * vh * vh;
+            mv2 += m[i] * vn * vn;
+            v[3 * i + k] = vn;
+            double x = s * r[3 * i + k] + dt * sh * vn;
+            double n = rint(x / boxn[k]);
+            r[3 * i + k] = x - boxn[k] * n;
+            image[3 * i + k] += (int)n;
+        }
+    }
+    double xin = xi + dt * w2 * (mv2 / g / T0 - 1.0);
+    state[1] += 0.5 * dt * (xi + xin);
+    state[0] = xin;
+    state[3] = nu;
+    state[2] = nu + 0.5 * dt * pos + dt * cP * (1.0 + 3.0 / g) * mv2;
+    for (int k = 0; k < 3; ++k) box[k] = boxn[k];
+    out[0] = Kt;
+    out[1] = mv2;
+}
+
+/* nsteps of NPT dynamics, step order O8.  The list is rebuilt at EVERY step (the box changes every step; any valid
+ * list gives the same forces, O5), by the cell search when use_cell != 0 and the box allows it, else the N^2 search.
+ * log (may be NULL): 9 doubles per step = U(t), K(t), W(t), xi(t), eta(t), H(t), nu(t), V(t), P(t) = (2 K + W)/(3 V),
+ *   H = K + U + P0 V + (g + 3) T0 nu^2 / (2 wP2) + g T0 xi^2 / (2 w2) + g T0 eta  (terms with w2 / wP2 = 0 dropped).
+ * state: 4 doubles (xi, eta, nu_o, nu(t) of the last step), see orc_integrate_npt.
+ * Returns the number of list builds, or -1 on allocation failure. */
+long orc_run_npt(int N, double *r, double *v, const double *m, int *image, const int *type, double *box, int nt,
+                 const double *pot, double skin, double dt, double T0, double tau, double P0, double tauP,
+                 double *state, long nsteps, int use_cell, double *log)
+{
+    int cap = 64;
+    int *count = (int *)malloc(sizeof(int) * (size_t)N);
+    int *list = (int *)malloc(sizeof(int) * (size_t)N * cap);
+    double *F = (double *)malloc(sizeof(double) * 3 * (size_t)N);
+    double *u = (double *)malloc(sizeof(double) * (size_t)N);
+    double *w = (double *)malloc(sizeof(double) * (size_t)N);
+    if (!count || !list || !F || !u || !w) return -1;
+    double g = 3.0 * N - 3.0; /* S10 */
+    double w2 = 0.0, wP2 = 0.0;
+    if (tau > 0.0 && isfinite(tau)) w2 = (2.0 * M_PI / tau) * (2.0 * M_PI / tau);
+    if (tauP > 0.0 && isfinite(tauP)) wP2 = (2.0 * M_PI / tauP) * (2.0 * M_PI / tauP);
+    long nbuild = 0;
+    for (long s = 0; s < nsteps; ++s) {
+        for (;;) {
+            int mc = -1;
+            if (use_cell) mc = orc_nblist_cell(N, r, type, box, nt, pot, skin, cap, count, list);
+            if (mc < 0) mc = orc_nblist_n2(N, r, type, box, nt, pot, skin, cap, count, list);
+            if (mc <= cap) break;
+            while (cap < mc) cap *= 2;
+            free(list);
+            list = (int *)malloc(sizeof(int) * (size_t)N * cap);
+            if (!list) return -1;
+        }
+        ++nbuild;
+        orc_forces_list(N, r, type, box, nt, pot, cap, count, list, F, u, w);
+        double U = 0.0, W = 0.0;
+        for (int i = 0; i < N; ++i) {
+            U += u[i];
+            W += w[i];
+        }
+        const double xi = state[0], eta = state[1], vol = box[0] * box[1] * box[2];
+        double out[2];
+        orc_integrate_npt(N, r, v, m, image, F, W, box, dt, T0, tau, P0, tauP, g, state, out);
+        const double nu = state[3]; /* the strain rate at the integer time t of this step */
+        if (log) {
+            double H = out[0] + U + P0 * vol + g * T0 * eta;
+            if (w2 > 0.0) H += 0.5 * g * T0 * xi * xi / w2;
+            if (wP2 > 0.0) H += 0.5 * (g + 3.0) * T0 * nu * nu / wP2;
+            double *l = log + 9 * s;
+            l[0] = U;
+            l[1] = out[0];
+            l[2] = W;
+            l[3] = xi;
+            l[4] = eta;
+            l[5] = H;
+            l[6] = nu;
+            l[7] = vol;
+            l[8] = (2.0 * out[0] + W) / (3.0 * vol);
+        }
+    }
+    free(count);
+    free(list);
+    free(F);
+    free(u);
+    free(w);
+    return nbuild;
+}
+

@@ -740,3 +740,128 @@ def test_extra_potentials_list_forces_equal_brute_force_and_newton():
     Um = oracle.forces_allpairs(r64 * (1 - lam), t, box * (1 - lam), pot)[1].sum()
     # only valid for continuous energies: the shifted-potential AB term is continuous in u, fine
     assert (Up - Um) / (2 * lam) == pytest.approx(-w.sum(), rel=2e-5)
+
+
+# ------------------------------------------------------------------ P13: NPT ("NPT [51]"; reading S32)
+
+
+def _lj_fluid(ncell=3, density=0.7, T=1.5, seed=11):
+    r, box = W.fcc_lattice(ncell, ncell, ncell, density)
+    rng = np.random.default_rng(seed)
+    N = r.shape[0]
+    m = np.ones(N)
+    v = W.maxwell_boltzmann(rng, m, T)
+    return r, v, m, np.zeros((N, 3), np.int32), np.zeros(N, np.int32), box, LJ
+
+
+def test_P13_npt_with_the_barostat_off_is_nvt_bit_for_bit():
+    """tau_P = inf and nu(0) = 0: the strain rate stays 0, exp(0) = 1, and every expression of the NPT step reduces
+    to the NVT step of O7 -- positions, velocities, thermostat and box identical bit for bit over 60 steps."""
+    r, v, m, im, t, box, pot = _lj_fluid()
+    a = oracle.run(r, v, m, im, t, box, pot, 0.3, 0.004, 60, mode=oracle.NVT, T0=1.2, tau=0.2)
+    b = oracle.run_npt(r, v, m, im, t, box, pot, 0.3, 0.004, 60, T0=1.2, tau=0.2, P0=3.0, tauP=float("inf"))
+    assert np.array_equal(a["r"], b["r"]) and np.array_equal(a["v"], b["v"]) and np.array_equal(a["image"], b["image"])
+    assert a["xi"] == b["xi"] and a["eta"] == b["eta"] and b["nu"] == 0.0 and np.array_equal(b["box"], box)
+    assert np.array_equal(a["log"][:, :5], b["log"][:, :5])
+    # ... and with P0 = 0 the conserved quantities coincide too (H_NPT = H_NVT + P0 V)
+    c = oracle.run_npt(r, v, m, im, t, box, pot, 0.3, 0.004, 60, T0=1.2, tau=0.2, P0=0.0, tauP=0.0)
+    assert np.array_equal(a["log"][:, 5], c["log"][:, 5])
+
+
+def test_P13_npt_free_flight_under_constant_strain_rate_closed_form():
+    """No forces (rc far below every distance is not needed: an empty potential table), thermostat off, barostat
+    frozen at nu = nu0 (tau_P = inf): the continuous equations integrate in closed form,
+        L(t) = L0 exp(nu0 t),   v(t) = v0 exp(-(1 + 3/g) nu0 t),   unwrapped r(t) = e^{nu0 t} [ r0 + v0 (1 - e^{-k t}) / k ],
+    k = (2 + 3/g) nu0.  The discrete box follows L0 exp(nu0 n dt) EXACTLY; velocities and positions converge to the
+    closed form with the second order of a leap-frog scheme (error ratio 4 when dt is halved)."""
+    N, L0, nu0, T = 5, 9.0, 0.37, 0.8
+    rng = np.random.default_rng(3)
+    r0 = rng.uniform(-1.0, 1.0, (N, 3))
+    v0 = rng.standard_normal((N, 3))
+    m = np.ones(N)
+    g = 3.0 * N - 3.0
+    pot = W.pot_table(1)                         # no potential terms at all: F = 0, W = 0
+    k = (2.0 + 3.0 / g) * nu0
+    errs = []
+    for n in (40, 80, 160):
+        dt = T / n
+        # leap-frog input velocities are v(-dt/2): the closed form evaluated there
+        vm = v0 * math.exp((1.0 + 3.0 / g) * nu0 * 0.5 * dt)
+        o = oracle.run_npt(r0, vm, m, np.zeros((N, 3), np.int32), np.zeros(N, np.int32), np.full(3, L0), pot, 0.3, dt, n,
+                           T0=1.0, tau=0.0, P0=0.0, tauP=float("inf"), nu=nu0)
+        assert np.allclose(o["box"], L0 * math.exp(nu0 * T), rtol=1e-13)        # product of exp(nu0 dt): exact
+        assert o["nu"] == nu0 and o["xi"] == 0.0
+        v_exact = v0 * math.exp(-(1.0 + 3.0 / g) * nu0 * (T - 0.5 * dt))         # v(T - dt/2)
+        r_exact = math.exp(nu0 * T) * (r0 + v0 * (1.0 - math.exp(-k * T)) / k)
+        r_unwrapped = o["r"] + o["image"] * o["box"]
+        errs.append((np.abs(o["v"] - v_exact).max(), np.abs(r_unwrapped - r_exact).max()))
+    for col in (0, 1):
+        assert errs[0][col] / errs[1][col] == pytest.approx(4.0, rel=0.15)
+        assert errs[1][col] / errs[2][col] == pytest.approx(4.0, rel=0.15)
+    assert errs[2][0] < 1e-5 and errs[2][1] < 1e-4
+
+
+def test_P13_npt_single_step_worked_example():
+    """One step with numbers chosen so the scale factors are powers of two: N = 2 (g = 3), xi = 0, barostat frozen
+    (tau_P = 0) at nu with nu dt / 2 = ln 2 -> sh = 2, s = 4, gam dt / 2 = (1 + 3/3) nu dt / 2 = 2 ln 2.  F = 0:
+        v' = (1 - 2 ln 2)/(1 + 2 ln 2) v,   r' = 4 r + dt * 2 * v',   L' = 4 L.
+    Then the strain-rate update with the barostat on (W = 7, P0 = 0.2, tau_P = 2): two half kicks of the position part
+    pos = cP (W - 3 V P0) around nu(t), one whole kick of the kinetic part (1 + 3/g) cP sum m v'^2."""
+    dt, ln2 = 0.5, math.log(2.0)
+    nu = 2.0 * ln2 / dt
+    r = np.array([[0.25, -0.5, 0.125], [-0.75, 0.5, 0.375]])
+    v = np.array([[1.0, -2.0, 0.5], [-1.0, 2.0, -0.5]])
+    m = np.array([1.0, 2.0])
+    box = np.array([4.0, 5.0, 6.0])
+    T0 = 1.5
+    rn, vn, im, boxn, xi, eta, nun, Kt, mv2 = oracle.integrate_npt(r, v, m, np.zeros((2, 3), np.int32), np.zeros((2, 3)), 0.0,
+                                                                   box, dt, T0, 0.0, 0.2, 0.0, nu=nu)
+    fac = (1.0 - 2.0 * ln2) / (1.0 + 2.0 * ln2)
+    assert np.allclose(vn, fac * v, rtol=1e-14)
+    assert np.allclose(boxn, 4.0 * box, rtol=1e-14)
+    x = 4.0 * r + dt * 2.0 * fac * v
+    assert np.allclose(rn + im * boxn, x, rtol=1e-13, atol=1e-14)
+    assert np.all(np.abs(rn) <= 0.5 * boxn + 1e-12)
+    assert mv2 == pytest.approx((m[:, None] * (fac * v) ** 2).sum(), rel=1e-14)
+    assert nun == nu and xi == 0.0 and eta == 0.0
+    assert Kt == pytest.approx(0.5 * (m[:, None] * (0.5 * (1.0 + fac) * v) ** 2).sum(), rel=1e-14)
+    # barostat on: V = 120, g = 3, cP = pi^2 / (6 T0) for tau_P = 2
+    Wv, P0 = 7.0, 0.2
+    cP = math.pi ** 2 / (6.0 * T0)
+    pos = cP * (Wv - 3.0 * 120.0 * P0)
+    nu_t = nu + 0.5 * dt * pos
+    gam = 2.0 * nu_t
+    v2 = (1.0 - 0.5 * gam * dt) / (1.0 + 0.5 * gam * dt) * v
+    smv2_old, smv2_new = (m[:, None] * v * v).sum(), (m[:, None] * v2 * v2).sum()
+    out = oracle.integrate_npt(r, v, m, np.zeros((2, 3), np.int32), np.zeros((2, 3)), Wv, box, dt, T0, 0.0, P0, 2.0, nu=nu)
+    assert np.allclose(out[1], v2, rtol=1e-13)
+    assert out[6] == pytest.approx(nu_t + 0.5 * dt * pos + dt * cP * 2.0 * smv2_new, rel=1e-13)
+    nu_h = nu_t + 0.5 * dt * pos + 0.5 * dt * cP * 2.0 * smv2_old
+    assert np.allclose(out[3], box * math.exp(nu_h * dt), rtol=1e-13)
+
+
+def test_P13_npt_conserved_quantity_and_target_pressure():
+    """LJ fluid, N = 500: (a) the conserved quantity H_NPT fluctuates ~ dt^2 with no drift; (b) started at a pressure
+    well below P0 the volume shrinks, and the time-averaged pressure settles at P0 (and <T_kin> at T0)."""
+    r, v, m, im, t, box, pot = _lj_fluid(ncell=5, density=0.5, T=2.0, seed=5)
+    N = r.shape[0]
+    T0, P0, tauP = 2.0, 2.0, 2.0
+    eq = oracle.run_npt(r, v, m, im, t, box, pot, 0.3, 0.004, 1500, T0=T0, tau=0.2, P0=P0, tauP=tauP)
+    assert eq["log"][0, 8] < 0.5 * P0                        # the start is far below the target pressure ...
+    assert np.prod(eq["box"]) < 0.95 * np.prod(box)          # ... so the box has shrunk
+    amp = []
+    for dt, n in ((0.004, 1000), (0.002, 2000)):
+        o = oracle.run_npt(eq["r"], eq["v"], m, eq["image"], t, eq["box"], pot, 0.3, dt, n, T0=T0, tau=0.2, P0=P0, tauP=tauP,
+                           xi=eq["xi"], eta=eq["eta"], nu=eq["nu"])
+        H = o["log"][:, 5] / N
+        tt = np.arange(n) * dt
+        fit = np.polyfit(tt, H, 1)
+        amp.append(np.std(H - np.polyval(fit, tt)))
+        assert abs(fit[0]) * n * dt < 2e-3                   # no drift over the run
+    assert amp[0] / amp[1] == pytest.approx(4.0, rel=0.4)    # fluctuation ~ dt^2
+    long = oracle.run_npt(eq["r"], eq["v"], m, eq["image"], t, eq["box"], pot, 0.3, 0.004, 6000, T0=T0, tau=0.2, P0=P0,
+                          tauP=tauP, xi=eq["xi"], eta=eq["eta"], nu=eq["nu"])
+    P = long["log"][:, 8]
+    Tk = 2.0 * long["log"][:, 1] / (3.0 * N - 3.0)
+    assert P.mean() == pytest.approx(P0, abs=0.08)
+    assert Tk.mean() == pytest.approx(T0, rel=0.02)
