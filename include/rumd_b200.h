@@ -65,7 +65,12 @@ typedef enum { /* P:73-75 "the cutoff methods: no shift, shifted potential and s
     RUMD_CUT_SHIFTED_POTENTIAL = 1, /* f = f(r),         u = u(r) - u(rc) */
     RUMD_CUT_NONE = 2               /* f = f(r),         u = u(r)  (plain truncation) */
 } rumd_cutoff;
-typedef enum { RUMD_INT_NVE_LEAPFROG = 0, RUMD_INT_NVT_NOSE_HOOVER = 1 } rumd_integrator;
+typedef enum {
+    RUMD_INT_NVE_LEAPFROG = 0,
+    RUMD_INT_NVT_NOSE_HOOVER = 1,
+    RUMD_INT_NPT_MTK = 2 /* P:78 "NPT [51]": isotropic Martyna-Tobias-Klein barostat + the Nose-Hoover thermostat;
+                            target pressure and barostat period from rumd_set_barostat */
+} rumd_integrator;
 typedef enum {
     RUMD_NB_N2 = 0,   /* P:173 "n2": tiled all-pairs list build */
     RUMD_NB_CELL = 1, /* P:276 "sort": spatial sort + cell-list build */
@@ -115,7 +120,8 @@ typedef struct {
  * U, W: sums over particles of u_i, w_i from the LAST force evaluation (O5; P:160 energy halving).
  * K: kinetic energy at the integer time of the last completed step, 1/2 sum m |(v_old+v_new)/2|^2 (O10).
  * mv2: sum m |v(t+dt/2)|^2 after the last step.  xi, eta: Nose-Hoover variables (O7).
- * H: K + U (+ thermostat terms for NVT, O10), valid when at least one step has run. */
+ * H: K + U (+ thermostat terms for NVT, O10; + P0 V + (g + 3) T0 nu^2 / (2 wP^2) for NPT), valid when at least one
+ * step has run. */
 typedef struct {
     double U, W, K, mv2, xi, eta, H;
     long long n_steps;    /* steps completed since rumd_bind_state */
@@ -181,6 +187,20 @@ rumd_status rumd_set_pair_potential(rumd_system* s, int type_i, int type_j, rumd
 /* P:54 `IntegratorNVT(timeStep, targetTemperature)`.  NVE leap-frog (O6) or Nose-Hoover leap-frog
  * (O7) with period tau (tau <= 0 or inf: thermostat off, identical to NVE).  g = 3N - 3 (S10). */
 rumd_status rumd_set_integrator(rumd_system* s, rumd_integrator kind, float dt, float target_T, float tau);
+
+/* NPT ("NPT [51]", Martyna-Tobias-Klein 1994, isotropic; the leap-frog form is DESIGN.md reading S32):
+ *     dr/dt = v + nu r, dL/dt = nu L, dv/dt = F/m - [xi + (1 + 3/g) nu] v,
+ *     dnu/dt = (2 pi / tau_P)^2 / ((g + 3) T0) [ (1 + 3/g) sum m v^2 + W - 3 V P0 ],  W = sum_i w_i.
+ * target_P, tau_P: host scalars; tau_P <= 0 or inf freezes the strain rate (with nu = 0 that is NVT).  Takes effect
+ * with rumd_set_integrator(s, RUMD_INT_NPT_MTK, dt, target_T, tau).  NPT runs on the per-step kernels (the tuning's
+ * `persistent` is ignored) with method RUMD_NB_N2 or RUMD_NB_NONE (the cell grid is sized for a fixed box:
+ * RUMD_ERR_INVALID_ARG otherwise) and a single system (no replicas); rumd_autotune is not available.  The box is then
+ * a device quantity: it starts as the box of rumd_create at every reset (bind, upload) and is read with rumd_get_box.
+ * If the box shrinks below 2 (rc_max + skin) the run stops being valid: RUMD_ERR_BOX_TOO_SMALL from rumd_get_thermo. */
+rumd_status rumd_set_barostat(rumd_system* s, float target_P, float tau_P);
+/* Current box lengths and strain rate (host outputs; box_out: 3 doubles; nu_out may be NULL).  For NVE / NVT the
+ * box of rumd_create and 0.  Synchronizes. */
+rumd_status rumd_get_box(rumd_system* s, double* box_out, double* nu_out);
 
 /* Launch parameters.  rumd_default_tuning fills the library's untuned defaults for this N. */
 rumd_status rumd_default_tuning(const rumd_system* s, rumd_tuning* out);

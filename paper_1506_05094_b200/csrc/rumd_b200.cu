@@ -5,6 +5,7 @@
 #include "rumd_dispatch.cuh"
 #include "rumd_persist.cuh"
 #include "rumd_ensemble.cuh"
+#include "rumd_npt.cuh"
 
 #include <algorithm>
 #include <cmath>
@@ -43,6 +44,7 @@ struct rumd_system {
     bool any_coul = false, any_generic = false; // a second term is set / one of them is not Coulomb
     int integ = 0;
     float dt = 0, T0 = 0, tau = 0;
+    float P0 = 0, tauP = 0; // NPT: target pressure, barostat period
     rumd_tuning tune;
     int cap = 0;
     size_t nc_carved = 0;   // cells the bound workspace was carved (and its histogram zeroed) for
@@ -225,7 +227,10 @@ extern "C" rumd_status rumd_create(rumd_system** out, int n_particles, int n_typ
         }
         s->own_stream = true;
     }
-    for (int k = 0; k < 3; ++k) s->box[k] = box_lengths[k];
+    for (int k = 0; k < 3; ++k) {
+        s->box[k] = box_lengths[k];
+        s->S.L[k] = box_lengths[k]; // (k_reset_scalars seeds the device box from it, before the first refresh)
+    }
     if (cudaMallocHost((void**)&s->h_thermo, sizeof(rumd_thermo)) != cudaSuccess ||
         cudaMallocHost((void**)&s->h_sc, sizeof(DevScalars)) != cudaSuccess) {
         delete s;
@@ -409,14 +414,25 @@ extern "C" rumd_status rumd_set_pair_potential(rumd_system* s, int ti, int tj, r
 extern "C" rumd_status rumd_set_integrator(rumd_system* s, rumd_integrator kind, float dt, float T, float tau)
 {
     if (!s) return RUMD_ERR_INVALID_ARG;
-    if (kind != RUMD_INT_NVE_LEAPFROG && kind != RUMD_INT_NVT_NOSE_HOOVER) return fail(s, RUMD_ERR_INVALID_ARG, "unknown integrator");
+    if (kind != RUMD_INT_NVE_LEAPFROG && kind != RUMD_INT_NVT_NOSE_HOOVER && kind != RUMD_INT_NPT_MTK)
+        return fail(s, RUMD_ERR_INVALID_ARG, "unknown integrator");
     if (!(dt > 0.f) || !std::isfinite(dt)) return fail(s, RUMD_ERR_INVALID_ARG, "dt must be > 0");
-    if (kind == RUMD_INT_NVT_NOSE_HOOVER && !(T > 0.f)) return fail(s, RUMD_ERR_INVALID_ARG, "target temperature must be > 0");
+    if (kind != RUMD_INT_NVE_LEAPFROG && !(T > 0.f)) return fail(s, RUMD_ERR_INVALID_ARG, "target temperature must be > 0");
     s->integ = (int)kind;
     s->dt = dt;
     s->T0 = T;
     s->tau = tau;
     s->integ_set = true;
+    s->params_dirty = true;
+    return RUMD_OK;
+}
+
+extern "C" rumd_status rumd_set_barostat(rumd_system* s, float target_P, float tau_P)
+{
+    if (!s) return RUMD_ERR_INVALID_ARG;
+    if (!std::isfinite(target_P)) return fail(s, RUMD_ERR_INVALID_ARG, "target pressure must be finite");
+    s->P0 = target_P;
+    s->tauP = tau_P;
     s->params_dirty = true;
     return RUMD_OK;
 }
@@ -509,6 +525,20 @@ static rumd_status refresh(rumd_system* s)
     S.omega2 = (tau > 0 && std::isfinite(tau)) ? (2.0 * M_PI / tau) * (2.0 * M_PI / tau) : 0.0;
     S.sort_interval = t.sort_interval;
     S.method = t.method;
+    S.npt = s->integ == RUMD_INT_NPT_MTK;
+    S.P0 = s->P0;
+    S.cP = 0.0;
+    S.rc_margin = (float)(rcm + 2.0 * skin + 1e-3);
+    S.rcl_max = (float)(rcm + skin);
+    S.skin = (float)skin;
+    if (S.npt) {
+        if (t.method != RUMD_NB_N2 && t.method != RUMD_NB_NONE)
+            return fail(s, RUMD_ERR_INVALID_ARG, "NPT needs the n2 or the none method (the cell grid is sized for a fixed box)");
+        if (s->nrep > 1) return fail(s, RUMD_ERR_INVALID_ARG, "NPT is not available for a batched ensemble");
+        const double tp = s->tauP;
+        if (tp > 0 && std::isfinite(tp)) S.cP = (2.0 * M_PI / tp) * (2.0 * M_PI / tp) / ((S.g + 3.0) * S.T0);
+        S.half_skin2 = (float)(0.16 * skin * skin); // 0.4 skin: 0.1 skin is kept for the change of the box (rumd_npt.cuh)
+    }
     S.r_out = S.r;
     {   // lanes per particle of the cell build: several while the machine is not full, one at large N (measured)
         const int btp = t.build_tp > 0 ? t.build_tp : s->N <= 32768 ? 8 : 1;
@@ -750,8 +780,23 @@ static const KernelSet* kernels_of(const rumd_system* s)
 static int coul_of(const rumd_system* s) { return s->any_coul ? (s->any_generic ? 2 : 1) : 0; }
 static bool one_of(const rumd_system* s) { return s->ntypes == 1; }
 
+template <int COUL> static void launch_force_npt(rumd_system* s, int nb)
+{
+    if (s->ntypes == 1) k_force_npt<COUL, true><<<nb, 256, 0, s->stream>>>(s->S);
+    else k_force_npt<COUL, false><<<nb, 256, 0, s->stream>>>(s->S);
+}
+
 static int launch_force(rumd_system* s)
 {
+    if (s->S.npt) { // box from device memory, energy and virial every step (rumd_npt.cuh)
+        const int nb = (int)(((long long)s->N * NPT_TP + 255) / 256);
+        switch ((s->any_coul ? (s->any_generic ? 2 : 1) : 0)) {
+        case 0: launch_force_npt<0>(s, nb); break;
+        case 1: launch_force_npt<1>(s, nb); break;
+        default: launch_force_npt<2>(s, nb); break;
+        }
+        return 1;
+    }
     if (s->tune.method == RUMD_NB_TILE) { // one block per tile, halo in shared memory
         kernels_of(s)->force_tile(coul_of(s), one_of(s), s->S, s->S.ntiles, tile_smem_bytes_force(s->S.hcap), s->stream);
         return 1;
@@ -828,7 +873,9 @@ static int launch_rebuild_chain(rumd_system* s)
         k_permute_store<<<nbp, 256, 0, s->stream>>>(S);
         n += 3;
     }
-    if (s->tune.method == RUMD_NB_TILE)
+    if (s->S.npt)
+        k_build_n2_npt<<<std::min((s->N + 3) / 4, cap128), 128, 0, s->stream>>>(S);
+    else if (s->tune.method == RUMD_NB_TILE)
         k_build_tile<<<std::min(S.ntiles, cap256), TILE_THREADS, tile_smem_bytes(S.hcap), s->stream>>>(S);
     else if (s->tune.method == RUMD_NB_CELL) {
         const long long threads = (long long)s->N << S.build_tp_shift;
@@ -840,6 +887,11 @@ static int launch_rebuild_chain(rumd_system* s)
 
 static int launch_integrate(rumd_system* s)
 {
+    if (s->S.npt) {
+        k_npt_prepare<<<1, 1024, 0, s->stream>>>(s->S);
+        k_integrate_npt<<<s->int_blocks, INT_THREADS, 0, s->stream>>>(s->S);
+        return 2;
+    }
     k_integrate<<<s->int_blocks, INT_THREADS, 0, s->stream>>>(s->S, s->integ == RUMD_INT_NVT_NOSE_HOOVER);
     return 1;
 }
@@ -925,7 +977,7 @@ static rumd_status get_graph(rumd_system* s, GraphCache& gc, int steps, int* ker
     cudaGraph_t g = nullptr;
     CUDA_TRY(s, cudaStreamBeginCapture(s->stream, cudaStreamCaptureModeThreadLocal));
     int n = 0;
-    if (steps % 2 == 0 && s->tune.method != RUMD_NB_TILE) // (the tile method has no fused per-step kernel)
+    if (steps % 2 == 0 && s->tune.method != RUMD_NB_TILE && !s->S.npt) // (tile method, NPT: no fused per-step kernel)
         for (int q = 0; q < steps; q += 2) n += launch_step_pair(s, q + 2 == steps);
     else
         for (int q = 0; q < steps; ++q) n += launch_step(s);
@@ -958,7 +1010,7 @@ extern "C" rumd_status rumd_run_steps(rumd_system* s, long n)
         }
         return RUMD_OK;
     }
-    if (s->tune.persistent) {
+    if (s->tune.persistent && !s->S.npt) { // (NPT runs on the per-step kernels, rumd_npt.cuh)
         // one cooperative launch per <= 2^16 steps (keeps the 32-bit arrival count of the grid barrier in range)
         for (long left = n; left > 0;) {
             const int chunk = (int)std::min<long>(left, 1L << 16);
@@ -1033,11 +1085,15 @@ extern "C" rumd_status rumd_get_thermo(rumd_system* s, rumd_thermo* out)
     out->xi = d.xi;
     out->eta = d.eta;
     double H = d.K + d.U;
-    if (s->integ == RUMD_INT_NVT_NOSE_HOOVER) { // O10
+    if (s->integ != RUMD_INT_NVE_LEAPFROG) { // O10
         // K and U belong to time t of the last step; xi, eta are already at t + dt, so H(t) uses the
         // values step_tail kept for time t (xi_t, eta_t).
         H += s->S.g * s->S.T0 * d.eta_t;
         if (s->S.omega2 > 0) H += 0.5 * s->S.g * s->S.T0 * d.xi_t * d.xi_t / s->S.omega2;
+    }
+    if (s->integ == RUMD_INT_NPT_MTK) { // reading S32: + P0 V(t) + Wb nu(t)^2 / 2, Wb = (g + 3) T0 / wP^2 = 1 / cP
+        H += s->S.P0 * d.vol_t;
+        if (s->S.cP > 0) H += 0.5 * d.nu_t * d.nu_t / s->S.cP;
     }
     out->H = H;
     out->n_steps = d.n_steps;
@@ -1054,6 +1110,7 @@ extern "C" rumd_status rumd_get_thermo(rumd_system* s, rumd_thermo* out)
         return fail(s, RUMD_ERR_NBL_OVERFLOW, "tile method: a tile's halo holds more than %d particles (density far from uniform): use a smaller tile or the cell method", s->S.hcap);
     if (d.overflow) return fail(s, RUMD_ERR_NBL_OVERFLOW, "neighbour list overflow: %d neighbours > capacity %d", max_nbrs, s->S.cap);
     if (d.nonfinite == 2) return fail(s, RUMD_ERR_CUDA, "persistent kernel: grid barrier timed out");
+    if (d.nonfinite == 3) return fail(s, RUMD_ERR_BOX_TOO_SMALL, "NPT: the box shrank below 2 (rc_max + skin)");
     if (d.nonfinite) return fail(s, RUMD_ERR_NONFINITE, "non-finite energy");
     return RUMD_OK;
 }
@@ -1094,6 +1151,20 @@ extern "C" rumd_status rumd_get_thermo_replicas(rumd_system* s, rumd_thermo* out
         else if (d.nonfinite && worst == RUMD_OK) worst = fail(s, RUMD_ERR_NONFINITE, "non-finite energy in replica %d", q);
     }
     return worst;
+}
+
+extern "C" rumd_status rumd_get_box(rumd_system* s, double* box_out, double* nu_out)
+{
+    SINGLE_ONLY(s);
+    rumd_status st = ready(s, false);
+    if (st != RUMD_OK) return st;
+    if (!box_out) return fail(s, RUMD_ERR_INVALID_ARG, "null output");
+    CUDA_TRY(s, cudaMemcpyAsync(s->h_sc, s->S.sc, sizeof(DevScalars), cudaMemcpyDeviceToHost, s->stream));
+    CUDA_TRY(s, cudaStreamSynchronize(s->stream));
+    const bool npt = s->integ == RUMD_INT_NPT_MTK;
+    for (int k = 0; k < 3; ++k) box_out[k] = npt ? s->h_sc->box[k] : (double)s->box[k];
+    if (nu_out) *nu_out = npt ? s->h_sc->nu_o : 0.0;
+    return RUMD_OK;
 }
 
 extern "C" rumd_status rumd_snapshot(rumd_system* s)
@@ -1386,6 +1457,7 @@ extern "C" rumd_status rumd_autotune(rumd_system* s, rumd_tuning* out, int steps
     SINGLE_ONLY(s);
     rumd_status st = ready(s, true);
     if (st != RUMD_OK) return st;
+    if (s->integ == RUMD_INT_NPT_MTK) return fail(s, RUMD_ERR_INVALID_ARG, "autotune is not available for NPT (per-step kernels, n2 / none only)");
     if (steps_per_trial < 8) steps_per_trial = 8;
     const rumd_tuning saved = s->tune;
     st = rumd_snapshot(s);

@@ -466,7 +466,18 @@ __device__ __forceinline__ void step_tail(const Sys& S, bool nvt, double kt, dou
             sc->xi = xin;
         }
         sc->n_steps += 1;
-        const unsigned pend = *((volatile unsigned*)&sc->pending);
+        unsigned pend = *((volatile unsigned*)&sc->pending);
+        if (S.npt) { // rumd_npt.cuh: the kinetic kick of the strain rate, the new box, and the guards that go with it
+            sc->nu_o += S.dt_d * S.cP * (1.0 + 3.0 / S.g) * b;
+            double lmin = sc->box_next[0];
+            for (int k = 0; k < 3; ++k) {
+                // the list tolerates 0.1 skin of box change since its build (the displacement test uses 0.4 skin)
+                if (fabs(sc->box_next[k] / sc->box_build[k] - 1.0) * (double)S.rcl_max > 0.1 * (double)S.skin) pend = 1u;
+                sc->box[k] = sc->box_next[k];
+                lmin = fmin(lmin, sc->box_next[k]);
+            }
+            if ((double)S.rcl_max > 0.5 * lmin) sc->nonfinite = 3; // the box shrank below 2 (rc_max + skin), O1
+        }
         sc->flag = pend;
         sc->pending = 0u;
         sc->ticket = 0u;
@@ -554,6 +565,7 @@ static __global__ void k_reset_scalars(const Sys S)
     DevScalars z;
     memset(&z, 0, sizeof(z));
     z.flag = 1u;
+    for (int k = 0; k < 3; ++k) z.box[k] = z.box_next[k] = z.box_build[k] = (double)S.L[k];
     *S.sc = z;
 }
 

@@ -124,6 +124,36 @@ __device__ __forceinline__ int tile_cell_key(const Sys& S, int cx, int cy, int c
 // warp boundary: particle i of tile t (own range starting at o0) has row index pbase(t) + (i - o0).
 __device__ __forceinline__ int tile_pbase(int o0, int t) { return ((o0 + 31) & ~31) + 32 * t; }
 
+// Box lengths as a kernel sees them.  NVE / NVT: the constants of the parameter block.  NPT: the box is a device
+// quantity that changes every step (DevScalars::box, rumd_npt.cuh).
+struct Box {
+    float L[3], h[3], invL[3];
+};
+
+__device__ __forceinline__ Box box_of_sys(const Sys& S)
+{
+    Box b;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        b.L[k] = S.L[k];
+        b.h[k] = S.h[k];
+        b.invL[k] = S.invL[k];
+    }
+    return b;
+}
+
+__device__ __forceinline__ Box box_of_doubles(const double* L)
+{
+    Box b;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        b.L[k] = (float)L[k];
+        b.h[k] = 0.5f * b.L[k];
+        b.invL[k] = (float)(1.0 / L[k]);
+    }
+    return b;
+}
+
 // ------------------------------------------------------------------------------------------ A2: N^2 build
 
 // P:173-224 Fig. 4.  One WARP per particle i; j-positions staged through shared memory in tiles
@@ -133,8 +163,9 @@ __device__ __forceinline__ int tile_pbase(int o0, int t) { return ((o0 + 31) & ~
 // and the overflow flag.  Block-cooperative: `blk`/`nblk` = this block's index / block count
 // in the virtual grid; blockDim.x must be a multiple of 32.  max_slot: &sc->max_nbrs[build & 1].
 #define N2_TILE 256
+template <bool NPT = false>
 __device__ __forceinline__ void ph_build_n2(const Sys& S, const float4* r, float4* tile, const float* s_rcl2,
-                                            int blk, int nblk, int* max_slot)
+                                            int blk, int nblk, int* max_slot, const Box* bx = nullptr)
 {
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
     const int ngroups = (S.N + nw - 1) / nw;
@@ -156,7 +187,15 @@ __device__ __forceinline__ void ph_build_n2(const Sys& S, const float4* r, float
                 const int j = j0 + jj;
                 if (jj < jend && have_i && j != i) {
                     const float4 rj = tile[jj];
-                    acc = list_dist2(S, ri, rj) < s_rcl2[trow + type_of(rj)]; // strict <, per type pair
+                    float d2;
+                    if (NPT) { // box read from device memory by the caller
+                        const float dx = min_image(ri.x, rj.x, bx->h[0], bx->invL[0]);
+                        const float dy = min_image(ri.y, rj.y, bx->h[1], bx->invL[1]);
+                        const float dz = min_image(ri.z, rj.z, bx->h[2], bx->invL[2]);
+                        d2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, dx * dx));
+                    } else
+                        d2 = list_dist2(S, ri, rj);
+                    acc = d2 < s_rcl2[trow + type_of(rj)]; // strict <, per type pair
                 }
                 const unsigned m = __ballot_sync(FULLMASK, acc);
                 if (acc) {

@@ -42,6 +42,13 @@ struct DevScalars {
     int max_nbrs[2];      // largest list length of build number b in slot b & 1
     int nonfinite;        // 1: NaN/Inf energy; 2: grid barrier timed out
     int last_max;         // largest list length of the last COMPLETED build (written when its force evaluation starts)
+    // NPT (rumd_npt.cuh): the box is a device quantity that changes every step
+    double box[3];        // current box lengths (set from the handle's box at every reset)
+    double box_next[3];   // box after the step in flight (k_npt_prepare -> k_integrate_npt)
+    double box_build[3];  // box at the last list build
+    double nu_o, nu_t;    // strain rate as the last step left it; strain rate at the integer time t of the last step
+    double vol_t;         // volume at the integer time t of the last step
+    double npt_a, npt_b, npt_s, npt_sh; // leap-frog factors of the step in flight
 };
 
 struct CellGrid {
@@ -60,6 +67,11 @@ struct Sys {
     float dt, half_skin2;   // (skin/2)^2
     double dt_d, T0, omega2, g;
     int sort_interval, method;
+    int npt;                // 1: NPT integrator, box lengths live in DevScalars
+    double P0, cP;          // NPT: target pressure; wP^2 / ((g + 3) T0)
+    float rc_margin;        // rc_max + 2 skin + 1e-3 (hin = L/2 - rc_margin); rc_max + skin in rcl_max
+    float rcl_max;
+    float skin;
     CellGrid grid;
     // caller-owned state
     float4* r; float4* v; float4* f; float* w; int4* image; int* id;

@@ -21,12 +21,12 @@ POT_LJ_12_6, POT_COULOMB, POT_IPL, POT_YUKAWA, POT_GAUSSIAN_CORE, POT_BUCKINGHAM
 POT_GEN_LJ, POT_GIRIFALCO, POT_DZUGUTOV = 6, 7, 8
 _SECOND_NPARAMS = (1, 2, 2, 2, 3, 4, 3, 2)  # of (a, b, c, d), by kind - 1; rcut follows
 CUT_SHIFTED_FORCE, CUT_SHIFTED_POTENTIAL, CUT_NONE = 0, 1, 2
-INT_NVE_LEAPFROG, INT_NVT_NOSE_HOOVER = 0, 1
+INT_NVE_LEAPFROG, INT_NVT_NOSE_HOOVER, INT_NPT_MTK = 0, 1, 2
 NB_N2, NB_CELL, NB_NONE, NB_TILE = 0, 1, 2, 3
 
 EXPORTS = [
     "rumd_create", "rumd_destroy", "rumd_bind_state", "rumd_workspace_bytes", "rumd_bind_workspace",
-    "rumd_set_pair_potential", "rumd_set_integrator", "rumd_default_tuning", "rumd_set_tuning",
+    "rumd_set_pair_potential", "rumd_set_integrator", "rumd_set_barostat", "rumd_get_box", "rumd_default_tuning", "rumd_set_tuning",
     "rumd_get_tuning", "rumd_autotune", "rumd_autotune_cached", "rumd_build_nblist", "rumd_compute_forces", "rumd_run_steps",
     "rumd_export_nblist", "rumd_get_thermo", "rumd_snapshot", "rumd_restore", "rumd_upload_state",
     "rumd_download_state", "rumd_launch_count", "rumd_profile_step", "rumd_time_force", "rumd_profile_persistent", "rumd_measure_fp32_peak", "rumd_set_replicas", "rumd_get_thermo_replicas", "rumd_last_error", "rumd_version",
@@ -78,6 +78,8 @@ def lib():
         L.rumd_bind_workspace.argtypes = [vp, vp, C.c_size_t, ip]
         L.rumd_set_pair_potential.argtypes = [vp, ip, ip, ip, ip, C.POINTER(C.c_float), ip]
         L.rumd_set_integrator.argtypes = [vp, ip, C.c_float, C.c_float, C.c_float]
+        L.rumd_set_barostat.argtypes = [vp, C.c_float, C.c_float]
+        L.rumd_get_box.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.rumd_default_tuning.argtypes = [vp, C.POINTER(Tuning)]
         L.rumd_set_tuning.argtypes = [vp, C.POINTER(Tuning)]
         L.rumd_get_tuning.argtypes = [vp, C.POINTER(Tuning)]
@@ -224,6 +226,16 @@ class System:
 
     def set_integrator(self, kind, dt, T0=1.0, tau=0.2):
         self._check(self.L.rumd_set_integrator(self.h, int(kind), float(dt), float(T0), float(tau)))
+
+    def set_barostat(self, P0, tauP):
+        self._check(self.L.rumd_set_barostat(self.h, float(P0), float(tauP)))
+
+    def get_box(self):
+        """-> (box lengths (3,) float64, strain rate): the current box of an NPT run."""
+        box = (C.c_double * 3)()
+        nu = C.c_double()
+        self._check(self.L.rumd_get_box(self.h, box, C.byref(nu)))
+        return np.array(list(box)), float(nu.value)
 
     def default_tuning(self) -> Tuning:
         t = Tuning()

@@ -1274,3 +1274,146 @@ def test_tile_method_refuses_what_it_cannot_do(rumd):
         s.compute_forces()
     assert e.value.status == rumd.ERR_BOX_TOO_SMALL
     s.close()
+
+
+# ------------------------------------------------------------------ NPT ("NPT [51]"; reading S32)
+
+
+def _npt_system(rumd, N=1000, tp=8, method=None, P0=2.0, tauP=2.0, T0=2.0, density=0.5, seed=5):
+    ncell = {500: 5, 864: 6, 2048: 8}.get(N)
+    if ncell:
+        r, box = W.fcc_lattice(ncell, ncell, ncell, density)
+    else:
+        n = round(N ** (1.0 / 3.0))
+        r, box, _ = W.sc_lattice(n, n, n, density)
+    N = r.shape[0]
+    rng = np.random.default_rng(seed)
+    m = np.ones(N)
+    v = W.maxwell_boltzmann(rng, m, T0)
+    wl = W.Workload(name="npt", r=W._fold32(r, box), v=v.astype(np.float32), m=m.astype(np.float32),
+                    types=np.zeros(N, np.int32), box=box.astype(np.float32), pot=W.lj_single(), skin=W.f32(0.3),
+                    dt=W.f32(0.004), integrator=rumd.INT_NPT_MTK, T0=W.f32(T0), tau=W.f32(0.2))
+    wl.r = W.perturb(wl.r, wl.box, 0.05, 3)
+    s = rumd.System(wl.r, wl.v, wl.m, wl.types, wl.box, wl.pot)
+    s.set_barostat(P0, tauP)
+    s.set_integrator(rumd.INT_NPT_MTK, wl.dt, wl.T0, wl.tau)
+    s.set_tuning(method=rumd.NB_N2 if method is None else method, tp=tp, pb=256 // tp, skin=float(wl.skin), persistent=0,
+                 use_graph=0)
+    return s, wl
+
+
+@pytest.mark.parametrize("N,method,use_graph", [(500, 0, 0), (1000, 0, 1), (864, 2, 0)])
+def test_npt_steps_match_oracle(rumd, N, method, use_graph):
+    """NPT (Martyna-Tobias-Klein barostat + Nose-Hoover thermostat, reading S32) on the per-step kernels against the
+    oracle from identical inputs: after 1 step positions, velocities, box, thermostat and strain rate; after 25 more
+    the box, nu, xi, U, K, H still track (before chaos separates the trajectories)."""
+    s, wl = _npt_system(rumd, N=N, method=method)
+    s.set_tuning(use_graph=use_graph, steps_per_graph=4)
+    P0, tauP = 2.0, 2.0
+    N = wl.N
+    r64, v64, m64 = wl.r.astype(np.float64), wl.v.astype(np.float64), wl.m.astype(np.float64)
+    box = wl.box.astype(np.float64)
+    args = dict(T0=float(wl.T0), tau=float(wl.tau), P0=P0, tauP=tauP)
+    o = oracle.run_npt(r64, v64, m64, np.zeros((N, 3), np.int32), wl.types, box, wl.pot, 0.3, float(wl.dt), 1, **args)
+    s.run_steps(1)
+    th = s.get_thermo()
+    st = s.state()
+    gbox, gnu = s.get_box()
+    assert np.allclose(gbox, o["box"], rtol=1e-7)
+    # nu = dt cP [ (1 + 3/g) sum m v^2 + W - 3 V P0 ]: the three terms nearly cancel, so the 1e-5 relative accuracy of
+    # the fp32 virial sum W (north_star) is the scale of the tolerance, not nu itself
+    g = 3.0 * N - 3.0
+    cP = (2.0 * np.pi / tauP) ** 2 / ((g + 3.0) * float(wl.T0))
+    # (in this fluid the per-particle virials w_i have both signs and W = sum w_i nearly cancels: as for U on the KA
+    # lattice start, DESIGN.md S29, the scale of the fp32 sum's 1e-5 is sum |w_i|)
+    w_scale = np.abs(oracle.forces_allpairs(r64, wl.types, box, wl.pot)[2]).sum()
+    nu_tol = float(wl.dt) * cP * ENERGY_TOL * w_scale
+    assert gnu == pytest.approx(o["nu"], abs=nu_tol)
+    d = st["r"].astype(np.float64) + st["image"] * gbox - (o["r"] + o["image"] * o["box"])
+    assert np.abs(d).max() < 3e-6
+    assert np.abs(st["v"] - o["v"]).max() < 1e-5 * max(1.0, np.abs(o["v"]).max())
+    assert th["U"] == pytest.approx(o["log"][0, 0], rel=ENERGY_TOL)
+    assert abs(th["W"] - o["log"][0, 2]) <= ENERGY_TOL * w_scale
+    assert th["K"] == pytest.approx(o["log"][0, 1], rel=ENERGY_TOL)
+    assert th["H"] == pytest.approx(o["log"][0, 5], rel=ENERGY_TOL)
+    # xi = dt w^2 (T_kin / T0 - 1) with T_kin within 1e-3 of T0 here: the fp32 velocities' 1e-7 sets the absolute scale
+    assert th["xi"] == pytest.approx(o["xi"], rel=1e-4, abs=float(wl.dt) * (2.0 * np.pi / float(wl.tau)) ** 2 * 3e-7)
+    # 25 more steps
+    o2 = oracle.run_npt(r64, v64, m64, np.zeros((N, 3), np.int32), wl.types, box, wl.pot, 0.3, float(wl.dt), 26, **args)
+    s.run_steps(25)
+    th = s.get_thermo()
+    gbox, gnu = s.get_box()
+    assert np.allclose(gbox, o2["box"], rtol=1e-6)
+    assert gnu == pytest.approx(o2["nu"], rel=1e-3, abs=30.0 * nu_tol)
+    assert th["xi"] == pytest.approx(o2["xi"], rel=1e-3, abs=1e-6)
+    assert th["U"] == pytest.approx(o2["log"][-1, 0], rel=1e-4)
+    assert th["K"] == pytest.approx(o2["log"][-1, 1], rel=1e-4)
+    assert th["H"] == pytest.approx(o2["log"][-1, 5], rel=1e-4)
+    assert th["n_steps"] == 26
+    # forces of the configuration the GPU now holds, in ITS box
+    s.compute_forces()
+    st = s.state()
+    F, u, w = oracle.forces_allpairs(st["r"].astype(np.float64), wl.types, gbox, wl.pot)
+    rms = np.sqrt((F * F).sum(1).mean())
+    assert np.sqrt(((st["F"] - F) ** 2).sum(1)).max() <= FORCE_TOL * rms
+    s.close()
+
+
+def test_npt_with_the_barostat_off_equals_the_nvt_kernels_bitwise(rumd):
+    """tau_P = 0 freezes the strain rate at 0: every factor of the NPT step reduces to the NVT step (reading S32), and
+    with 8 lanes per particle both paths add the pair forces in the same order -> bit-identical while the two lists
+    are the same (the NPT list is rebuilt at 0.4 skin instead of skin/2, so only up to the first rebuild)."""
+    s, wl = _npt_system(rumd, N=1000, tauP=0.0)
+    s.run_steps(6)
+    a, ta = s.state(), s.get_thermo()
+    s.close()
+    s2 = rumd.System(wl.r, wl.v, wl.m, wl.types, wl.box, wl.pot)
+    s2.set_integrator(rumd.INT_NVT_NOSE_HOOVER, wl.dt, wl.T0, wl.tau)
+    s2.set_tuning(method=rumd.NB_N2, tp=8, pb=32, skin=float(wl.skin), persistent=0, use_graph=0)
+    s2.run_steps(6)
+    b, tb = s2.state(), s2.get_thermo()
+    s2.close()
+    assert ta["n_rebuilds"] == tb["n_rebuilds"] == 1
+    for key in ("r", "v", "image"):
+        assert np.array_equal(a[key], b[key]), key
+    assert ta["xi"] == tb["xi"] and ta["K"] == pytest.approx(tb["K"], rel=1e-12)
+
+
+def test_npt_reaches_the_target_pressure_and_conserves_its_invariant(rumd):
+    """LJ fluid started well below the target pressure: the box shrinks, <P> settles at P0, <T_kin> at T0, and the
+    conserved quantity of the extended system does not drift (slope of H/N over 1e4 steps <= 1e-3; fp32 positions
+    and forces, no 1e-4 bar is claimed for NPT: the paper only requires NVE to be drift-free-ish)."""
+    s, wl = _npt_system(rumd, N=2048, density=0.5, P0=2.0, tauP=2.0)
+    N = wl.N
+    V0 = float(np.prod(wl.box.astype(np.float64)))
+    s.run_steps(3000)
+    gbox, _ = s.get_box()
+    assert np.prod(gbox) < 0.95 * V0
+    P, T, H = [], [], []
+    for _ in range(100):
+        s.run_steps(100)
+        th = s.get_thermo()
+        gbox, _ = s.get_box()
+        P.append((2.0 * th["K"] + th["W"]) / (3.0 * np.prod(gbox)))
+        T.append(2.0 * th["K"] / (3.0 * N - 3.0))
+        H.append(th["H"] / N)
+    assert np.mean(P) == pytest.approx(2.0, abs=0.1)
+    assert np.mean(T) == pytest.approx(2.0, rel=0.03)
+    slope = np.polyfit(np.arange(100) * 100.0, np.array(H), 1)[0]
+    assert abs(slope * 1e4) <= 1e-3
+    assert s.get_thermo()["n_rebuilds"] > 100
+    s.close()
+
+
+def test_npt_refuses_cell_methods_and_autotune(rumd):
+    s, wl = _npt_system(rumd, N=1000)
+    s.set_tuning(method=rumd.NB_CELL)
+    with pytest.raises(rumd.RumdError) as e:
+        s.run_steps(1)
+    assert e.value.status == rumd.ERR_INVALID_ARG
+    s.set_tuning(method=rumd.NB_N2)
+    with pytest.raises(rumd.RumdError):
+        s.autotune(steps_per_trial=10)
+    s.run_steps(3)
+    assert s.get_thermo()["n_steps"] == 3
+    s.close()
