@@ -236,7 +236,11 @@ def run_gpu(args, rank, world, local_rank):
     inner = args.inner
     equilibrate(s, wl, args.equil)
     tune_info = {}
-    if args.autotune:
+    if args.set_tuning:
+        kv = dict(item.split("=") for item in args.set_tuning.split(","))
+        s.set_tuning(**{k: (float(v) if k == "skin" else int(v)) for k, v in kv.items()})
+        tune_info = {"autotuned": False, "tuning_fixed_by": "--set-tuning " + args.set_tuning}
+    elif args.autotune:
         t, tps = s.autotune(steps_per_trial=args.tune_steps, cache_path=TUNING_CACHE if args.tuning_cache else None)
         tune_info = {"autotuned": True, "tuning_from_cache": bool(s.tuning_from_cache), "trial_tps": tps}
     tun = s.get_tuning().as_dict()
@@ -583,6 +587,8 @@ def main():
     ap.add_argument("--no-tuning-cache", dest="tuning_cache", action="store_false",
                     help="tune from scratch instead of reading / appending paper_1506_05094_b200/tuning_b200.jsonl")
     ap.add_argument("--tune-steps", type=int, default=300)
+    ap.add_argument("--set-tuning", default=None, metavar="K=V,...",
+                    help="fix the headline workload's tuning instead of autotuning it, e.g. method=3,tile=6,tp=1,pb=256,skin=0.25")
     ap.add_argument("--no-cpu-baseline", dest="cpu", action="store_false")
     ap.add_argument("--no-sweep", dest="sweep_default", action="store_false",
                     help="skip the N sweep rows of the default run")
