@@ -138,10 +138,11 @@ __device__ __forceinline__ void pair_accumulate(const float4 pf, const float4 pc
 template <bool NC> __device__ __forceinline__ int load_idx(const int* p) { return NC ? __ldg(p) : __ldcs(p); }
 template <bool NC> __device__ __forceinline__ float4 load_pos(const float4* p) { return NC ? __ldg(p) : *p; }
 
-template <int TP, int COUL, bool ONE_TYPE, int UNROLL, bool NC, bool ENERGY, bool WRAP, bool MASKED>
+// PRE: the index loads of iteration 0 were issued by the caller before it knew the row length (jpre)
+template <int TP, int COUL, bool ONE_TYPE, int UNROLL, bool NC, bool ENERGY, bool WRAP, bool MASKED, bool PRE = false>
 __device__ __forceinline__ void force_loop(const Sys& S, const float4* r, const float4* s_pp, const int* base,
                                            int it_begin, int nit, int it_end, const float4 ri, float& fx, float& fy,
-                                           float& fz, float& u, float& w)
+                                           float& fz, float& u, float& w, const int* jpre = nullptr)
 {
     const int trow = ONE_TYPE ? 0 : 4 * type_of(ri) * S.ntypes;
     float4 pf, pc, pe, px;
@@ -161,7 +162,10 @@ __device__ __forceinline__ void force_loop(const Sys& S, const float4* r, const 
 #pragma unroll
         for (int q = 0; q < UNROLL; ++q) {
             ok[q] = !MASKED || (it + q) < nit;
-            j[q] = ok[q] ? load_idx<NC>(base + (size_t)(it + q) * 32) : 0; // masked lanes gather slot 0 (always valid)
+            if (PRE && it == 0)
+                j[q] = ok[q] ? jpre[q] : 0;
+            else
+                j[q] = ok[q] ? load_idx<NC>(base + (size_t)(it + q) * 32) : 0; // masked lanes gather slot 0 (always valid)
         }
 #pragma unroll
         for (int q = 0; q < UNROLL; ++q) rj[q] = load_pos<NC>(&r[j[q]]);
@@ -195,20 +199,29 @@ __device__ __forceinline__ void force_group(const Sys& S, const float4* r, const
                                             float& fz, float& u, float& w)
 {
     const int lane = threadIdx.x & 31;
+    const int* base = S.nbl + (size_t)vwarp * S.cap_it * 32 + lane;
+    // Small systems (wide lane groups, persistent kernel): a time step is a chain of dependent L2 round trips, so the
+    // first UNROLL list entries of every lane are requested BEFORE the row length is known (the row is allocated up
+    // to the capacity; what lies beyond the length is masked below and never dereferenced).
+    constexpr bool PRE = TP >= 8 && !NC;
+    int jpre[UNROLL];
+    if (PRE) {
+#pragma unroll
+        for (int q = 0; q < UNROLL; ++q) jpre[q] = q < S.cap_it ? load_idx<NC>(base + (size_t)q * 32) : 0;
+    }
     int nit = (cnt - t + TP - 1) / TP; // entries t, t+TP, ... < cnt
     if (nit < 0) nit = 0;
     const int nit_w = __reduce_max_sync(FULLMASK, nit);
-    const int* base = S.nbl + (size_t)vwarp * S.cap_it * 32 + lane;
     fx = fy = fz = u = w = 0.f;
     // iterations every lane of the warp has (no masks needed), then the ragged tail
     const int nit_all = __reduce_min_sync(FULLMASK, have_i ? nit : 0) / UNROLL * UNROLL;
     const bool interior = fabsf(ri.x) < S.hin[0] && fabsf(ri.y) < S.hin[1] && fabsf(ri.z) < S.hin[2];
     if (__any_sync(FULLMASK, have_i && !interior)) {
-        force_loop<TP, COUL, ONE_TYPE, UNROLL, NC, ENERGY, true, false>(S, r, s_pp, base, 0, nit, nit_all, ri, fx, fy, fz, u, w);
-        force_loop<TP, COUL, ONE_TYPE, UNROLL, NC, ENERGY, true, true>(S, r, s_pp, base, nit_all, nit, nit_w, ri, fx, fy, fz, u, w);
+        force_loop<TP, COUL, ONE_TYPE, UNROLL, NC, ENERGY, true, false, PRE>(S, r, s_pp, base, 0, nit, nit_all, ri, fx, fy, fz, u, w, jpre);
+        force_loop<TP, COUL, ONE_TYPE, UNROLL, NC, ENERGY, true, true, PRE>(S, r, s_pp, base, nit_all, nit, nit_w, ri, fx, fy, fz, u, w, jpre);
     } else {
-        force_loop<TP, COUL, ONE_TYPE, UNROLL, NC, ENERGY, false, false>(S, r, s_pp, base, 0, nit, nit_all, ri, fx, fy, fz, u, w);
-        force_loop<TP, COUL, ONE_TYPE, UNROLL, NC, ENERGY, false, true>(S, r, s_pp, base, nit_all, nit, nit_w, ri, fx, fy, fz, u, w);
+        force_loop<TP, COUL, ONE_TYPE, UNROLL, NC, ENERGY, false, false, PRE>(S, r, s_pp, base, 0, nit, nit_all, ri, fx, fy, fz, u, w, jpre);
+        force_loop<TP, COUL, ONE_TYPE, UNROLL, NC, ENERGY, false, true, PRE>(S, r, s_pp, base, nit_all, nit, nit_w, ri, fx, fy, fz, u, w, jpre);
     }
 #pragma unroll
     for (int o = TP / 2; o; o >>= 1) {

@@ -187,10 +187,10 @@ __global__ void __launch_bounds__(PERSIST_THREADS, PERSIST_MINB) k_persist(const
         PROF_LAP(0)
 
         // ---------------------------------------------------------------- Nose-Hoover factors of this step (O7)
-        // Warp 0 of EVERY block adds the previous step's per-block sums of m v^2 in the same fixed order and
+        // One warp of EVERY block adds the previous step's per-block sums of m v^2 in the same fixed order and
         // advances xi identically; the other warps start on the forces and pick the factors up from shared
         // memory only when they integrate.
-        if (nvt && wid == 0) {
+        if (nvt && wid == nw - 1) { // the LAST warp: with fewer virtual warps than warps (small N) it has no force work
             double sm = 0.0;
             if (k > 0) sm = warp_sum_partials(S.partial + (size_t)((k - 1) & 1) * gridDim.x * 2 + 1, gridDim.x);
             if (lane == 0) {
@@ -236,9 +236,8 @@ __global__ void __launch_bounds__(PERSIST_THREADS, PERSIST_MINB) k_persist(const
         };
         if constexpr (TILE) {
             // tile method: the block's tiles in turn -- halo into shared memory, forces of the owned particles out of
-            // it, leap-frog; the tiles are split into gridDim.x contiguous, equally long runs
-            const int t0 = (int)((long long)S.ntiles * blockIdx.x / gridDim.x), t1 = (int)((long long)S.ntiles * (blockIdx.x + 1) / gridDim.x);
-            for (int t = t0; t < t1; ++t) {
+            // it, leap-frog
+            for (int t = blockIdx.x; t < S.ntiles; t += gridDim.x) { // strided: every block gets its share of the (dearer) boundary tiles
                 __syncthreads();
                 tile_load_halo<false>(S, rc, t, s_pos);
                 __syncthreads();
