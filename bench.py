@@ -170,6 +170,7 @@ def count_listed(s):
     none = t.method == rumd.NB_NONE
     if none:
         s.set_tuning(method=rumd.NB_N2)
+    s.build_nblist()          # a fresh list of the current positions (the one in flight is a few steps old)
     s.compute_forces()
     cnt, _ = s.export_nblist()
     if none:
