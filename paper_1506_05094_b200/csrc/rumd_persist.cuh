@@ -87,7 +87,7 @@ __device__ __forceinline__ double warp_sum_partials(const double* p, int n)
 // TILE: the instantiation for the tile method (RUMD_NB_TILE: halo in dynamic shared memory); the other methods share
 // the TILE = false instantiation, whose register budget the tile code must not touch.
 template <int TP, int COUL, bool ONE_TYPE, int UNROLL, bool TILE>
-__global__ void __launch_bounds__(PERSIST_THREADS, PERSIST_MINB) k_persist(const Sys S, const int nsteps, const int nvt)
+__global__ void __launch_bounds__(PERSIST_THREADS, (TP == 8 && !TILE) ? 2 : PERSIST_MINB) k_persist(const Sys S, const int nsteps, const int nvt)
 {
     __shared__ float4 s_pp[4 * RUMD_MAXT * RUMD_MAXT];
     __shared__ float s_rcl2[RUMD_MAXT * RUMD_MAXT];
