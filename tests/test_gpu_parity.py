@@ -1417,3 +1417,47 @@ def test_npt_refuses_cell_methods_and_autotune(rumd):
     s.run_steps(3)
     assert s.get_thermo()["n_steps"] == 3
     s.close()
+
+
+def test_tile_method_ragged_gas_four_types_and_halo_overflow(rumd):
+    """Tile method away from lattices: a jittered gas of N = 4099 particles (not a multiple of anything) of four types
+    with six different pair potentials in an orthorhombic box -- list as a set, forces, a 37-step trajectory against
+    the oracle; then a configuration squeezed into one corner of the box, whose halo cannot fit the shared-memory
+    slots sized for a uniform density: the sticky overflow error must come back, not a wrong list."""
+    nt = 4
+    pot = W.pot_table(nt)
+    for a in range(nt):
+        for b in range(a, nt):
+            W.set_lj(pot, a, b, 1.0 + 0.1 * (a + b), 1.0 - 0.04 * (a + b), 2.5 * (1.0 - 0.04 * (a + b)))
+    box = (15.0, 19.0, 23.0)
+    r, v, m, types, boxf, pot = _gas(4099, nt, box, 4242, pot)
+    s = rumd.System(r, v, m, types, boxf, pot)
+    s.set_integrator(rumd.INT_NVE_LEAPFROG, 0.004)
+    s.set_tuning(method=rumd.NB_TILE, tp=2, pb=128, skin=0.3, tile=3)
+    s.compute_forces()
+    r64, b64 = r.astype(np.float64), boxf.astype(np.float64)
+    check_nblist(s, r64, types, b64, pot, 0.3)
+    F, u, w = oracle.forces_allpairs(r64, types, b64, pot)
+    st = s.state()
+    scale = max(1e-3, np.sqrt((F * F).sum(1).mean()))
+    assert np.sqrt(((st["F"] - F) ** 2).sum(1)).max() <= FORCE_TOL * scale
+    assert np.abs(st["u"] - u).max() <= 1e-5 * max(1.0, np.abs(u).max())
+    s.run_steps(37)
+    th = s.get_thermo()
+    assert th["n_steps"] == 37 and th["overflow"] == 0
+    o = oracle.run(r64, v.astype(np.float64), m.astype(np.float64), np.zeros((4099, 3), np.int32), types, b64, pot, 0.3,
+                   0.004, 37)
+    st = s.state()
+    d = st["r"].astype(np.float64) + st["image"] * b64 - (o["r"] + o["image"] * b64)
+    assert np.abs(d).max() < 2e-4
+    s.close()
+    # everything in one octant: eight times the mean density there
+    rc = (0.5 * r - 0.25 * boxf).astype(np.float32)
+    s = rumd.System(rc, v, m, types, boxf, pot)
+    s.set_integrator(rumd.INT_NVE_LEAPFROG, 0.001)
+    s.set_tuning(method=rumd.NB_TILE, tp=2, pb=128, skin=0.3, tile=3)
+    s.compute_forces()
+    with pytest.raises(rumd.RumdError) as e:
+        s.get_thermo()
+    assert e.value.status == rumd.ERR_NBL_OVERFLOW
+    s.close()
