@@ -362,8 +362,22 @@ def run_gpu(args, rank, world, local_rank):
         out["_eq_state"] = (eq_state, eq_thermo)
         out["_headline_row"] = sweep_row(args.workload, N, tps, ms / tsteps, tun, rl, th1["n_rebuilds"] - th0["n_rebuilds"],
                                          tsteps, tune_info)
+        if tun["persistent"]:
+            add_phases(out["_headline_row"], phases, rl, peaks, args.phases)
     s.close()
     return out
+
+
+def add_phases(row, phases, rl, peaks, keep_all):
+    """In-kernel phase timers of k_persist (block 0's SM-cycle counters, rumd_profile_persistent), per time step: the
+    force + integrate phase is the production path's pair-force work (no energies, warm L2, no launch), so its
+    fraction of the FP32 peak is reported beside the stand-alone kernel's."""
+    us = phases["force_integrate_us"]
+    ach = rl["flop_per_listed_pair"] * rl["listed_pairs"] / (us * 1e-6) / 1e12
+    row.update({"force_phase_us": us, "force_phase_frac_fp32": ach / fp32_peak_tflops(peaks["sm_max_mhz"]),
+                "rebuild_us_per_timestep": phases["rebuild_us"], "barrier_us_per_timestep": phases["barrier_us"]})
+    if keep_all:
+        row["phases_us_per_timestep"] = phases
 
 
 def sweep_row(name, N, tps, ms_per_timestep, tun, rl, rebuilds, tsteps, info):
@@ -425,8 +439,8 @@ def run_sweep(args, names, fp32_measured):
         tun = s.get_tuning().as_dict()
         rl = roofline_of(s, wl, name, tun, ms / (reps * inner), inner, peaks, fp32_measured, peaks["sm_max_mhz"])
         row = sweep_row(name, N, tps, ms / (reps * inner), tun, rl, th1["n_rebuilds"] - th0["n_rebuilds"], reps * inner, info)
-        if tun["persistent"] and args.phases:
-            row["phases_us_per_timestep"] = s.profile_persistent(inner)
+        if tun["persistent"]:
+            add_phases(row, s.profile_persistent(inner), rl, peaks, args.phases)
         row["wall_s"] = time.perf_counter() - t_row
         out.append(row)
         print("sweep %s: %.0f timesteps/s, k_force %.1f us = %.3f of FP32" % (name, tps, row["k_force_us"],
