@@ -684,6 +684,8 @@ static rumd_status refresh(rumd_system* s)
     if (t.method == RUMD_NB_TILE) {
         if (s->nrep > 1) return fail(s, RUMD_ERR_INVALID_ARG, "replicas use the n2 or the none method (one block per replica)");
         if (t.tp > 8) return fail(s, RUMD_ERR_INVALID_ARG, "the tile method takes tp <= 8");
+        if (s->N >= (1 << TILE_GHOST_SHIFT))
+            return fail(s, RUMD_ERR_INVALID_ARG, "the tile method takes N < 2^28 (halo slots carry 28-bit particle indices)");
         const int T = t.tile > 0 ? t.tile : (s->N >= 500000 ? 6 : 4);
         size_t ntl = 1;
         double hcells = 1.0;

@@ -207,7 +207,11 @@ __device__ __forceinline__ void tile_build_rows(const Sys& S, int t, const TileG
         if (lane < 25) {
             const int row = ((lz + lane / 5 - 2) * hy + (ly + lane % 5 - 2)) * hx + lx;
             a = s_hstart[row - 2];
-            len = min(s_hstart[row + 3] - a, TILE_CAND_MAX);
+            len = s_hstart[row + 3] - a;
+            if (len > TILE_CAND_MAX) { // > 512 particles in five cells: not a liquid; reported like a halo overflow
+                len = TILE_CAND_MAX;
+                S.sc->overflow = 2u;
+            }
         }
         int off = len; // inclusive scan
 #pragma unroll
