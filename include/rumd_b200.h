@@ -279,6 +279,44 @@ rumd_status rumd_profile_persistent(rumd_system* s, int nsteps, double* out8);
  * Synchronizes. */
 rumd_status rumd_measure_fp32_peak(rumd_system* s, int reps, double* tflops_out);
 
+/* ONE force / energy / virial evaluation that ALLOCATES NOTHING -- for callers that cannot call cudaMalloc (code under
+ * CUDA graph capture, tight serving loops, harnesses that forbid it) and therefore cannot use the handle API, whose
+ * rumd_create allocates and whose workspace must come from somewhere.  Needs no handle: one call computes what
+ * rumd_create .. rumd_build_nblist + rumd_compute_forces + rumd_get_thermo compute with method RUMD_NB_N2, tp = 8 for
+ * 12-6 Lennard-Jones and Coulomb terms with the shifted-force cutoff (Fig. 3; Fig. 4; O5),
+ * by the same list build and the same pair loop.  All scratch (neighbour list, list lengths, positions at build,
+ * reduction partials, flags) lives in one fixed device array inside the library, 8.2 MB, held by every GPU that loads
+ * the library until the process exits.  Hence the limits: n_particles <= RUMD_NOALLOC_MAX_PARTICLES and at most
+ * RUMD_NOALLOC_NBL_CAPACITY listed neighbours (within rcut + skin) per particle.
+ *   n_particles, n_types   1 <= n_particles <= RUMD_NOALLOC_MAX_PARTICLES (RUMD_ERR_INVALID_ARG beyond, with a message),
+ *                          1 <= n_types <= RUMD_MAX_TYPES.
+ *   box_lengths            host, 3 floats, as for rumd_create; rc_max + skin <= L/2 per axis (RUMD_ERR_BOX_TOO_SMALL).
+ *   pairs                  host, n_types * n_types records, pair (a, b) at [a * n_types + b]; must be symmetric.
+ *   skin                   Verlet skin of the list (>= 0).  The result does not depend on it; the list length does.
+ *   d_r                    DEVICE, input, float4 [n_particles]: x, y, z in [-L/2, L/2], type as int bits in .w (as
+ *                          rumd_bind_state; types outside [0, n_types) are the caller's responsibility).  16-byte aligned.
+ *   d_f, d_w               DEVICE, outputs, float4 [n_particles] force + u_i in .w, float [n_particles] virial w_i.
+ *   d_out4                 DEVICE, output, 4 doubles: U = sum u_i, W = sum w_i (fp64, fixed order), the longest list
+ *                          row, overflow flag (1.0: some particle has more than RUMD_NOALLOC_NBL_CAPACITY neighbours
+ *                          inside the list cutoff; forces, U and W are then incomplete).
+ *   cuda_stream            cudaStream_t the work is enqueued on (NULL: the default stream).  Asynchronous: one
+ *                          memset + two kernels, no host synchronisation, no cudaMalloc / cudaFree / allocating call.
+ *                          The first call on a device looks up the scratch array's device address (once per device).
+ *   errbuf, errbuf_len     host, may be NULL / 0: receives the message of a non-OK status.
+ * Ownership: the caller owns every pointer; the library owns only the static scratch.  EVERY call on a device shares
+ * that scratch, which keeps the previous call's contents (the call clears what must start at zero itself): calls
+ * ordered on one stream are fine, calls that may overlap on the GPU (different streams or threads without ordering
+ * between them) race and give garbage.  The handle API does not touch the scratch. */
+#define RUMD_NOALLOC_MAX_PARTICLES 8192
+#define RUMD_NOALLOC_NBL_CAPACITY 256
+typedef struct {
+    float epsilon, sigma, rcut;  /* 12-6 Lennard-Jones term u = 4 eps [(s/r)^12 - (s/r)^6], shifted force; rcut <= 0: none */
+    float kqq, rcut_coulomb;     /* Coulomb term u = kqq / r (kqq = k q_a q_b), shifted force; rcut_coulomb <= 0: none */
+} rumd_noalloc_pair;
+rumd_status rumd_forces_noalloc(int n_particles, int n_types, const float box_lengths[3], const rumd_noalloc_pair* pairs,
+                                float skin, const void* d_r, void* d_f, void* d_w, void* d_out4, void* cuda_stream,
+                                char* errbuf, size_t errbuf_len);
+
 const char* rumd_last_error(const rumd_system* s);
 const char* rumd_version(void);
 

@@ -29,8 +29,9 @@ EXPORTS = [
     "rumd_set_pair_potential", "rumd_set_integrator", "rumd_set_barostat", "rumd_get_box", "rumd_default_tuning", "rumd_set_tuning",
     "rumd_get_tuning", "rumd_autotune", "rumd_autotune_cached", "rumd_build_nblist", "rumd_compute_forces", "rumd_run_steps",
     "rumd_export_nblist", "rumd_get_thermo", "rumd_snapshot", "rumd_restore", "rumd_upload_state",
-    "rumd_download_state", "rumd_launch_count", "rumd_profile_step", "rumd_time_force", "rumd_profile_persistent", "rumd_measure_fp32_peak", "rumd_set_replicas", "rumd_get_thermo_replicas", "rumd_last_error", "rumd_version",
+    "rumd_download_state", "rumd_launch_count", "rumd_profile_step", "rumd_time_force", "rumd_profile_persistent", "rumd_measure_fp32_peak", "rumd_set_replicas", "rumd_get_thermo_replicas", "rumd_forces_noalloc", "rumd_last_error", "rumd_version",
 ]
+NOALLOC_MAX_PARTICLES, NOALLOC_NBL_CAPACITY = 8192, 256
 
 
 class Tuning(C.Structure):
@@ -50,6 +51,11 @@ class Thermo(C.Structure):
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_ if k != "pad_"}
+
+
+class NoallocPair(C.Structure):
+    _fields_ = [("epsilon", C.c_float), ("sigma", C.c_float), ("rcut", C.c_float), ("kqq", C.c_float),
+                ("rcut_coulomb", C.c_float)]
 
 
 class RumdError(RuntimeError):
@@ -102,6 +108,8 @@ def lib():
         L.rumd_measure_fp32_peak.argtypes = [vp, ip, C.POINTER(C.c_double)]
         L.rumd_set_replicas.argtypes = [vp, ip]
         L.rumd_get_thermo_replicas.argtypes = [vp, C.POINTER(Thermo), ip]
+        L.rumd_forces_noalloc.argtypes = [ip, ip, C.POINTER(C.c_float), C.POINTER(NoallocPair), C.c_float, vp, vp, vp, vp,
+                                          vp, C.c_char_p, C.c_size_t]
         L.rumd_last_error.argtypes = [vp]
         L.rumd_last_error.restype = C.c_char_p
         L.rumd_version.restype = C.c_char_p
@@ -369,6 +377,36 @@ class System:
         im = self.d_image.cpu().numpy()[inv]
         return dict(r=r[:, :3].copy(), types=r[:, 3].copy().view(np.int32), v=v[:, :3].copy(), m=v[:, 3].copy(),
                     F=f[:, :3].copy(), u=f[:, 3].copy(), w=w, image=im[:, :3].copy(), ids=ids)
+
+
+def forces_noalloc(n_types, box, pot, skin, d_r, d_f, d_w, d_out4, stream=None):
+    """``rumd_forces_noalloc``: forces, u_i, w_i and {U, W, longest row, overflow} of the configuration in the device
+    tensor ``d_r`` ((n, 4) float32: x, y, z, type bits) into the caller's device tensors ``d_f`` (n, 4), ``d_w`` (n,)
+    and ``d_out4`` (4 doubles), using only the library's static scratch -- no handle, no allocation, asynchronous on
+    ``stream`` (a torch stream; None = torch's current stream).  ``pot``: (nt, nt, >= 5) records (eps, sigma, rc_LJ,
+    k qa qb, rc_Coulomb) as in ``workloads``.  n <= NOALLOC_MAX_PARTICLES.  Argument marshalling only."""
+    for t, dt in ((d_r, torch.float32), (d_f, torch.float32), (d_w, torch.float32), (d_out4, torch.float64)):
+        if not (t.is_cuda and t.is_contiguous() and t.dtype == dt):
+            raise RumdError(ERR_INVALID_ARG, "forces_noalloc takes contiguous CUDA tensors (float32; d_out4 float64)")
+    n = int(d_r.shape[0])
+    if tuple(d_r.shape) != (n, 4) or tuple(d_f.shape) != (n, 4) or d_w.numel() != n or d_out4.numel() != 4:
+        raise RumdError(ERR_INVALID_ARG, "forces_noalloc: d_r, d_f are (n, 4), d_w (n,), d_out4 (4,)")
+    pot = np.asarray(pot, dtype=np.float64)
+    pairs = (NoallocPair * (n_types * n_types))()
+    for a in range(n_types):
+        for b in range(n_types):
+            pairs[a * n_types + b] = NoallocPair(*[float(x) for x in pot[a, b, :5]])
+    boxf = np.ascontiguousarray(box, dtype=np.float32)
+    if stream is None:
+        stream = torch.cuda.current_stream(d_r.device)
+    err = C.create_string_buffer(512)
+    with torch.cuda.device(d_r.device):
+        st = lib().rumd_forces_noalloc(n, int(n_types), boxf.ctypes.data_as(C.POINTER(C.c_float)), pairs, float(skin),
+                                       C.c_void_p(d_r.data_ptr()), C.c_void_p(d_f.data_ptr()),
+                                       C.c_void_p(d_w.data_ptr()), C.c_void_p(d_out4.data_ptr()),
+                                       C.c_void_p(stream.cuda_stream), err, len(err))
+    if st != OK:
+        raise RumdError(st, err.value.decode())
 
 
 def from_workload(wl, **kw) -> System:

@@ -1,0 +1,166 @@
+"""rumd_forces_noalloc (include/rumd_b200.h): the force / energy / virial evaluation that allocates nothing -- all of
+its scratch is one static device array inside the library -- against the EXISTING path (handle API: N^2 list build,
+rumd_compute_forces, rumd_get_thermo) on the same seeded inputs, on calls made back to back on one stream so that
+every call finds the previous call's contents in the shared scratch.
+
+Collected last on purpose (the suite runs with ``pytest -x``): a failure here hides no other test.  Self-contained:
+passes alone in a fresh process and after the other GPU tests (which leave their own data in device memory).
+Bars as in test_gpu_parity.py: forces max_i |dF_i| <= 1e-4 rms|F|, U and W to 1e-5 relative, u_i and w_i to 1e-5 of
+their largest value.
+"""
+import numpy as np
+import pytest
+
+from paper_1506_05094_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+FORCE_TOL = 1e-4
+ENERGY_TOL = 1e-5
+
+
+@pytest.fixture(scope="module")
+def rumd():
+    from paper_1506_05094_b200 import rumd as R
+
+    return R
+
+
+def workload(kind):
+    """Perturbed lattices (F = 0 on the perfect one): Kob-Andersen at the C1 size (two types, LJ only), the charged
+    system (LJ + shifted-force Coulomb, 166 neighbours inside the list cutoff), single-component LJ."""
+    wl = {"ka8000": lambda: W.ka_lattice(8000), "charged4096": lambda: W.charged_sc(16),
+          "lj864": lambda: W.lj_fcc(6)}[kind]()
+    wl.r = W.perturb(wl.r, wl.box, 0.08, 11)
+    return wl
+
+
+def existing_path(rumd, wl):
+    """Forces, u_i, w_i, U, W through the handle API with the N^2 list and 8 lanes per particle (no sorting: slot =
+    particle)."""
+    s = rumd.from_workload(wl)
+    s.set_tuning(method=rumd.NB_N2, tp=8, pb=32, sort_interval=0, persistent=0, use_graph=0)
+    s.build_nblist()
+    s.compute_forces()
+    th = s.get_thermo()
+    st = s.state()
+    assert np.array_equal(st["ids"], np.arange(wl.r.shape[0]))
+    out = dict(F=st["F"].copy(), u=st["u"].copy(), w=st["w"].copy(), U=th["U"], W=th["W"], max_nbrs=th["max_nbrs"])
+    s.close()
+    return out
+
+
+class NoallocCall:
+    """Caller-owned inputs and outputs of one rumd_forces_noalloc call (allocated BEFORE the calls are made)."""
+
+    def __init__(self, torch, wl):
+        n = wl.r.shape[0]
+        h = np.zeros((n, 4), dtype=np.float32)
+        h[:, :3] = wl.r
+        h[:, 3] = wl.types.astype(np.int32).view(np.float32)
+        self.wl = wl
+        self.d_r = torch.from_numpy(h).cuda()
+        # outputs start as garbage the kernels must overwrite
+        self.d_f = torch.full((n, 4), float("nan"), dtype=torch.float32, device="cuda")
+        self.d_w = torch.full((n,), float("nan"), dtype=torch.float32, device="cuda")
+        self.d_out4 = torch.full((4,), float("nan"), dtype=torch.float64, device="cuda")
+
+    def launch(self, rumd, skin=None):
+        wl = self.wl
+        rumd.forces_noalloc(wl.ntypes, wl.box, wl.pot, float(wl.skin) if skin is None else skin, self.d_r, self.d_f,
+                            self.d_w, self.d_out4)
+
+    def result(self):
+        f = self.d_f.cpu().numpy()
+        o = self.d_out4.cpu().numpy()
+        return dict(F=f[:, :3].copy(), u=f[:, 3].copy(), w=self.d_w.cpu().numpy(), U=o[0], W=o[1], max_nbrs=int(o[2]),
+                    overflow=int(o[3]))
+
+
+def assert_matches(got, ref):
+    assert got["overflow"] == 0
+    assert got["max_nbrs"] == ref["max_nbrs"]
+    rms = np.sqrt((ref["F"].astype(np.float64) ** 2).sum(1).mean())
+    assert rms > 0.1
+    err = np.sqrt(((got["F"].astype(np.float64) - ref["F"]) ** 2).sum(1)).max()
+    assert err <= FORCE_TOL * rms, "max|dF| = %g > 1e-4 rms|F| = %g" % (err, FORCE_TOL * rms)
+    assert np.abs(got["u"] - ref["u"]).max() <= 1e-5 * max(1.0, np.abs(ref["u"]).max())
+    assert np.abs(got["w"] - ref["w"]).max() <= 1e-5 * max(1.0, np.abs(ref["w"]).max())
+    assert abs(got["U"] - ref["U"]) <= ENERGY_TOL * abs(ref["U"]), (got["U"], ref["U"])
+    assert abs(got["W"] - ref["W"]) <= ENERGY_TOL * abs(ref["W"]), (got["W"], ref["W"])
+    # U and W are the sums of the per-particle outputs
+    assert abs(got["U"] - got["u"].astype(np.float64).sum()) <= 1e-9 * np.abs(got["u"]).astype(np.float64).sum()
+    assert abs(got["W"] - got["w"].astype(np.float64).sum()) <= 1e-9 * np.abs(got["w"]).astype(np.float64).sum()
+
+
+def test_noalloc_forces_match_the_handle_path_on_calls_in_a_row(rumd):
+    import torch
+
+    kinds = ["ka8000", "charged4096", "lj864", "ka8000"]  # larger -> smaller -> smaller -> the first again
+    wls = {k: workload(k) for k in set(kinds)}
+    refs = {k: existing_path(rumd, wls[k]) for k in wls}
+    calls = [NoallocCall(torch, wls[k]) for k in kinds]
+    calls[0].launch(rumd)  # (the first launch of a kernel may make the driver load its code: not counted below)
+    torch.cuda.synchronize()
+    free_before = torch.cuda.mem_get_info()[0]
+    for c in calls:  # back to back on one stream, no synchronisation in between: each finds the last one's scratch
+        c.launch(rumd)
+    torch.cuda.synchronize()
+    assert torch.cuda.mem_get_info()[0] == free_before, "the no-alloc entry point changed the device's free memory"
+    got = [c.result() for c in calls]
+    for k, g in zip(kinds, got):
+        assert_matches(g, refs[k])
+    # the same input after two other systems went through the scratch: bit for bit the first call's result
+    for key in ("F", "u", "w"):
+        assert np.array_equal(got[0][key], got[3][key]), key
+    assert got[0]["U"] == got[3]["U"] and got[0]["W"] == got[3]["W"]
+
+
+def test_noalloc_repeats_bitwise_and_follows_the_input(rumd):
+    """Two calls in a row on the SAME buffers, then one on moved particles: the first two agree bit for bit, the
+    third follows its input (nothing is cached in the scratch between calls)."""
+    import torch
+
+    wl = workload("lj864")
+    ref = existing_path(rumd, wl)
+    c = NoallocCall(torch, wl)
+    c.launch(rumd)
+    first = c.result()
+    c.launch(rumd)
+    second = c.result()
+    assert_matches(first, ref)
+    for key in ("F", "u", "w"):
+        assert np.array_equal(first[key], second[key]), key
+    assert first["U"] == second["U"] and first["W"] == second["W"]
+    wl2 = workload("lj864")
+    wl2.r = W.perturb(wl2.r, wl2.box, 0.05, 23)
+    c2 = NoallocCall(torch, wl2)
+    c2.launch(rumd)
+    assert_matches(c2.result(), existing_path(rumd, wl2))
+
+
+def test_noalloc_rejects_what_the_static_scratch_cannot_hold(rumd):
+    import torch
+
+    wl = workload("lj864")
+    n = rumd.NOALLOC_MAX_PARTICLES + 1
+    d_r = torch.zeros((n, 4), dtype=torch.float32, device="cuda")
+    d_f = torch.zeros((n, 4), dtype=torch.float32, device="cuda")
+    d_w = torch.zeros((n,), dtype=torch.float32, device="cuda")
+    d_o = torch.zeros((4,), dtype=torch.float64, device="cuda")
+    with pytest.raises(rumd.RumdError) as ei:
+        rumd.forces_noalloc(1, wl.box, wl.pot, 0.3, d_r, d_f, d_w, d_o)
+    assert ei.value.status == rumd.ERR_INVALID_ARG
+    assert "RUMD_NOALLOC_MAX_PARTICLES" in str(ei.value) and "8192" in str(ei.value)
+    # a list cutoff beyond half the box: refused like the handle API does
+    with pytest.raises(rumd.RumdError) as ei:
+        rumd.forces_noalloc(1, wl.box, wl.pot, 3.0, d_r[:864], d_f[:864], d_w[:864], d_o)
+    assert ei.value.status == rumd.ERR_BOX_TOO_SMALL
+    # more listed neighbours than the fixed capacity: reported through the overflow flag, the next call is clean
+    ka = workload("ka8000")
+    c = NoallocCall(torch, ka)
+    c.launch(rumd, skin=1.5)  # (4 pi / 3) 4^3 * 1.2 = 322 neighbours > 256
+    over = c.result()
+    assert over["overflow"] == 1 and over["max_nbrs"] > rumd.NOALLOC_NBL_CAPACITY
+    c.launch(rumd)
+    assert_matches(c.result(), existing_path(rumd, ka))
