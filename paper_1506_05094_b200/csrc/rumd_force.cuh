@@ -139,7 +139,12 @@ template <bool NC> __device__ __forceinline__ int load_idx(const int* p) { retur
 template <bool NC> __device__ __forceinline__ float4 load_pos(const float4* p) { return NC ? __ldg(p) : *p; }
 
 // PRE: the index loads of iteration 0 were issued by the caller before it knew the row length (jpre)
-template <int TP, int COUL, bool ONE_TYPE, int UNROLL, bool NC, bool ENERGY, bool WRAP, bool MASKED, bool PRE = false>
+// TWO: the system has exactly two particle types and COUL < 2 (Kob-Andersen, the charged mixture): the two parameter
+// records a lane can need -- (type of i, 0) and (type of i, 1) -- sit in registers and each pair SELECTS between them by
+// its neighbour's type.  The table lookup it replaces costs one LDS.128 per record and pair, i.e. four cycles of the
+// SM's load/store data path each, as many as the position gather itself needs at best (ncu: that path, not FP32
+// issue, bounds the kernel); a select is one ALU instruction per register.
+template <int TP, int COUL, bool ONE_TYPE, int UNROLL, bool NC, bool ENERGY, bool WRAP, bool MASKED, bool PRE = false, bool TWO = false>
 __device__ __forceinline__ void force_loop(const Sys& S, const float4* r, const float4* s_pp, const int* base,
                                            int it_begin, int nit, int it_end, const float4 ri, float& fx, float& fy,
                                            float& fz, float& u, float& w, const int* jpre = nullptr)
@@ -152,6 +157,20 @@ __device__ __forceinline__ void force_loop(const Sys& S, const float4* r, const 
         if (COUL) pc = s_pp[1];
         if (ENERGY) pe = s_pp[2];
         if (COUL == 2) px = s_pp[3];
+    }
+    float4 pf0, pc0, pe0, pf1, pc1, pe1; // TWO: records of (type of i, 0) and (type of i, 1)
+    pf0 = pc0 = pe0 = pf1 = pc1 = pe1 = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (TWO) {
+        pf0 = s_pp[trow];
+        pf1 = s_pp[trow + 4];
+        if (COUL) {
+            pc0 = s_pp[trow + 1];
+            pc1 = s_pp[trow + 5];
+        }
+        if (ENERGY) {
+            pe0 = s_pp[trow + 2];
+            pe1 = s_pp[trow + 6];
+        }
     }
     const float hx = S.h[0], hy = S.h[1], hz = S.h[2];
     const float ix = S.invL[0], iy = S.invL[1], iz = S.invL[2];
@@ -181,7 +200,12 @@ __device__ __forceinline__ void force_loop(const Sys& S, const float4* r, const 
                 dy = ri.y - rj[q].y;
                 dz = ri.z - rj[q].z;
             }
-            if (!ONE_TYPE) {
+            if (TWO) {
+                const bool b = type_of(rj[q]) != 0;
+                pf = make_float4(b ? pf1.x : pf0.x, b ? pf1.y : pf0.y, b ? pf1.z : pf0.z, b ? pf1.w : pf0.w);
+                if (COUL) pc = make_float4(b ? pc1.x : pc0.x, b ? pc1.y : pc0.y, b ? pc1.z : pc0.z, 0.f);
+                if (ENERGY) pe = make_float4(b ? pe1.x : pe0.x, b ? pe1.y : pe0.y, b ? pe1.z : pe0.z, b ? pe1.w : pe0.w);
+            } else if (!ONE_TYPE) {
                 const int o = trow + 4 * type_of(rj[q]);
                 pf = s_pp[o];
                 if (COUL) pc = s_pp[o + 1];
@@ -216,7 +240,17 @@ __device__ __forceinline__ void force_group(const Sys& S, const float4* r, const
     // iterations every lane of the warp has (no masks needed), then the ragged tail
     const int nit_all = __reduce_min_sync(FULLMASK, have_i ? nit : 0) / UNROLL * UNROLL;
     const bool interior = fabsf(ri.x) < S.hin[0] && fabsf(ri.y) < S.hin[1] && fabsf(ri.z) < S.hin[2];
-    if (__any_sync(FULLMASK, have_i && !interior)) {
+    const bool wrap = __any_sync(FULLMASK, have_i && !interior);
+    constexpr bool CAN2 = !ONE_TYPE && COUL < 2; // two-type systems: parameter records in registers (force_loop, TWO)
+    if (CAN2 && S.ntypes == 2) {
+        if (wrap) {
+            force_loop<TP, COUL, ONE_TYPE, UNROLL, NC, ENERGY, true, false, PRE, CAN2>(S, r, s_pp, base, 0, nit, nit_all, ri, fx, fy, fz, u, w, jpre);
+            force_loop<TP, COUL, ONE_TYPE, UNROLL, NC, ENERGY, true, true, PRE, CAN2>(S, r, s_pp, base, nit_all, nit, nit_w, ri, fx, fy, fz, u, w, jpre);
+        } else {
+            force_loop<TP, COUL, ONE_TYPE, UNROLL, NC, ENERGY, false, false, PRE, CAN2>(S, r, s_pp, base, 0, nit, nit_all, ri, fx, fy, fz, u, w, jpre);
+            force_loop<TP, COUL, ONE_TYPE, UNROLL, NC, ENERGY, false, true, PRE, CAN2>(S, r, s_pp, base, nit_all, nit, nit_w, ri, fx, fy, fz, u, w, jpre);
+        }
+    } else if (wrap) {
         force_loop<TP, COUL, ONE_TYPE, UNROLL, NC, ENERGY, true, false, PRE>(S, r, s_pp, base, 0, nit, nit_all, ri, fx, fy, fz, u, w, jpre);
         force_loop<TP, COUL, ONE_TYPE, UNROLL, NC, ENERGY, true, true, PRE>(S, r, s_pp, base, nit_all, nit, nit_w, ri, fx, fy, fz, u, w, jpre);
     } else {
