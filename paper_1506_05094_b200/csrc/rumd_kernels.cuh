@@ -427,9 +427,14 @@ __device__ __forceinline__ void ph_permute_store(const Sys& S, float4* r, int fi
 // (two when the row wraps around the box in x).  The group walks its ranges in lock step and hands out list
 // slots by ballot + popc, so rows of the list come out in the fixed order (round, position in range, lane)
 // and the list is bitwise reproducible.  `first`/`stride` index the virtual grid of N*G threads.
+// queue != nullptr: the warps take their units of 32 virtual threads from this device counter (which holds the number
+// of warps of the grid when the phase starts) instead of the fixed stride.  A warp next to a face of the box walks the general stencil path for all its
+// lanes, about twice the work of an interior one, and with ~9 units per warp at N = 10^6 the slowest warp of a fixed
+// assignment finished 30 % after the average one (the others waited at the grid barrier).  The list does not depend
+// on who builds a row.
 template <int G>
 __device__ __forceinline__ void ph_build_cell(const Sys& S, const float4* r, const float* s_rcl2, int first,
-                                              int stride, int* max_slot)
+                                              int stride, int* max_slot, int* queue = nullptr)
 {
     const int lane = threadIdx.x & 31;
     const int l = lane & (G - 1);
@@ -437,7 +442,16 @@ __device__ __forceinline__ void ph_build_cell(const Sys& S, const float4* r, con
     const unsigned lt = gmask & ((1u << lane) - 1u);
     const int nx = S.grid.n[0], ny = S.grid.n[1], nz = S.grid.n[2];
     const long long total = (long long)S.N * G;
-    for (long long vt = first; vt - lane < total; vt += stride) {
+    // dynamic assignment: the unit this warp works on next.  The first one is the warp's own index (the counter starts
+    // at the number of warps: no burst of same-address atomics when the phase begins); the request for the one after is
+    // in flight while the current one is worked on.
+    int unit = first >> 5;
+    for (long long vt = first;; vt += stride) {
+        if (queue) {
+            vt = (long long)unit * 32 + lane;
+            if (vt - lane < total && lane == 0) unit = atomicAdd(queue, 1);
+        }
+        if (vt - lane >= total) break;
         const int i = (int)(vt / G);
         const bool have_i = i < S.N;
         float4 ri = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -564,19 +578,20 @@ __device__ __forceinline__ void ph_build_cell(const Sys& S, const float4* r, con
         }
         const int wmax = __reduce_max_sync(FULLMASK, count); // one atomic per warp, not per particle
         if (lane == 0) atomicMax(max_slot, wmax);
+        if (queue) unit = __shfl_sync(FULLMASK, unit, 0);
     }
 }
 
 __device__ __forceinline__ void build_cell_dispatch(const Sys& S, const float4* r, const float* s_rcl2, int first,
-                                                    int stride, int* max_slot)
+                                                    int stride, int* max_slot, int* queue = nullptr)
 {
     switch (S.build_tp_shift) {
-    case 0: ph_build_cell<1>(S, r, s_rcl2, first, stride, max_slot); break;
-    case 1: ph_build_cell<2>(S, r, s_rcl2, first, stride, max_slot); break;
-    case 2: ph_build_cell<4>(S, r, s_rcl2, first, stride, max_slot); break;
-    case 3: ph_build_cell<8>(S, r, s_rcl2, first, stride, max_slot); break;
-    case 4: ph_build_cell<16>(S, r, s_rcl2, first, stride, max_slot); break;
-    default: ph_build_cell<32>(S, r, s_rcl2, first, stride, max_slot); break;
+    case 0: ph_build_cell<1>(S, r, s_rcl2, first, stride, max_slot, queue); break;
+    case 1: ph_build_cell<2>(S, r, s_rcl2, first, stride, max_slot, queue); break;
+    case 2: ph_build_cell<4>(S, r, s_rcl2, first, stride, max_slot, queue); break;
+    case 3: ph_build_cell<8>(S, r, s_rcl2, first, stride, max_slot, queue); break;
+    case 4: ph_build_cell<16>(S, r, s_rcl2, first, stride, max_slot, queue); break;
+    default: ph_build_cell<32>(S, r, s_rcl2, first, stride, max_slot, queue); break;
     }
 }
 

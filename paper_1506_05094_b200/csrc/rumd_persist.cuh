@@ -148,7 +148,10 @@ __global__ void __launch_bounds__(PERSIST_THREADS, (TP == 8 && !TILE) ? 2 : PERS
         // ---------------------------------------------------------------- (rebuild if flag) A2 / A3 / A4
         if (flag && S.method != 2) { // (the "none" method keeps no list)
             int* max_slot = &sc->max_nbrs[n_rebuilds & 1];
-            if (blockIdx.x == 0 && threadIdx.x == 0) sc->max_nbrs[(n_rebuilds + 1) & 1] = 0;
+            if (blockIdx.x == 0 && threadIdx.x == 0) {
+                sc->max_nbrs[(n_rebuilds + 1) & 1] = 0;
+                sc->build_queue = stride >> 5; // units 0 .. warps-1 are taken (the cell build is at least one grid barrier away)
+            }
             const float4* rsrc = rc; // where the build reads the positions from
             if (sort_on_rebuild(S, n_rebuilds)) {
                 ph_cell_assign(S, rc, first, stride);
@@ -177,7 +180,11 @@ __global__ void __launch_bounds__(PERSIST_THREADS, (TP == 8 && !TILE) ? 2 : PERS
                 for (int t = blockIdx.x; t < S.ntiles; t += gridDim.x)
                     ph_build_tile(S, rsrc, t, s_pos, s_hstart, s_scratch, s_warp, s_rcl2, max_slot);
             } else if (S.method == 1)
-                build_cell_dispatch(S, rsrc, s_rcl2, first, stride, max_slot);
+            {
+                // several units per warp: hand them out dynamically (see ph_build_cell); else one fixed pass
+                const long long units = (((long long)S.N << S.build_tp_shift) + 31) >> 5;
+                build_cell_dispatch(S, rsrc, s_rcl2, first, stride, max_slot, units >= 4LL * (stride >> 5) ? &sc->build_queue : nullptr);
+            }
             else
                 ph_build_n2(S, rsrc, s_tile, s_rcl2, blockIdx.x, gridDim.x, max_slot);
             n_rebuilds += 1;

@@ -42,6 +42,8 @@ struct DevScalars {
     int max_nbrs[2];      // largest list length of build number b in slot b & 1
     int nonfinite;        // 1: NaN/Inf energy; 2: grid barrier timed out
     int last_max;         // largest list length of the last COMPLETED build (written when its force evaluation starts)
+    int build_queue;      // cell build inside the persistent kernel: next unit of 32 virtual threads (dynamic assignment)
+    int pad_queue_;
     // NPT (rumd_npt.cuh): the box is a device quantity that changes every step
     double box[3];        // current box lengths (set from the handle's box at every reset)
     double box_next[3];   // box after the step in flight (k_npt_prepare -> k_integrate_npt)
