@@ -1461,3 +1461,68 @@ def test_tile_method_ragged_gas_four_types_and_halo_overflow(rumd):
         s.get_thermo()
     assert e.value.status == rumd.ERR_NBL_OVERFLOW
     s.close()
+
+
+@pytest.mark.parametrize("kind,kw,tp", [("ka", dict(N=4096), 8), ("ka", dict(N=16384), 2), ("ch", dict(n=16), 4)])
+def test_two_type_register_select_equals_the_table_lookup_bitwise(rumd, kind, kw, tp):
+    """A5, two-type systems: force_loop keeps both parameter records of a lane in registers and selects per pair (TWO).
+    The same system declared with a THIRD, unused particle type goes through the generic shared-memory table instead;
+    the arithmetic is the same, so forces, energies, virials and a short NVE trajectory agree bit for bit -- through the
+    stand-alone force kernel, the persistent kernel and the per-step kernels."""
+    wl2 = perturbed(make(kind, **kw))
+    wl2.integrator = W.NVE
+    wl3 = perturbed(make(kind, **kw))
+    wl3.integrator = W.NVE
+    pot3 = W.pot_table(3)
+    pot3[:2, :2] = wl2.pot
+    W.set_lj(pot3, 0, 2, 1.0, 1.0, 2.0)   # a type nobody has; cutoffs below rc_max, so the cell grid is the same
+    W.set_lj(pot3, 1, 2, 1.0, 1.0, 2.0)
+    W.set_lj(pot3, 2, 2, 1.0, 1.0, 2.0)
+    wl3.pot = pot3
+    assert wl3.ntypes == 3 and wl2.ntypes == 2 and wl3.rc_max() == wl2.rc_max()
+    for persistent in (1, 0):
+        res = []
+        for wl in (wl2, wl3):
+            s = rumd.from_workload(wl)
+            s.set_tuning(method=rumd.NB_CELL, tp=tp, pb=256 // tp, persistent=persistent, use_graph=0)
+            s.compute_forces()
+            st0 = s.state()
+            s.run_steps(25)
+            res.append((st0, s.state(), s.get_thermo()))
+            s.close()
+        (a0, a1, ta), (b0, b1, tb) = res
+        for key in ("F", "u", "w"):
+            assert np.array_equal(a0[key], b0[key]), key
+        for key in ("r", "v", "F", "u", "w", "image"):
+            assert np.array_equal(a1[key], b1[key]), (key, persistent)
+        assert ta["U"] == tb["U"] and ta["W"] == tb["W"] and ta["n_rebuilds"] == tb["n_rebuilds"]
+    # and the two-type path against the oracle, on the same state
+    s = rumd.from_workload(wl2)
+    s.set_tuning(method=rumd.NB_CELL, tp=tp, pb=256 // tp)
+    s.compute_forces()
+    check_forces(s, wl2.r.astype(np.float64), wl2.types, wl2.box.astype(np.float64), wl2.pot, cancelling=kind == "ka")
+    s.close()
+
+
+@pytest.mark.parametrize("kind,kw,tp,build_tp", [("ka", dict(N=131072), 2, 4), ("lj", dict(ncell=64), 1, 1)])
+def test_list_built_inside_the_persistent_kernel_from_the_unit_queue(rumd, kind, kw, tp, build_tp):
+    """A4 inside A7 at sizes where a warp has several units to build: k_persist hands them out from a device counter
+    (DevScalars::build_queue).  The list the first step builds -- at the initial positions, after the spatial sort --
+    is compared with the oracle's as a set, ALL rows (1e-6 band), and the forces of that step's evaluation with it."""
+    wl = perturbed(make(kind, **kw))
+    wl.integrator = W.NVE
+    s = rumd.from_workload(wl)
+    s.set_tuning(method=rumd.NB_CELL, tp=tp, pb=256 // tp, build_tp=build_tp, persistent=1)
+    s.run_steps(1)
+    th = s.get_thermo()
+    assert th["n_rebuilds"] == 1 and th["overflow"] == 0
+    r64 = wl.r.astype(np.float64)
+    box = wl.box.astype(np.float64)
+    gcnt, npairs, nband = check_nblist_rows(s, r64, wl.types, box, wl.pot, float(wl.skin))
+    assert int(gcnt.sum()) in range(npairs - nband, npairs + nband + 1) and th["max_nbrs"] == gcnt.max()
+    # forces of the step's (only) force evaluation belong to the initial positions too
+    st = s.state()
+    F, u, w = oracle.forces_list(r64, wl.types, box, wl.pot, *oracle.nblist(r64, wl.types, box, wl.pot, 0.0, method="cell"))
+    rms = np.sqrt((F * F).sum(1).mean())
+    assert np.sqrt(((st["F"].astype(np.float64) - F) ** 2).sum(1)).max() <= FORCE_TOL * rms
+    s.close()
