@@ -150,8 +150,9 @@ def whole_job_rate(units_per_rank: float, seconds_local: float, world: int, devi
 # ncu --set full captures of the dominant kernels (dram__bytes_read.sum + dram__bytes_write.sum per launch) live
 # under profiles/ and are named here; `roofline.traffic` carries a number only when bench.py is pointed at one that
 # was taken on the same workload and commit (it is a profiler measurement, never re-measured inside a timed run).
-TRAFFIC_PROFILES = {"ka8000": "profiles/r02_persist_c1_ncu.md", "lj1m": "profiles/r02_force_lj1m_ncu.md",
-                    "ka65536": "profiles/r02_force_ka65536_ncu.md"}
+TRAFFIC_PROFILES = {"ka8000": "profiles/r02_persist_c1_ncu.md", "lj1m": "profiles/r02_persist_lj1m_ncu.md",
+                    "ka65536": "profiles/r02_ka65536_ncu.md", "ka1000": "profiles/r02_persist_ka1000_ncu.md",
+                    "charged": "profiles/r02_charged_ncu.md"}
 
 # The paper's parameter file (P:382 step 8): tunings found by rumd_autotune on "NVIDIA B200", keyed by GPU name, N,
 # box, potentials, integrator; a hit costs no trial run, a miss tunes and appends.

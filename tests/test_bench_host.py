@@ -93,3 +93,15 @@ def test_bench_refuses_to_run_without_a_gpu():
     r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--steps", "1"], capture_output=True, text=True,
                        timeout=300)
     assert r.returncode != 0 and "no CPU fallback" in (r.stderr + r.stdout)
+
+
+def test_traffic_profiles_named_by_bench_exist_and_name_their_command():
+    """`roofline.traffic` is null with a pointer to an ncu capture under profiles/ (`traffic_source`): every file
+    bench.py can point at is committed and states the command that made it."""
+    import bench
+
+    for name, rel in bench.TRAFFIC_PROFILES.items():
+        path = os.path.join(ROOT, rel)
+        assert os.path.exists(path), (name, rel)
+        txt = open(path).read()
+        assert "ncu --set full" in txt and "bench.py" in txt and "dram__bytes_read.sum" in txt, rel
