@@ -345,20 +345,48 @@ def test_c1_nvt_conserved_quantity_drift(rumd):
 
 
 def test_c3_nve_energy_drift(rumd):
-    """S26 on configs[3] (N = 1 048 576, cell build + re-sorting in flight): 1000 NVE steps, slope of E/N scaled
-    to 1e4 steps <= 1e-4 per particle."""
+    """S26 on configs[3] (N = 1 048 576, cell build + re-sorting in flight, the unit queue of the build): the FULL 1e4
+    NVE steps of the north_star bar, slope of E/N times the run length <= 1e-4 per particle."""
     wl = make("lj", ncell=64)
     s = rumd.from_workload(wl)
     s.run_steps(200)                # melt off the lattice
     E = []
-    for _ in range(10):
+    for _ in range(100):
         s.run_steps(100)
         th = s.get_thermo()
         E.append((th["K"] + th["U"]) / wl.N)
     E = np.array(E)
     slope = np.polyfit(np.arange(E.size) * 100.0, E, 1)[0]
     assert abs(slope * 1e4) <= 1e-4, "drift %g per particle per 1e4 steps" % (slope * 1e4)
-    assert s.get_thermo()["n_rebuilds"] >= 20
+    assert np.abs(E - E[0]).max() < 5e-3
+    assert s.get_thermo()["n_rebuilds"] >= 500
+    s.close()
+
+
+@pytest.mark.parametrize("kind,kw,tuning", [
+    ("ch", dict(n=32), dict(method=1, tp=2, pb=128, build_tp=2, skin=0.345)),       # configs[4] with its bench tuning
+    ("ka", dict(N=131072), dict(method=1, tp=2, pb=128, build_tp=4, skin=0.30)),    # largest configs[2] entry
+    ("ka", dict(N=8000), dict(method=1, tp=8, pb=32, build_tp=8, skin=0.397)),      # configs[1] run as NVE
+])
+def test_nve_energy_drift_at_the_other_bench_sizes(rumd, kind, kw, tuning):
+    """S26 / north_star drift bar at the remaining bench sizes, run as NVE (two particle types: the register-select
+    force loop; C4: the Coulomb term): 1e4 steps after 2000 steps of equilibration under the workload's thermostat,
+    slope of E/N times the run length <= 1e-4 per particle."""
+    wl = make(kind, **kw)
+    s = rumd.from_workload(wl)
+    s.set_tuning(**tuning)
+    s.run_steps(2000)               # off the lattice and to temperature (NVT)
+    s.set_integrator(W.NVE, wl.dt, wl.T0, wl.tau)
+    s.run_steps(100)
+    E = []
+    for _ in range(100):
+        s.run_steps(100)
+        th = s.get_thermo()
+        E.append((th["K"] + th["U"]) / wl.N)
+    E = np.array(E)
+    slope = np.polyfit(np.arange(E.size) * 100.0, E, 1)[0]
+    assert abs(slope * 1e4) <= 1e-4, "drift %g per particle per 1e4 steps" % (slope * 1e4)
+    assert np.abs(E - E[0]).max() < 5e-3
     s.close()
 
 
