@@ -82,3 +82,26 @@ def test_binding_constants_match_the_header_enums():
     body = re.sub(r"/\*.*?\*/", "", body, flags=re.S)
     fields = [m.group(1) for m in re.finditer(r"\b(?:int|float)\s+(\w+)\s*;", body)]
     assert fields == [f[0] for f in rumd.Tuning._fields_]
+
+
+def test_noalloc_entry_point_rejects_oversize_before_touching_the_device(libpath):
+    """rumd_forces_noalloc validates its sizes on the host first: beyond RUMD_NOALLOC_MAX_PARTICLES it returns
+    RUMD_ERR_INVALID_ARG with a message that names the limit -- with or without a GPU (no compute call is made)."""
+    from paper_1506_05094_b200 import rumd
+
+    src = open(HEADER).read()
+    limit = int(re.search(r"#define\s+RUMD_NOALLOC_MAX_PARTICLES\s+(\d+)", src).group(1))
+    cap = int(re.search(r"#define\s+RUMD_NOALLOC_NBL_CAPACITY\s+(\d+)", src).group(1))
+    assert (limit, cap) == (rumd.NOALLOC_MAX_PARTICLES, rumd.NOALLOC_NBL_CAPACITY)
+    L = rumd.lib()
+    box = (C.c_float * 3)(20, 20, 20)
+    pair = (rumd.NoallocPair * 1)(rumd.NoallocPair(1.0, 1.0, 2.5, 0.0, 0.0))
+    err = C.create_string_buffer(256)
+    fake = C.c_void_p(256)  # never dereferenced: the size check comes first
+    st = L.rumd_forces_noalloc(limit + 1, 1, box, pair, 0.3, fake, fake, fake, fake, None, err, len(err))
+    assert st == rumd.ERR_INVALID_ARG
+    assert b"RUMD_NOALLOC_MAX_PARTICLES" in err.value and str(limit).encode() in err.value
+    st = L.rumd_forces_noalloc(0, 1, box, pair, 0.3, fake, fake, fake, fake, None, err, len(err))
+    assert st == rumd.ERR_INVALID_ARG and err.value
+    st = L.rumd_forces_noalloc(100, 5, box, pair, 0.3, fake, fake, fake, fake, None, err, len(err))
+    assert st == rumd.ERR_INVALID_ARG and b"n_types" in err.value
