@@ -76,6 +76,14 @@ __device__ __forceinline__ bool barrier_arrive_wait(unsigned long long* counters
         }                                                                                                \
     } while (0)
 
+// warp_sum over values that are zero except in every TP-th lane (lane 0 holds the total)
+template <int TP> __device__ __forceinline__ double warp_sum_strided(double x)
+{
+#pragma unroll
+    for (int o = 16; o >= TP; o >>= 1) x += __shfl_xor_sync(FULLMASK, x, o);
+    return x;
+}
+
 // Fixed-order sum over the per-block partials of one step by ONE warp; every lane returns the total.
 __device__ __forceinline__ double warp_sum_partials(const double* p, int n)
 {
@@ -298,8 +306,10 @@ __global__ void __launch_bounds__(PERSIST_THREADS, (TP == 8 && !TILE) ? 2 : PERS
 
         // ---------------------------------------------------------------- block sums, then the step's barrier
         {
-            const double wm = (nvt || last) ? warp_sum(mv2) : 0.0;
-            const double wk = last ? warp_sum(kt) : 0.0;
+            // (only the lanes with t == 0, every TP-th, hold a particle's contribution: the butterfly levels below TP
+            // would add zeros; leaving them out gives the same bits and takes them off the step's critical path)
+            const double wm = (nvt || last) ? warp_sum_strided<TP>(mv2) : 0.0;
+            const double wk = last ? warp_sum_strided<TP>(kt) : 0.0;
             const bool wmoved = __any_sync(FULLMASK, moved);
             if (lane == 0) {
                 s_redm[wid] = wm;
