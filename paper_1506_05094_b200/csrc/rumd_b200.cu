@@ -820,7 +820,16 @@ static rumd_status launch_persistent(rumd_system* s, int nsteps)
     const bool tile = s->tune.method == RUMD_NB_TILE;
     const void* fn = (tile ? kernels_of(s)->persist_tile : kernels_of(s)->persist)[coul_of(s)][one_of(s) ? 1 : 0];
     if (!fn) return fail(s, RUMD_ERR_INVALID_ARG, "the tile method takes tp <= 8");
-    const int threads = persist_threads_of(s->tune);
+    int threads = persist_threads_of(s->tune);
+    {   // blocks of 512 threads when blocks of 256 would need two per SM and 512 fit one per SM: half the
+        // barrier arrivals and thermostat partial sums for the same warps per SM
+        const void* wide = tile ? nullptr : kernels_of(s)->persist_wide[coul_of(s)][one_of(s) ? 1 : 0];
+        const long long lanes = (long long)s->N * s->tune.tp;
+        if (wide && (lanes + threads - 1) / threads > s->num_sms && (lanes + 2 * threads - 1) / (2 * threads) <= s->num_sms) {
+            fn = wide;
+            threads *= 2;
+        }
+    }
     const size_t smem = tile ? tile_smem_bytes(s->S.hcap) : 0;
     const int sig = s->tune.tp * 4096 + threads + (s->any_coul ? 1 << 20 : 0) + (s->ntypes == 1 ? 1 << 21 : 0) +
                     (s->any_generic ? 1 << 22 : 0) + (tile ? 1 << 23 : 0);

@@ -74,6 +74,11 @@ template <int TP, int COUL, bool ONE> static const void* persist_tile_fn()
     else return nullptr;
 }
 
+template <int TP, int COUL, bool ONE> static const void* persist_wide_fn()
+{
+    return (const void*)&k_persist<TP, COUL, ONE, UnrollOf<TP>::value, false, 512>;
+}
+
 template <int TP> static const KernelSet* kernel_set()
 {
     static const KernelSet ks = {
@@ -83,6 +88,9 @@ template <int TP> static const KernelSet* kernel_set()
         {{persist_tile_fn<TP, 0, false>(), persist_tile_fn<TP, 0, true>()},
          {persist_tile_fn<TP, 1, false>(), persist_tile_fn<TP, 1, true>()},
          {persist_tile_fn<TP, 2, false>(), persist_tile_fn<TP, 2, true>()}},
+        {{persist_wide_fn<TP, 0, false>(), persist_wide_fn<TP, 0, true>()},
+         {persist_wide_fn<TP, 1, false>(), persist_wide_fn<TP, 1, true>()},
+         {persist_wide_fn<TP, 2, false>(), persist_wide_fn<TP, 2, true>()}},
         {{(const void*)&k_ensemble<TP, 0, false, UnrollOf<TP>::value>, (const void*)&k_ensemble<TP, 0, true, UnrollOf<TP>::value>},
          {(const void*)&k_ensemble<TP, 1, false, UnrollOf<TP>::value>, (const void*)&k_ensemble<TP, 1, true, UnrollOf<TP>::value>},
          {(const void*)&k_ensemble<TP, 2, false, UnrollOf<TP>::value>, (const void*)&k_ensemble<TP, 2, true, UnrollOf<TP>::value>}},
