@@ -828,6 +828,15 @@ static rumd_status launch_persistent(rumd_system* s, int nsteps)
         if (wide && (lanes + threads - 1) / threads > s->num_sms && (lanes + 2 * threads - 1) / (2 * threads) <= s->num_sms) {
             fn = wide;
             threads *= 2;
+        } else {
+            // more work than that (tp < 8, 80 registers): ONE block of 768 threads per SM instead of three of 256 -- a
+            // third of the barrier arrivals, and the 24 warps of an SM work on consecutive particles (N = 10^6: 246 ->
+            // 227 us per step, N = 131072: 50.7 -> 47.9)
+            const void* wide3 = tile ? nullptr : kernels_of(s)->persist_wide3[coul_of(s)][one_of(s) ? 1 : 0];
+            if (wide3 && (lanes + 2 * threads - 1) / (2 * threads) > s->num_sms) {
+                fn = wide3;
+                threads *= 3;
+            }
         }
     }
     const size_t smem = tile ? tile_smem_bytes(s->S.hcap) : 0;

@@ -13,6 +13,7 @@ struct KernelSet {
     const void* persist[3][2];  // k_persist<TP, coul, one, unroll, false>
     const void* persist_tile[3][2]; // k_persist<TP, coul, one, unroll, true> (tile method; null for tp > 8)
     const void* persist_wide[3][2]; // k_persist<TP, coul, one, unroll, false, 512>: blocks of 512 threads, one per SM
+    const void* persist_wide3[3][2]; // k_persist<TP, coul, one, unroll, false, 768>: blocks of 768 threads (tp < 8), one per SM
     const void* ensemble[3][2]; // k_ensemble<TP, coul, one>
     const void* force_fn[3][2]; // k_force<TP, coul, one, unroll>
     void (*force)(int coul, bool one, const Sys& S, int nblocks, int nthreads, cudaStream_t stream);

@@ -79,6 +79,12 @@ template <int TP, int COUL, bool ONE> static const void* persist_wide_fn()
     return (const void*)&k_persist<TP, COUL, ONE, UnrollOf<TP>::value, false, 512>;
 }
 
+template <int TP, int COUL, bool ONE> static const void* persist_wide3_fn()
+{
+    if constexpr (TP < 8) return (const void*)&k_persist<TP, COUL, ONE, UnrollOf<TP>::value, false, 768>;
+    else return nullptr;
+}
+
 template <int TP> static const KernelSet* kernel_set()
 {
     static const KernelSet ks = {
@@ -91,6 +97,9 @@ template <int TP> static const KernelSet* kernel_set()
         {{persist_wide_fn<TP, 0, false>(), persist_wide_fn<TP, 0, true>()},
          {persist_wide_fn<TP, 1, false>(), persist_wide_fn<TP, 1, true>()},
          {persist_wide_fn<TP, 2, false>(), persist_wide_fn<TP, 2, true>()}},
+        {{persist_wide3_fn<TP, 0, false>(), persist_wide3_fn<TP, 0, true>()},
+         {persist_wide3_fn<TP, 1, false>(), persist_wide3_fn<TP, 1, true>()},
+         {persist_wide3_fn<TP, 2, false>(), persist_wide3_fn<TP, 2, true>()}},
         {{(const void*)&k_ensemble<TP, 0, false, UnrollOf<TP>::value>, (const void*)&k_ensemble<TP, 0, true, UnrollOf<TP>::value>},
          {(const void*)&k_ensemble<TP, 1, false, UnrollOf<TP>::value>, (const void*)&k_ensemble<TP, 1, true, UnrollOf<TP>::value>},
          {(const void*)&k_ensemble<TP, 2, false, UnrollOf<TP>::value>, (const void*)&k_ensemble<TP, 2, true, UnrollOf<TP>::value>}},

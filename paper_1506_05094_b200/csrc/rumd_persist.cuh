@@ -95,7 +95,8 @@ __device__ __forceinline__ double warp_sum_partials(const double* p, int n)
 // TILE: the instantiation for the tile method (RUMD_NB_TILE: halo in dynamic shared memory); the other methods share
 // the TILE = false instantiation, whose register budget the tile code must not touch.
 // NT: threads per block.  512 (one block per SM, up to 128 registers) is launched when blocks of 256 would need two per
-// SM and 512 fit one: half the barrier arrivals and thermostat partials for the same 16 warps per SM (C1 7.75 -> 7.5 us).
+// SM and 512 fit one: half the barrier arrivals and thermostat partials for the same 16 warps per SM (C1 7.75 -> 7.5 us);
+// 768 (tp < 8, 85 registers) instead of three blocks of 256 per SM at large N.
 template <int TP, int COUL, bool ONE_TYPE, int UNROLL, bool TILE, int NT = PERSIST_THREADS>
 __global__ void __launch_bounds__(NT, NT > PERSIST_THREADS ? 1 : (TP == 8 && !TILE) ? 2 : PERSIST_MINB) k_persist(const Sys S, const int nsteps, const int nvt)
 {
