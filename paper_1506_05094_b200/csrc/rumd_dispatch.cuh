@@ -12,8 +12,8 @@ template <int TP> struct UnrollOf { static constexpr int value = TP >= 16 ? 4 : 
 struct KernelSet {
     const void* persist[3][2];  // k_persist<TP, coul, one, unroll, false>
     const void* persist_tile[3][2]; // k_persist<TP, coul, one, unroll, true> (tile method; null for tp > 8)
-    const void* persist_wide[3][2]; // k_persist<TP, coul, one, unroll, false, 512>: blocks of 512 threads, one per SM
-    const void* persist_wide3[3][2]; // k_persist<TP, coul, one, unroll, false, 768>: blocks of 768 threads (tp < 8), one per SM
+    const void* persist_wide[3][2]; // k_persist<TP, coul, one, unroll, false, 512>: blocks of 512 threads, one per SM (null for coul = 2)
+    const void* persist_wide3[3][2]; // k_persist<TP, coul, one, unroll, false, 768>: blocks of 768 threads (tp < 8, coul < 2), one per SM
     const void* ensemble[3][2]; // k_ensemble<TP, coul, one>
     const void* force_fn[3][2]; // k_force<TP, coul, one, unroll>
     void (*force)(int coul, bool one, const Sys& S, int nblocks, int nthreads, cudaStream_t stream);

@@ -76,12 +76,14 @@ template <int TP, int COUL, bool ONE> static const void* persist_tile_fn()
 
 template <int TP, int COUL, bool ONE> static const void* persist_wide_fn()
 {
-    return (const void*)&k_persist<TP, COUL, ONE, UnrollOf<TP>::value, false, 512>;
+    // (not for the generic second-term kinds, COUL == 2: they keep blocks of 256 threads; a third less to compile)
+    if constexpr (COUL < 2) return (const void*)&k_persist<TP, COUL, ONE, UnrollOf<TP>::value, false, 512>;
+    else return nullptr;
 }
 
 template <int TP, int COUL, bool ONE> static const void* persist_wide3_fn()
 {
-    if constexpr (TP < 8) return (const void*)&k_persist<TP, COUL, ONE, UnrollOf<TP>::value, false, 768>;
+    if constexpr (TP < 8 && COUL < 2) return (const void*)&k_persist<TP, COUL, ONE, UnrollOf<TP>::value, false, 768>;
     else return nullptr;
 }
 
