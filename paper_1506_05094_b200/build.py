@@ -3,7 +3,7 @@
     python -m paper_1506_05094_b200.build [--force] [-v]
 
 The kernels templated on threads-per-particle live in one translation unit per tp (csrc/rumd_inst_tp*.cu); the
-eight translation units are compiled in parallel and linked into one shared library.
+fourteen translation units are compiled in parallel and linked into one shared library.
 """
 from __future__ import annotations
 
@@ -16,7 +16,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJDIR = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "librumd_b200.so")
-SOURCES = ["rumd_b200.cu", "rumd_noalloc.cu"] + ["rumd_inst_tp%d.cu" % tp for tp in (1, 2, 4, 8, 16, 32)]
+SOURCES = (["rumd_b200.cu", "rumd_noalloc.cu"] + ["rumd_inst_tp%d.cu" % tp for tp in (1, 2, 4, 8, 16, 32)] +
+           ["rumd_inst_wide_tp%d.cu" % tp for tp in (1, 2, 4, 8, 16, 32)])
 HEADERS = sorted(f for f in os.listdir(CSRC) if f.endswith(".cuh")) + ["../../include/rumd_b200.h"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC"]
 

@@ -22,6 +22,10 @@ struct KernelSet {
     cudaError_t (*force_tile)(int coul, bool one, const Sys& S, int nblocks, size_t smem, cudaStream_t stream);
 };
 
+// the two wider instantiations of k_persist (512 and 768 threads per block) are compiled in translation units of their
+// own (rumd_inst_wide_tp*.cu: twice the parallelism for the build); each defines this for its tp
+template <int TP> void rumd_fill_wide(const void* (*wide)[2], const void* (*wide3)[2]);
+
 const KernelSet* rumd_kernels_tp1();
 const KernelSet* rumd_kernels_tp2();
 const KernelSet* rumd_kernels_tp4();

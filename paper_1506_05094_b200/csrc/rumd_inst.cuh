@@ -74,34 +74,18 @@ template <int TP, int COUL, bool ONE> static const void* persist_tile_fn()
     else return nullptr;
 }
 
-template <int TP, int COUL, bool ONE> static const void* persist_wide_fn()
-{
-    // (not for the generic second-term kinds, COUL == 2: they keep blocks of 256 threads; a third less to compile)
-    if constexpr (COUL < 2) return (const void*)&k_persist<TP, COUL, ONE, UnrollOf<TP>::value, false, 512>;
-    else return nullptr;
-}
-
-template <int TP, int COUL, bool ONE> static const void* persist_wide3_fn()
-{
-    if constexpr (TP < 8 && COUL < 2) return (const void*)&k_persist<TP, COUL, ONE, UnrollOf<TP>::value, false, 768>;
-    else return nullptr;
-}
-
 template <int TP> static const KernelSet* kernel_set()
 {
-    static const KernelSet ks = {
+    static const KernelSet ks = [] {
+    KernelSet k = {
         {{(const void*)&k_persist<TP, 0, false, UnrollOf<TP>::value, false>, (const void*)&k_persist<TP, 0, true, UnrollOf<TP>::value, false>},
          {(const void*)&k_persist<TP, 1, false, UnrollOf<TP>::value, false>, (const void*)&k_persist<TP, 1, true, UnrollOf<TP>::value, false>},
          {(const void*)&k_persist<TP, 2, false, UnrollOf<TP>::value, false>, (const void*)&k_persist<TP, 2, true, UnrollOf<TP>::value, false>}},
         {{persist_tile_fn<TP, 0, false>(), persist_tile_fn<TP, 0, true>()},
          {persist_tile_fn<TP, 1, false>(), persist_tile_fn<TP, 1, true>()},
          {persist_tile_fn<TP, 2, false>(), persist_tile_fn<TP, 2, true>()}},
-        {{persist_wide_fn<TP, 0, false>(), persist_wide_fn<TP, 0, true>()},
-         {persist_wide_fn<TP, 1, false>(), persist_wide_fn<TP, 1, true>()},
-         {persist_wide_fn<TP, 2, false>(), persist_wide_fn<TP, 2, true>()}},
-        {{persist_wide3_fn<TP, 0, false>(), persist_wide3_fn<TP, 0, true>()},
-         {persist_wide3_fn<TP, 1, false>(), persist_wide3_fn<TP, 1, true>()},
-         {persist_wide3_fn<TP, 2, false>(), persist_wide3_fn<TP, 2, true>()}},
+        {{nullptr, nullptr}, {nullptr, nullptr}, {nullptr, nullptr}}, // persist_wide, persist_wide3: filled below
+        {{nullptr, nullptr}, {nullptr, nullptr}, {nullptr, nullptr}},
         {{(const void*)&k_ensemble<TP, 0, false, UnrollOf<TP>::value>, (const void*)&k_ensemble<TP, 0, true, UnrollOf<TP>::value>},
          {(const void*)&k_ensemble<TP, 1, false, UnrollOf<TP>::value>, (const void*)&k_ensemble<TP, 1, true, UnrollOf<TP>::value>},
          {(const void*)&k_ensemble<TP, 2, false, UnrollOf<TP>::value>, (const void*)&k_ensemble<TP, 2, true, UnrollOf<TP>::value>}},
@@ -112,5 +96,8 @@ template <int TP> static const KernelSet* kernel_set()
         &step_tp<TP>,
         &force_tile_tp<TP>,
     };
+    rumd_fill_wide<TP>(k.persist_wide, k.persist_wide3);
+    return k;
+    }();
     return &ks;
 }
